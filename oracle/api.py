@@ -1,0 +1,233 @@
+"""ctypes binding of the CPU oracle (TEST INFRASTRUCTURE ONLY -- see godunov_oracle.cpp).
+
+Only tests/, ``__graft_entry__.smoke()`` and ``bench.py``'s cpu_baseline / ``--impl reference``
+legs may import this module.  It never imports the CUDA package.
+
+Arrays are numpy, layout ``U[field, patch, k, j, i]`` WITH ghosts (M = n + 2g per side).
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+CNT_NAMES = ("positivity_fallback_cells", "hll_fallback_faces", "degenerate_D", "nonpositive_rho_after")
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.oracle_smax.restype = C.c_double
+        _lib.oracle_limited_slope.restype = C.c_double
+        _lib.oracle_limited_slope.argtypes = [C.c_double, C.c_double, C.c_int]
+    return _lib
+
+
+def _dt(a: np.ndarray) -> int:
+    if a.dtype == np.float64:
+        return 1
+    if a.dtype == np.float32:
+        return 0
+    raise TypeError(a.dtype)
+
+
+def _p(a: Optional[np.ndarray]):
+    if a is None:
+        return None
+    assert a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _ip(a) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a, dtype=np.int32))
+
+
+def default_eps(dtype) -> float:
+    """HLLD degeneracy threshold (reading A7): 1e-12 in fp64, 1e-6 in fp32."""
+    return 1e-12 if np.dtype(dtype) == np.float64 else 1e-6
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def fill_ghosts(Ug: np.ndarray, g: int, origin, domain_cells, bc, self_periodic: bool) -> np.ndarray:
+    """O0 (i)+(ii) in place.  Returns mask[npatch, M, M, M]: 1 = interior or filled, 0 = left for O8."""
+    nf, npch, M = Ug.shape[0], Ug.shape[1], Ug.shape[2]
+    mask = np.zeros((npch, M, M, M), dtype=np.uint8)
+    o, d, b = _ip(origin), _ip(domain_cells), _ip(bc)
+    lib().oracle_fill_ghosts(_dt(Ug), _p(Ug), _p(mask), npch, M - 2 * g, g, nf, _p(o), _p(d), _p(b),
+                             int(bool(self_periodic)))
+    return mask
+
+
+def step(Ug: np.ndarray, g: int, dt: float, dx: float, gamma: float, limiter: int, riemann: int,
+         ch: float = 0.0, alpha: float = 0.0, eps: Optional[float] = None, want_flux: bool = False,
+         want_face_states: bool = False):
+    """O1..O6 on every patch.  Returns dict(U=ghosted array with updated interiors (ghosts copied
+    from the input), counters=..., F=[3, nf, np, M, M, M] or None, FS=[3, 2, nf, np, M, M, M] or None)."""
+    nf, npch, M = Ug.shape[0], Ug.shape[1], Ug.shape[2]
+    out = Ug.copy()
+    F = np.zeros((3,) + Ug.shape, dtype=Ug.dtype) if want_flux else None
+    FS = np.zeros((3, 2) + Ug.shape, dtype=Ug.dtype) if want_face_states else None
+    cnt = np.zeros(4, dtype=np.int64)
+    if eps is None:
+        eps = default_eps(Ug.dtype)
+    rc = lib().oracle_step(_dt(Ug), _p(Ug), _p(out), _p(F), _p(FS), npch, M - 2 * g, g, nf,
+                           C.c_double(dt), C.c_double(dx), C.c_double(gamma), int(limiter), int(riemann),
+                           C.c_double(ch), C.c_double(alpha), C.c_double(eps), _p(cnt))
+    if rc != 0:
+        raise ValueError("oracle_step rejected its arguments")
+    return dict(U=out, counters=dict(zip(CNT_NAMES, cnt.tolist())), F=F, FS=FS)
+
+
+def smax(Ug: np.ndarray, g: int, gamma: float) -> float:
+    """O7: max over interior cells and directions of |v_d| + c_d."""
+    nf, npch, M = Ug.shape[0], Ug.shape[1], Ug.shape[2]
+    return float(lib().oracle_smax(_dt(Ug), _p(Ug), npch, M - 2 * g, g, nf, C.c_double(gamma)))
+
+
+def totals(Ug: np.ndarray, g: int) -> np.ndarray:
+    nf, npch, M = Ug.shape[0], Ug.shape[1], Ug.shape[2]
+    out = np.zeros(nf)
+    lib().oracle_totals(_dt(Ug), _p(Ug), npch, M - 2 * g, g, nf, _p(out))
+    return out
+
+
+def riemann(WL, WR, gamma: float, solver: int, ch: float = 1.0, eps: float = 1e-12):
+    WL = np.ascontiguousarray(WL, dtype=np.float64)
+    WR = np.ascontiguousarray(WR, dtype=np.float64)
+    nf = WL.shape[0]
+    F = np.zeros(nf)
+    cnt = np.zeros(4, dtype=np.int64)
+    lib().oracle_riemann(nf, _p(WL), _p(WR), C.c_double(gamma), C.c_double(ch), int(solver),
+                         C.c_double(eps), _p(F), _p(cnt))
+    return F, dict(zip(CNT_NAMES, cnt.tolist()))
+
+
+def hlld_states(WL, WR, gamma: float, ch: float, eps: float = 1e-12):
+    """HLLD flux plus its intermediate fan: dict(S[5], U[6,7], FL[7], FR[7], ptstar, Bn, path, F[9])."""
+    WL = np.ascontiguousarray(WL, dtype=np.float64)
+    WR = np.ascontiguousarray(WR, dtype=np.float64)
+    F = np.zeros(9)
+    out = np.zeros(64)
+    lib().oracle_hlld_states(_p(WL), _p(WR), C.c_double(gamma), C.c_double(ch), C.c_double(eps), _p(F), _p(out))
+    return dict(S=out[0:5].copy(), U=out[5:47].reshape(6, 7).copy(), FL=out[47:54].copy(),
+                FR=out[54:61].copy(), ptstar=out[61], Bn=out[62], path=int(out[63]), F=F)
+
+
+def limited_slope(a: float, b: float, lim: int) -> float:
+    return float(lib().oracle_limited_slope(a, b, lim))
+
+
+# ----------------------------------------------------------------------------------------------
+# drivers (sequencing only; all arithmetic is in the C++ routines above)
+# ----------------------------------------------------------------------------------------------
+
+def ghosted(U: np.ndarray, g: int, dtype=np.float64) -> np.ndarray:
+    nf, npch, n = U.shape[0], U.shape[1], U.shape[2]
+    M = n + 2 * g
+    out = np.zeros((nf, npch, M, M, M), dtype=dtype)
+    out[:, :, g:g + n, g:g + n, g:g + n] = U.astype(dtype)
+    return out
+
+
+def interior(Ug: np.ndarray, g: int) -> np.ndarray:
+    M = Ug.shape[2]
+    return np.ascontiguousarray(Ug[:, :, g:M - g, g:M - g, g:M - g])
+
+
+def advance(level, wl, nsteps: int, dtype=np.float64, dt_fixed: Optional[float] = None,
+            limiter: Optional[int] = None, riemann_solver: Optional[int] = None, eps: Optional[float] = None):
+    """Single-level evolution exactly as the harness sequences it: every step = O0 ghost fill,
+    O7 smax -> dt = cfl dx / smax and c_h = smax, O1..O6.  `level`/`wl` are workloads.Level/Workload
+    (read as plain data).  Returns dict(U=final interior, dts=[...], smaxs=[...], counters=[...])."""
+    g = level.g
+    Ug = ghosted(level.U, g, dtype)
+    lim = wl.limiter if limiter is None else limiter
+    rs = wl.riemann if riemann_solver is None else riemann_solver
+    dts, smaxs, counters = [], [], []
+    for _ in range(nsteps):
+        fill_ghosts(Ug, g, level.origin, level.domain_cells, level.bc, level.self_periodic)
+        sm = smax(Ug, g, wl.gamma)
+        dt = dt_fixed if dt_fixed is not None else wl.cfl * level.dx / sm
+        r = step(Ug, g, dt, level.dx, wl.gamma, lim, rs, ch=sm, alpha=wl.alpha, eps=eps)
+        Ug = r["U"]
+        dts.append(dt)
+        smaxs.append(sm)
+        counters.append(r["counters"])
+    return dict(U=interior(Ug, g), dts=dts, smaxs=smaxs, counters=counters)
+
+
+def _geom_args(level):
+    return _ip(level.origin), _ip(level.domain_cells)
+
+
+def prolong_ghosts(Uf, mask, lf, Ucold, Ucnew, lc, theta: float):
+    of, df = _geom_args(lf)
+    oc, dc = _geom_args(lc)
+    nf, npf, M = Uf.shape[0], Uf.shape[1], Uf.shape[2]
+    lib().oracle_prolong_ghosts(_dt(Uf), _p(Uf), _p(mask), npf, lf.n, lf.g, nf, _p(of), _p(df),
+                                _p(Ucold), _p(Ucnew), Ucold.shape[1], _p(oc), _p(dc), C.c_double(theta))
+
+
+def restrict(Uf, lf, Uc, lc):
+    of, df = _geom_args(lf)
+    oc, dc = _geom_args(lc)
+    lib().oracle_restrict(_dt(Uf), _p(Uf), Uf.shape[1], lf.n, lf.g, Uf.shape[0], _p(of), _p(df),
+                          _p(Uc), Uc.shape[1], _p(oc), _p(dc))
+
+
+def reflux(Uc, lc, Fc, lf, Ffsum, dt0: float):
+    of, df = _geom_args(lf)
+    oc, dc = _geom_args(lc)
+    lib().oracle_reflux(_dt(Uc), _p(Uc), Uc.shape[1], lc.n, lc.g, Uc.shape[0], _p(oc), _p(dc), _p(Fc),
+                        Ffsum.shape[2], _p(of), _p(df), _p(Ffsum), C.c_double(dt0), C.c_double(lc.dx))
+
+
+def composite_totals(Uc, lc, Uf, lf) -> np.ndarray:
+    of, df = _geom_args(lf)
+    oc, dc = _geom_args(lc)
+    out = np.zeros(Uc.shape[0])
+    lib().oracle_composite_totals(_dt(Uc), _p(Uc), Uc.shape[1], lc.n, lc.g, Uc.shape[0], _p(oc), _p(dc),
+                                  _p(Uf), Uf.shape[1], _p(of), _p(df), C.c_double(lc.dx), _p(out))
+    return out
+
+
+def two_level_step(wl, dtype=np.float64, eps: Optional[float] = None, do_reflux: bool = True):
+    """O9: one coarse step with two fine substeps (Berger-Colella order).  Returns dict with the
+    final coarse/fine interiors, dt0, smax and the composite totals before/after."""
+    lc, lf = wl.levels
+    g = lc.g
+    Uc = ghosted(lc.U, g, dtype)
+    Uf = ghosted(lf.U, g, dtype)
+    tot0 = composite_totals(Uc, lc, Uf, lf)
+    sm = max(smax(Uc, g, wl.gamma), smax(Uf, g, wl.gamma))                       # (1)
+    dt0 = wl.cfl * lc.dx / sm
+    fill_ghosts(Uc, g, lc.origin, lc.domain_cells, lc.bc, False)                 # (2)
+    rc = step(Uc, g, dt0, lc.dx, wl.gamma, wl.limiter, wl.riemann, ch=sm, alpha=wl.alpha, eps=eps,
+              want_flux=True)                                                    # (3)
+    Ucnew = rc["U"]
+    fill_ghosts(Ucnew, g, lc.origin, lc.domain_cells, lc.bc, False)             # ghosts of U0^{n+1} for theta=1/2
+    Ffsum = None
+    counters = [rc["counters"]]
+    for theta in (0.0, 0.5):                                                     # (4), (5)
+        mask = fill_ghosts(Uf, g, lf.origin, lf.domain_cells, lf.bc, False)
+        prolong_ghosts(Uf, mask, lf, Uc, Ucnew, lc, theta)
+        rf = step(Uf, g, 0.5 * dt0, lf.dx, wl.gamma, wl.limiter, wl.riemann, ch=sm, alpha=wl.alpha,
+                  eps=eps, want_flux=True)
+        Uf = rf["U"]
+        Ffsum = rf["F"] if Ffsum is None else Ffsum + rf["F"]
+        counters.append(rf["counters"])
+    restrict(Uf, lf, Ucnew, lc)                                                  # (6)
+    if do_reflux:
+        reflux(Ucnew, lc, rc["F"], lf, Ffsum, dt0)                               # (7)
+    tot1 = composite_totals(Ucnew, lc, Uf, lf)
+    return dict(Uc=interior(Ucnew, g), Uf=interior(Uf, g), dt0=dt0, smax=sm, totals_before=tot0,
+                totals_after=tot1, counters=counters)

@@ -1,0 +1,409 @@
+"""Input generators for the five BASELINE.json configs.
+
+Data only.  Every random array comes from ``numpy.random.default_rng([SEED, config, stream])``
+in float64.  Array index order is ``U[field, patch, k, j, i]`` with ``i`` (x) fastest; the field
+order is rho, m_x, m_y, m_z, E [, B_x, B_y, B_z, psi] (reading A20).  Units with mu_0 = 1.
+"""
+from __future__ import annotations
+
+import dataclasses
+from typing import List, Optional, Sequence
+
+import numpy as np
+
+SEED = 14120934
+FIELDS_HYDRO = ("rho", "mx", "my", "mz", "E")
+FIELDS_MHD = FIELDS_HYDRO + ("Bx", "By", "Bz", "psi")
+
+BC_PERIODIC = 0
+BC_OUTFLOW = 1
+
+LIM_NONE, LIM_MINMOD, LIM_MC = 0, 1, 2
+RS_HLL, RS_HLLC, RS_HLLD = 0, 1, 2
+
+
+@dataclasses.dataclass
+class Level:
+    """One refinement level = one batch of equal-size cubic patches (interiors only)."""
+
+    n: int                      # interior cells per side
+    g: int                      # ghost layers carried by the API (3)
+    level: int
+    dx: float
+    origin: np.ndarray          # int32 [npatch, 3] lower corner (x, y, z) in level-cell units
+    domain_cells: tuple         # extent of this level's index space (x, y, z)
+    bc: tuple                   # 6 entries: xlo, xhi, ylo, yhi, zlo, zhi
+    self_periodic: bool
+    U: np.ndarray               # float64 [nfields, npatch, n, n, n]
+
+    @property
+    def npatch(self) -> int:
+        return int(self.U.shape[1])
+
+    @property
+    def nfields(self) -> int:
+        return int(self.U.shape[0])
+
+    @property
+    def ncells(self) -> int:
+        return self.npatch * self.n ** 3
+
+
+@dataclasses.dataclass
+class Workload:
+    name: str
+    levels: List[Level]
+    gamma: float
+    mhd: bool
+    limiter: int
+    riemann: int
+    cfl: float
+    nsteps: int
+    alpha: float = 0.4
+    note: str = ""
+
+
+# --------------------------------------------------------------------------------------
+# geometry helpers
+# --------------------------------------------------------------------------------------
+
+def _part1by2(v: np.ndarray) -> np.ndarray:
+    """Spread the low 10 bits of v so that there are two zero bits between each."""
+    v = v.astype(np.uint64) & np.uint64(0x3FF)
+    v = (v | (v << np.uint64(16))) & np.uint64(0x30000FF)
+    v = (v | (v << np.uint64(8))) & np.uint64(0x300F00F)
+    v = (v | (v << np.uint64(4))) & np.uint64(0x30C30C3)
+    v = (v | (v << np.uint64(2))) & np.uint64(0x9249249)
+    return v
+
+
+def morton_key(px, py, pz) -> np.ndarray:
+    px, py, pz = (np.asarray(a) for a in (px, py, pz))
+    return _part1by2(px) | (_part1by2(py) << np.uint64(1)) | (_part1by2(pz) << np.uint64(2))
+
+
+def morton_patch_origins(npx: int, npy: int, npz: int, n: int) -> np.ndarray:
+    """Origins (cell units) of an npx*npy*npz tiling by n^3 patches, ordered along a Morton
+    (Z-order) curve -- the paper's own first step (space-filling-curve order)."""
+    pz, py, px = np.meshgrid(np.arange(npz), np.arange(npy), np.arange(npx), indexing="ij")
+    px, py, pz = px.ravel(), py.ravel(), pz.ravel()
+    order = np.argsort(morton_key(px, py, pz), kind="stable")
+    return (np.stack([px[order], py[order], pz[order]], axis=1) * n).astype(np.int32)
+
+
+def split_into_patches(G: np.ndarray, n: int, origin: np.ndarray) -> np.ndarray:
+    """G[nf, Nz, Ny, Nx] -> U[nf, npatch, n, n, n] for the given patch origins."""
+    nf = G.shape[0]
+    out = np.empty((nf, origin.shape[0], n, n, n), dtype=G.dtype)
+    for p, (ox, oy, oz) in enumerate(origin):
+        out[:, p] = G[:, oz:oz + n, oy:oy + n, ox:ox + n]
+    return out
+
+
+def join_patches(U: np.ndarray, origin: np.ndarray, shape: Sequence[int]) -> np.ndarray:
+    """Inverse of split_into_patches; shape = (Nz, Ny, Nx)."""
+    nf, _, n = U.shape[0], U.shape[1], U.shape[2]
+    G = np.zeros((nf,) + tuple(shape), dtype=U.dtype)
+    for p, (ox, oy, oz) in enumerate(origin):
+        G[:, oz:oz + n, oy:oy + n, ox:ox + n] = U[:, p]
+    return G
+
+
+def add_ghost_frame(U: np.ndarray, g: int, fill: float = np.nan) -> np.ndarray:
+    """[nf, np, n, n, n] -> [nf, np, n+2g, n+2g, n+2g]; ghost cells set to `fill`."""
+    nf, npch, n = U.shape[0], U.shape[1], U.shape[2]
+    m = n + 2 * g
+    out = np.full((nf, npch, m, m, m), fill, dtype=U.dtype)
+    out[:, :, g:g + n, g:g + n, g:g + n] = U
+    return out
+
+
+def strip_ghost_frame(Ug: np.ndarray, g: int) -> np.ndarray:
+    m = Ug.shape[2]
+    return np.ascontiguousarray(Ug[:, :, g:m - g, g:m - g, g:m - g])
+
+
+def primitive_to_conserved(rho, v, p, gamma: float, B=None) -> np.ndarray:
+    """Initial data are specified in primitive variables; this applies the ideal-gas energy
+    definition E = p/(gamma-1) + rho|v|^2/2 [+ |B|^2/2] (SURVEY.md §8(c) Notation) to form the
+    conserved input arrays.  psi = 0 initially (A8)."""
+    rho = np.asarray(rho, dtype=np.float64)
+    fields = [rho, rho * v[0], rho * v[1], rho * v[2]]
+    E = np.asarray(p, dtype=np.float64) / (gamma - 1.0) + 0.5 * rho * (v[0] ** 2 + v[1] ** 2 + v[2] ** 2)
+    if B is not None:
+        E = E + 0.5 * (B[0] ** 2 + B[1] ** 2 + B[2] ** 2)
+    fields.append(E)
+    if B is not None:
+        fields += [np.asarray(B[0], dtype=np.float64) + 0.0 * rho,
+                   np.asarray(B[1], dtype=np.float64) + 0.0 * rho,
+                   np.asarray(B[2], dtype=np.float64) + 0.0 * rho,
+                   np.zeros_like(rho)]
+    return np.stack([np.broadcast_to(f, rho.shape) for f in fields]).astype(np.float64)
+
+
+# --------------------------------------------------------------------------------------
+# Gaussian random fields (reading A21)
+# --------------------------------------------------------------------------------------
+
+def _kgrid(N: int):
+    kx = np.fft.rfftfreq(N) * N
+    kf = np.fft.fftfreq(N) * N
+    KZ, KY, KX = np.meshgrid(kf, kf, kx, indexing="ij")
+    return KX, KY, KZ
+
+
+def _amplitude(N: int, index: float):
+    KX, KY, KZ = _kgrid(N)
+    k = np.sqrt(KX ** 2 + KY ** 2 + KZ ** 2)
+    amp = np.zeros_like(k)
+    keep = (k > 0) & (k <= N / 2)
+    amp[keep] = k[keep] ** (index / 2.0)
+    return amp, (KX, KY, KZ), k
+
+
+def _fft():
+    import scipy.fft as sfft
+    return sfft
+
+
+def gaussian_random_field(N: int, index: float, rng: np.random.Generator) -> np.ndarray:
+    """White noise -> rfftn -> * k^(index/2) (k=0 and k>N/2 zeroed) -> irfftn -> zero mean,
+    unit variance.  `index` is the 3-D power-per-mode spectral index n in P(k) ~ k^n."""
+    sfft = _fft()
+    w = rng.standard_normal((N, N, N))
+    amp, _, _ = _amplitude(N, index)
+    wh = sfft.rfftn(w, workers=-1)
+    del w
+    wh *= amp
+    f = sfft.irfftn(wh, s=(N, N, N), workers=-1)
+    del wh
+    f -= f.mean()
+    f /= f.std()
+    return f
+
+
+def solenoidal_random_field(N: int, index: float, rng: np.random.Generator) -> np.ndarray:
+    """Three filtered white-noise fields, projected B^ <- B^ - k (k.B^)/k^2, inverse
+    transformed, mean removed, scaled so that <B.B> = 1.  Returns [3, N, N, N] (x, y, z)."""
+    sfft = _fft()
+    amp, (KX, KY, KZ), k = _amplitude(N, index)
+    k2 = np.where(k > 0, k * k, 1.0)
+    hats = []
+    for _ in range(3):
+        w = rng.standard_normal((N, N, N))
+        h = sfft.rfftn(w, workers=-1)
+        h *= amp
+        hats.append(h)
+        del w
+    kdotb = (KX * hats[0] + KY * hats[1] + KZ * hats[2]) / k2
+    hats[0] -= KX * kdotb
+    hats[1] -= KY * kdotb
+    hats[2] -= KZ * kdotb
+    del kdotb
+    out = np.empty((3, N, N, N))
+    for c in range(3):
+        out[c] = sfft.irfftn(hats[c], s=(N, N, N), workers=-1)
+        out[c] -= out[c].mean()
+    hats.clear()
+    out /= np.sqrt(np.mean(out[0] ** 2 + out[1] ** 2 + out[2] ** 2))
+    return out
+
+
+def _rng(config: int, stream: int) -> np.random.Generator:
+    return np.random.default_rng([SEED, config, stream])
+
+
+# --------------------------------------------------------------------------------------
+# the five configs
+# --------------------------------------------------------------------------------------
+
+def config1_sod(n: int = 32, axis: int = 0) -> Workload:
+    """Config 1: Sod tube along `axis` on ONE n^3 patch, g=3, outflow, gamma=1.4, domain [0,1]^3.
+    Left (cells 0..n/2-1): rho=1, p=1; right: rho=0.125, p=0.1; v=0.  The discontinuity sits on
+    the cell face x=0.5."""
+    gamma = 1.4
+    idx = np.arange(n)
+    shape = [1, 1, 1]
+    shape[2 - axis] = n                      # array order is (k, j, i) = (z, y, x)
+    left = (idx < n // 2).reshape(shape)
+    rho = np.broadcast_to(np.where(left, 1.0, 0.125), (n, n, n)).copy()
+    p = np.broadcast_to(np.where(left, 1.0, 0.1), (n, n, n)).copy()
+    zero = np.zeros((n, n, n))
+    U = primitive_to_conserved(rho, (zero, zero, zero), p, gamma)[:, None]
+    lev = Level(n=n, g=3, level=0, dx=1.0 / n, origin=np.zeros((1, 3), np.int32),
+                domain_cells=(n, n, n), bc=(BC_OUTFLOW,) * 6, self_periodic=False,
+                U=np.ascontiguousarray(U))
+    return Workload("config1_sod", [lev], gamma, False, LIM_MINMOD, RS_HLLC, 0.4, 20)
+
+
+def config2_random_patches(npatch: int = 512, n: int = 16) -> Workload:
+    """Config 2: `npatch` independent self-periodic hydro patches.  Per patch p (stream = p):
+    rho = exp(0.5 g0) / patch mean; v_d = (c_s/sqrt3) g_d with c_s = sqrt(gamma); p = 1."""
+    gamma = 5.0 / 3.0
+    cs = np.sqrt(gamma * 1.0 / 1.0)
+    U = np.empty((5, npatch, n, n, n))
+    for p in range(npatch):
+        rng = _rng(2, p)
+        g = rng.standard_normal((4, n, n, n))
+        rho = np.exp(0.5 * g[0])
+        rho /= rho.mean()
+        v = (cs / np.sqrt(3.0)) * g[1:4]
+        U[:, p] = primitive_to_conserved(rho, v, np.ones_like(rho), gamma)
+    origin = np.zeros((npatch, 3), np.int32)
+    lev = Level(n=n, g=3, level=0, dx=1.0 / n, origin=origin, domain_cells=(n, n, n),
+                bc=(BC_PERIODIC,) * 6, self_periodic=True, U=U)
+    return Workload("config2_random_patches", [lev], gamma, False, LIM_MC, RS_HLLC, 0.4, 1)
+
+
+def orszag_tang_state(N: int, eps: float = 0.2) -> np.ndarray:
+    """Reading A16: 3-D (z-modulated) Orszag-Tang vortex at cell centres of an N^3 grid on
+    [0,1]^3.  Returns conserved G[9, N, N, N]."""
+    gamma = 5.0 / 3.0
+    c = (np.arange(N) + 0.5) / N
+    Z, Y, X = np.meshgrid(c, c, c, indexing="ij")
+    rho = np.full((N, N, N), 25.0 / (36.0 * np.pi))
+    p = np.full((N, N, N), 5.0 / (12.0 * np.pi))
+    B0 = 1.0 / np.sqrt(4.0 * np.pi)
+    mod = 1.0 + eps * np.sin(2 * np.pi * Z)
+    vx = -mod * np.sin(2 * np.pi * Y)
+    vy = mod * np.sin(2 * np.pi * X)
+    vz = eps * np.sin(2 * np.pi * Z)
+    Bx = -B0 * np.sin(2 * np.pi * Y)
+    By = B0 * np.sin(4 * np.pi * X)
+    Bz = np.zeros_like(Bx)
+    return primitive_to_conserved(rho, (vx, vy, vz), p, gamma, B=(Bx, By, Bz))
+
+
+def uniform_grid_workload(name: str, G: np.ndarray, n: int, gamma: float, mhd: bool, limiter: int,
+                          riemann: int, cfl: float, nsteps: int, alpha: float = 0.4,
+                          bc=(BC_PERIODIC,) * 6) -> Workload:
+    """Tile a global grid G[nf, Nz, Ny, Nx] (domain [0,1] along x) into n^3 patches in Morton order."""
+    Nz, Ny, Nx = G.shape[1:]
+    origin = morton_patch_origins(Nx // n, Ny // n, Nz // n, n)
+    U = split_into_patches(G, n, origin)
+    lev = Level(n=n, g=3, level=0, dx=1.0 / Nx, origin=origin, domain_cells=(Nx, Ny, Nz),
+                bc=tuple(bc), self_periodic=False, U=U)
+    return Workload(name, [lev], gamma, mhd, limiter, riemann, cfl, nsteps, alpha)
+
+
+def config3_orszag_tang(N: int = 256, n: int = 16, eps: float = 0.2) -> Workload:
+    """Config 3: Orszag-Tang on N^3 periodic, (N/n)^3 patches of n^3 in Morton order; MC + HLLD +
+    GLM alpha=0.4, cfl 0.3, 5 steps."""
+    G = orszag_tang_state(N, eps)
+    return uniform_grid_workload("config3_orszag_tang", G, n, 5.0 / 3.0, True, LIM_MC, RS_HLLD,
+                                 0.3, 5)
+
+
+def turbulence_state(N: int, config: int = 5, mach: float = 3.0, beta: float = 100.0,
+                     index: float = -11.0 / 3.0) -> np.ndarray:
+    """Config-5 state on an N^3 grid: rho=1, p=1, v = GRFs with P(k) ~ k^index scaled to
+    sqrt<v.v> = mach*sqrt(gamma); B solenoidal, zero mean, <B.B> = 2p/beta."""
+    gamma = 5.0 / 3.0
+    cs = np.sqrt(gamma)
+    v = np.stack([gaussian_random_field(N, index, _rng(config, s)) for s in range(3)])
+    v *= mach * cs / np.sqrt(np.mean(v[0] ** 2 + v[1] ** 2 + v[2] ** 2))
+    B = solenoidal_random_field(N, index, _rng(config, 3))
+    B *= np.sqrt(2.0 * 1.0 / beta)
+    one = np.ones((N, N, N))
+    return primitive_to_conserved(one, v, one, gamma, B=B)
+
+
+def config5_turbulence(N: int = 512, n: int = 32) -> Workload:
+    """Config 5: N^3 periodic MHD turbulence, (N/n)^3 patches of n^3, Morton order; MC + HLLD +
+    GLM, cfl 0.3, 10 steps."""
+    G = turbulence_state(N)
+    return uniform_grid_workload("config5_turbulence", G, n, 5.0 / 3.0, True, LIM_MC, RS_HLLD,
+                                 0.3, 10)
+
+
+# sigma(ln rho) tuned once (reading A15: start 1.2 flags 4007 blocks; 0.517 flags ~102) so that ~100 of the 4096 aligned 8^3 root blocks are
+# flagged; the resulting count is recorded in Workload.note and DESIGN.md.
+CONFIG4_SIGMA = 0.517
+
+
+def config4_two_level(mhd: bool, nfine: int = 256, n: int = 16, sigma: float = CONFIG4_SIGMA,
+                      threshold: float = 4.0) -> Workload:
+    """Config 4: root (nfine/2)^3 periodic as n^3 patches + level-1 n^3 patches on aligned
+    (n/2)^3 root blocks that contain a root cell with rho > threshold*mean (A15)."""
+    gamma = 5.0 / 3.0
+    N = nfine
+    Gln = gaussian_random_field(N, -2.0, _rng(4, 0))
+    rho = np.exp(sigma * Gln)
+    rho /= rho.mean()
+    v = np.stack([gaussian_random_field(N, -2.0, _rng(4, 1 + s)) for s in range(3)])
+    v *= 2.0 * np.sqrt(gamma * 1.0 / 1.0) / np.sqrt(np.mean(v[0] ** 2 + v[1] ** 2 + v[2] ** 2))
+    p = np.ones_like(rho)
+    if mhd:
+        dB = solenoidal_random_field(N, -2.0, _rng(4, 4)) * 1.0e-4
+        B = (dB[0], dB[1], dB[2] + 1.0e-3)
+        Gf = primitive_to_conserved(rho, v, p, gamma, B=B)
+    else:
+        Gf = primitive_to_conserved(rho, v, p, gamma)
+    nf = Gf.shape[0]
+    Nc = N // 2
+    # root = 2x2x2 mean of the conserved variables
+    Gc = Gf.reshape(nf, Nc, 2, Nc, 2, Nc, 2).mean(axis=(2, 4, 6))
+    # flag aligned (n/2)^3 root blocks
+    nb = n // 2
+    nblk = Nc // nb
+    blkmax = Gc[0].reshape(nblk, nb, nblk, nb, nblk, nb).max(axis=(1, 3, 5))
+    bz, by, bx = np.nonzero(blkmax > threshold * Gc[0].mean())
+    order = np.argsort(morton_key(bx, by, bz), kind="stable")
+    bx, by, bz = bx[order], by[order], bz[order]
+    origin1 = (np.stack([bx, by, bz], axis=1) * n).astype(np.int32)      # level-1 cell units
+    origin0 = morton_patch_origins(Nc // n, Nc // n, Nc // n, n)
+    lev0 = Level(n=n, g=3, level=0, dx=1.0 / Nc, origin=origin0, domain_cells=(Nc, Nc, Nc),
+                 bc=(BC_PERIODIC,) * 6, self_periodic=False, U=split_into_patches(Gc, n, origin0))
+    lev1 = Level(n=n, g=3, level=1, dx=1.0 / N, origin=origin1, domain_cells=(N, N, N),
+                 bc=(BC_PERIODIC,) * 6, self_periodic=False, U=split_into_patches(Gf, n, origin1))
+    w = Workload("config4_two_level_" + ("mhd" if mhd else "hydro"), [lev0, lev1], gamma, mhd,
+                 LIM_MC, RS_HLLD if mhd else RS_HLLC, 0.3, 1)
+    w.note = "sigma=%g refined_blocks=%d extra_cell_fraction=%.4f" % (
+        sigma, origin1.shape[0], origin1.shape[0] * n ** 3 / float(Nc ** 3))
+    return w
+
+
+# --------------------------------------------------------------------------------------
+# smooth test states (pins P10, P12): single self-periodic patch of n^3 on [0,1]^3
+# --------------------------------------------------------------------------------------
+
+def smooth_wave_patchset(kind: str, N: int, axis: int = 0, t: float = 0.0, n: int = 8) -> Workload:
+    """Plane wave along `axis` on a periodic domain of N cells along the axis and n cells across,
+    tiled by n^3 patches; dx = 1/N.
+    `density`: rho = 1 + 0.2 sin(2 pi (s - t)), u_axis = 1, p = 1 (exact: translation).
+    `alfven`: circularly polarised Alfven wave along `axis` (rho=1, p=0.1, B_par=1,
+    B_perp = 0.1 (cos, sin)(2 pi (s - t)), v_perp = -B_perp: travels in +axis at speed 1).
+    Evaluated at cell centres at time t, so t>0 gives the exact solution to compare with."""
+    gamma = 5.0 / 3.0
+    dims = [n, n, n]                          # (Nx, Ny, Nz)
+    dims[axis] = N
+    c = (np.arange(N) + 0.5) / N
+    shape = [1, 1, 1]
+    shape[2 - axis] = N
+    full = (dims[2], dims[1], dims[0])
+    s = np.broadcast_to(c.reshape(shape), full)
+    ph = 2.0 * np.pi * (s - t)
+    zero = np.zeros(full)
+    a, b1, b2 = axis, (axis + 1) % 3, (axis + 2) % 3
+    if kind == "density":
+        v = [zero, zero, zero]
+        v[a] = zero + 1.0
+        G = primitive_to_conserved(1.0 + 0.2 * np.sin(ph), v, zero + 1.0, gamma)
+        mhd = False
+    elif kind == "alfven":
+        B = [None, None, None]
+        v = [None, None, None]
+        B[a] = zero + 1.0
+        B[b1] = 0.1 * np.cos(ph)
+        B[b2] = 0.1 * np.sin(ph)
+        v[a] = zero
+        v[b1] = -B[b1]
+        v[b2] = -B[b2]
+        G = primitive_to_conserved(zero + 1.0, v, zero + 0.1, gamma, B=B)
+        mhd = True
+    else:
+        raise ValueError(kind)
+    w = uniform_grid_workload("smooth_" + kind, G, n, gamma, mhd, LIM_MC, RS_HLLD if mhd else RS_HLLC,
+                              0.3, 0)
+    w.levels[0].dx = 1.0 / N
+    return w
