@@ -1,0 +1,147 @@
+/* amr_godunov.h -- C-ABI of libamrgodunov.so: the per-patch second-order Godunov hydro/MHD update
+ * of arXiv 1412.0934 ("Numerical cosmology on the GPU with Enzo and Ramses") on NVIDIA B200.
+ *
+ * What the paper offloads (PAPER.md:43 "Piecewise Linear Method"; :57 "inner cells plus boundary
+ * cells, properly calculated through interpolation"; :58 "hydro equations are solved on the chunk";
+ * :76 "All fluxes necessary to update the patch's cells are computed on the GPU", "only fluxes
+ * required for flux correction ... are moved back", "MHD solver"; :31 refinement "in space as well
+ * as in time") is built here as one resident-arena library.  The concrete scheme (MUSCL-Hancock
+ * PLM + limiter, HLL/HLLC or GLM+HLL/HLLD flux, conservative update, CFL reduction) is fixed by
+ * BASELINE.json:north_star; its formulas are the readings O0..O9 / A1..A22 of DESIGN.md §3
+ * (SURVEY.md §8(c)).
+ *
+ * Conventions
+ *  - Plain C.  Every call returns an int status (AMR_OK = 0, negative = error); after an error
+ *    amr_last_error() gives a thread-local message.  No call throws, none aborts.
+ *  - "host" / "device" is stated for every pointer.  Host metadata is copied at create time.
+ *  - The DEVICE ARENA is allocated by the caller (e.g. a torch uint8 tensor) and only BORROWED:
+ *    the library never frees it and keeps pointers into it until amr_patch_batch_destroy.
+ *  - Calls enqueue work on the cudaStream_t given at create time and do not synchronise, except
+ *    the ones that return host data (upload/download, amr_cfl_dt, amr_conserved_totals,
+ *    amr_step_counters), which synchronise that stream.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns AMR_ECUDA.
+ *
+ * Data layout
+ *  - Field order rho, m_x, m_y, m_z, E [, B_x, B_y, B_z, psi]  (mu_0 = 1; reading A20).
+ *  - Host arrays are U[field][patch][k][j][i], i (x) fastest, either interiors only (n^3 per
+ *    patch) or with nghost ghost layers ((n+2g)^3 per patch).
+ *  - In the arena the state is stored INTERIORS ONLY, SoA, U[field][patch][n^3], in two buffers
+ *    (old/new) that every step swaps.  Ghost zones are not stored: the step kernel assembles the
+ *    radius-2 halo of each tile from the neighbouring patches' interiors through a 27-entry
+ *    neighbour table per patch (periodic wrap and outflow clamp resolved on the host at create
+ *    time), and from the prolongation halo buffer for fine patches next to a coarser level.
+ */
+#ifndef AMR_GODUNOV_H_
+#define AMR_GODUNOV_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { AMR_OK = 0, AMR_EINVAL = -1, AMR_ENOMEM = -2, AMR_ECUDA = -3, AMR_ESTATE = -4 };
+enum { AMR_F32 = 0, AMR_F64 = 1 };
+enum { AMR_BC_PERIODIC = 0, AMR_BC_OUTFLOW = 1 };
+enum { AMR_LIM_NONE = 0, AMR_LIM_MINMOD = 1, AMR_LIM_MC = 2 };   /* O2, reading A4 */
+enum { AMR_RS_HLL = 0, AMR_RS_HLLC = 1, AMR_RS_HLLD = 2 };       /* O5 */
+/* amr_step_counters slots (same meaning as the oracle's; reading A7/A10) */
+enum { AMR_CNT_POSITIVITY = 0, AMR_CNT_HLL_FALLBACK = 1, AMR_CNT_DEGENERATE_D = 2, AMR_CNT_NEG_STATE = 3 };
+
+typedef struct amr_patch_batch amr_patch_batch; /* opaque; one batch = all equal-size patches of one level */
+typedef struct amr_level_link amr_level_link;   /* opaque; coarse<->fine tables + flux registers */
+
+typedef struct {
+  int32_t npatch;          /* >= 1 */
+  int32_t n;               /* interior cells per side: 8, 16 or 32 (multiple of 8) */
+  int32_t nghost;          /* ghost layers of the HOST layout, 2..4 (configs use 3; the stencil uses 2, A11) */
+  int32_t nfields;         /* 5 = hydro, 9 = MHD */
+  int32_t dtype;           /* AMR_F32 | AMR_F64 */
+  int32_t level;           /* 0 = root.  level > 0 reserves the prolongation halo buffer */
+  double dx;               /* cell size of this level (> 0) */
+  const int32_t* origin;   /* host, [npatch][3] lower corner (x,y,z) in level-cell units; multiples of n */
+  int32_t domain_cells[3]; /* extent of this level's index space (multiples of n) */
+  int32_t bc[6];           /* xlo,xhi,ylo,yhi,zlo,zhi: AMR_BC_* */
+  int32_t self_periodic;   /* 1: every patch is its own periodic neighbour (config 2); origin ignored */
+} amr_batch_desc;
+
+/* Bytes of device arena amr_patch_batch_create needs for this desc (0 on an invalid desc). */
+size_t amr_patch_batch_bytes(const amr_batch_desc* desc);
+
+/* Build a batch inside the caller's device arena (device pointer, 256-byte aligned, `bytes` >=
+ * amr_patch_batch_bytes).  `cuda_stream` is a cudaStream_t (NULL = default stream).  Builds the
+ * neighbour tables on the host (O0: sibling copy with periodic wrap, outflow clamp; a region with
+ * no sibling on a level > 0 is marked "from the prolongation halo") and uploads them.
+ * Errors: AMR_EINVAL (null pointers, n, nfields, dtype, nghost, dx, origins not multiples of n or
+ * outside the domain, duplicate patches, a root-level region with no sibling and no BC, arena too
+ * small or misaligned), AMR_ECUDA. */
+int amr_patch_batch_create(const amr_batch_desc* desc, void* dev_arena, size_t bytes, void* cuda_stream,
+                           amr_patch_batch** out);
+int amr_patch_batch_destroy(amr_patch_batch* b);
+
+/* Host <-> arena copies of the CURRENT state (set-up and checking only; never needed per step).
+ * host: [nfields][npatch][(n+2g)^3] if with_ghosts else [nfields][npatch][n^3], batch dtype.
+ * upload ignores the ghost cells of a ghosted host array.  download with_ghosts=1 returns the
+ * ghost cells the step kernel would see (O0 rules (i)-(iii); cells on a level>0 that only O8 can
+ * supply come from the last amr_prolong_ghosts, NaN if there was none).  Both synchronise. */
+int amr_patch_batch_upload(amr_patch_batch* b, const void* host, int with_ghosts);
+int amr_patch_batch_download(amr_patch_batch* b, void* host, int with_ghosts);
+
+/* Device pointer of the current (which=0) or previous (which=1) state buffer, U[field][patch][n^3]. */
+void* amr_patch_batch_state(amr_patch_batch* b, int which);
+
+/* O0.  The halo is assembled inside the step kernel, so this only validates the batch and returns
+ * AMR_OK; it exists because the hierarchy code above the boundary calls it. */
+int amr_fill_ghosts(amr_patch_batch* b);
+
+/* O7 (reading A9): smax = max over interior cells and directions of |v_d| + c_d (c_d = sound speed,
+ * or the fast speed along d when mhd != 0); dt = cfl*dx/smax.  If the last call on this batch was a
+ * step with the same gamma, the value fused into that step's epilogue is returned (bitwise equal to
+ * the standalone reduction); otherwise a reduction kernel runs.  Synchronises.  dt_out/smax_out: host. */
+int amr_cfl_dt(amr_patch_batch* b, double gamma, double cfl, int mhd, double* dt_out, double* smax_out);
+
+/* O1..O6 for every patch of the batch: reads the current state (halo assembled on the fly), writes
+ * the other buffer, swaps.  amr_hydro_step: nfields must be 5, riemann HLL|HLLC.  amr_mhd_step:
+ * nfields 9, riemann HLL|HLLD, ch = GLM wave speed (> 0), alpha = damping constant (psi *=
+ * exp(-alpha*ch*dt/dx), reading A8).  Errors: AMR_EINVAL for dt <= 0, non-finite gamma or gamma <= 1,
+ * unknown limiter/riemann, wrong nfields; AMR_ESTATE if a level>0 batch was never given a halo. */
+int amr_hydro_step(amr_patch_batch* b, double dt, double gamma, int limiter, int riemann);
+int amr_mhd_step(amr_patch_batch* b, double dt, double gamma, int limiter, int riemann, double ch,
+                 double alpha);
+
+/* Sum over interior cells of each field (double accumulation, deterministic).  totals: host [nfields]. */
+int amr_conserved_totals(amr_patch_batch* b, double* totals);
+
+/* Event counters accumulated since the last call with reset != 0.  counters: host [4] (AMR_CNT_*).
+ * Face events are counted once per tile that computes the face. */
+int amr_step_counters(amr_patch_batch* b, long long* counters, int reset);
+
+/* ---- two-level operators (O8, O9; config 4) ------------------------------------------------- */
+/* Device workspace (flux registers + tables) a link needs; 0 on error. */
+size_t amr_link_bytes(const amr_patch_batch* coarse, const amr_patch_batch* fine, int ratio);
+/* Ties a fine batch to its parent level (ratio must be 2).  dev_ws: device, borrowed like an arena.
+ * From then on steps of both batches also record the face fluxes the reflux needs. */
+int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, void* dev_ws, size_t bytes,
+                    amr_level_link** out);
+int amr_link_destroy(amr_level_link* l);
+/* O8: fill the fine halo cells no sibling covers from the coarse level, coarse state =
+ * (1-theta)*U_old + theta*U_new where new/old are the coarse batch's current/previous buffers
+ * (theta in [0,1]; call after the coarse step).  Conservative minmod-limited linear interpolation. */
+int amr_prolong_ghosts(amr_level_link* l, double theta);
+/* Zero the flux registers (call before the coarse step of O9). */
+int amr_flux_clear(amr_level_link* l);
+/* O9(6): covered coarse cell <- mean of its 8 fine cells (current states). */
+int amr_restrict(amr_level_link* l);
+/* O9(7): U_c += s_f (dt_coarse/dx_coarse) (F_coarse - <F_fine>) on uncovered coarse cells next to a
+ * fine patch face, from the fluxes recorded since amr_flux_clear. */
+int amr_reflux(amr_level_link* l, double dt_coarse);
+
+const char* amr_last_error(void);
+/* Library/build description, e.g. "amr_godunov sm_100a ..." (static string). */
+const char* amr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AMR_GODUNOV_H_ */

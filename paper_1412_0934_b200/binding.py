@@ -1,0 +1,251 @@
+"""ctypes binding of libamrgodunov.so -- argument marshalling only (include/amr_godunov.h has the
+contract).  Every step of the hot path runs inside the library's CUDA kernels; nothing here computes.
+
+torch is imported lazily and used for exactly two things: the device arena (a uint8 tensor the
+library borrows) and the current CUDA stream handle.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+AMR_F32, AMR_F64 = 0, 1
+AMR_BC_PERIODIC, AMR_BC_OUTFLOW = 0, 1
+AMR_LIM_NONE, AMR_LIM_MINMOD, AMR_LIM_MC = 0, 1, 2
+AMR_RS_HLL, AMR_RS_HLLC, AMR_RS_HLLD = 0, 1, 2
+CNT_NAMES = ("positivity_fallback_cells", "hll_fallback_faces", "degenerate_D", "nonpositive_rho_after")
+
+# every symbol include/amr_godunov.h declares
+EXPORTS = (
+    "amr_patch_batch_bytes", "amr_patch_batch_create", "amr_patch_batch_destroy", "amr_patch_batch_upload",
+    "amr_patch_batch_download", "amr_patch_batch_state", "amr_fill_ghosts", "amr_cfl_dt", "amr_hydro_step",
+    "amr_mhd_step", "amr_conserved_totals", "amr_step_counters", "amr_link_bytes", "amr_link_levels",
+    "amr_link_destroy", "amr_prolong_ghosts", "amr_flux_clear", "amr_restrict", "amr_reflux", "amr_last_error",
+    "amr_version",
+)
+
+
+class AmrError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__("amr_godunov error %d: %s" % (code, msg))
+        self.code = code
+
+
+class _Desc(C.Structure):
+    _fields_ = [("npatch", C.c_int32), ("n", C.c_int32), ("nghost", C.c_int32), ("nfields", C.c_int32),
+                ("dtype", C.c_int32), ("level", C.c_int32), ("dx", C.c_double), ("origin", C.c_void_p),
+                ("domain_cells", C.c_int32 * 3), ("bc", C.c_int32 * 6), ("self_periodic", C.c_int32)]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return os.path.join(os.path.dirname(os.path.abspath(__file__)), "libamrgodunov.so")
+
+
+def lib():
+    """Load the C-ABI library.  Fails loudly if it has not been built (no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise ImportError("%s is missing: run `python -m paper_1412_0934_b200.build` (needs nvcc)" % path)
+        L = C.CDLL(path)
+        L.amr_last_error.restype = C.c_char_p
+        L.amr_version.restype = C.c_char_p
+        L.amr_patch_batch_bytes.restype = C.c_size_t
+        L.amr_patch_batch_bytes.argtypes = [C.POINTER(_Desc)]
+        L.amr_patch_batch_create.argtypes = [C.POINTER(_Desc), C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(C.c_void_p)]
+        L.amr_patch_batch_destroy.argtypes = [C.c_void_p]
+        L.amr_patch_batch_upload.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.amr_patch_batch_download.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.amr_patch_batch_state.restype = C.c_void_p
+        L.amr_patch_batch_state.argtypes = [C.c_void_p, C.c_int]
+        L.amr_fill_ghosts.argtypes = [C.c_void_p]
+        L.amr_cfl_dt.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.amr_hydro_step.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int]
+        L.amr_mhd_step.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double]
+        L.amr_conserved_totals.argtypes = [C.c_void_p, C.c_void_p]
+        L.amr_step_counters.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.amr_link_bytes.restype = C.c_size_t
+        L.amr_link_bytes.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
+        L.amr_link_levels.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.POINTER(C.c_void_p)]
+        L.amr_link_destroy.argtypes = [C.c_void_p]
+        L.amr_prolong_ghosts.argtypes = [C.c_void_p, C.c_double]
+        L.amr_flux_clear.argtypes = [C.c_void_p]
+        L.amr_restrict.argtypes = [C.c_void_p]
+        L.amr_reflux.argtypes = [C.c_void_p, C.c_double]
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise AmrError(rc, lib().amr_last_error().decode())
+
+
+def _np_dtype(dtype: int):
+    return np.float64 if dtype == AMR_F64 else np.float32
+
+
+def _host_ptr(a) -> int:
+    """Host pointer of a C-contiguous numpy array or (pinned) CPU torch tensor."""
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return a.ctypes.data
+    assert a.device.type == "cpu" and a.is_contiguous()
+    return a.data_ptr()
+
+
+class PatchBatch:
+    """amr_patch_batch: all equal-size patches of one level, resident in one device arena."""
+
+    def __init__(self, npatch: int, n: int, nfields: int, dtype: int, dx: float, origin=None,
+                 domain_cells: Sequence[int] = (0, 0, 0), bc: Sequence[int] = (0,) * 6, self_periodic: bool = False,
+                 nghost: int = 3, level: int = 0, device: str = "cuda:0", stream: Optional[int] = None):
+        import torch  # device memory + stream only
+        self._torch = torch
+        L = lib()
+        d = _Desc()
+        d.npatch, d.n, d.nghost, d.nfields, d.dtype, d.level, d.dx = npatch, n, nghost, nfields, dtype, level, dx
+        self._origin = None
+        if origin is not None:
+            self._origin = np.ascontiguousarray(np.asarray(origin, dtype=np.int32).reshape(-1, 3))
+            if self._origin.shape[0] != npatch:
+                raise ValueError("origin must be [npatch, 3]")
+            d.origin = self._origin.ctypes.data
+        d.domain_cells[:] = [int(v) for v in domain_cells]
+        d.bc[:] = [int(v) for v in bc]
+        d.self_periodic = int(bool(self_periodic))
+        self.npatch, self.n, self.nghost, self.nfields, self.dtype, self.dx, self.level = npatch, n, nghost, nfields, dtype, dx, level
+        nbytes = L.amr_patch_batch_bytes(C.byref(d))
+        if nbytes == 0:
+            raise AmrError(-1, L.amr_last_error().decode())
+        self.device = torch.device(device)
+        with torch.cuda.device(self.device):
+            self.arena = torch.empty(nbytes, dtype=torch.uint8, device=self.device)  # borrowed by the library
+            self.stream = int(torch.cuda.current_stream().cuda_stream) if stream is None else int(stream)
+            h = C.c_void_p()
+            _check(L.amr_patch_batch_create(C.byref(d), self.arena.data_ptr(), nbytes, self.stream, C.byref(h)))
+        self._h = h
+        self.arena_bytes = int(nbytes)
+
+    @classmethod
+    def from_level(cls, level, dtype: int, **kw):
+        """Build from a workloads.Level (plain data) and upload its interiors."""
+        b = cls(level.npatch, level.n, level.nfields, dtype, level.dx, origin=level.origin,
+                domain_cells=level.domain_cells, bc=level.bc, self_periodic=level.self_periodic, nghost=level.g,
+                level=level.level, **kw)
+        b.upload(np.ascontiguousarray(level.U.astype(_np_dtype(dtype))))
+        return b
+
+    @property
+    def handle(self):
+        return self._h
+
+    @property
+    def np_dtype(self):
+        return _np_dtype(self.dtype)
+
+    @property
+    def ncells(self) -> int:
+        return self.npatch * self.n ** 3
+
+    def _shape(self, with_ghosts: bool):
+        m = self.n + (2 * self.nghost if with_ghosts else 0)
+        return (self.nfields, self.npatch, m, m, m)
+
+    def upload(self, host, with_ghosts: bool = False):
+        assert tuple(host.shape) == self._shape(with_ghosts), (tuple(host.shape), self._shape(with_ghosts))
+        _check(lib().amr_patch_batch_upload(self._h, _host_ptr(host), int(with_ghosts)))
+
+    def download(self, with_ghosts: bool = False, out=None):
+        if out is None:
+            out = np.empty(self._shape(with_ghosts), dtype=self.np_dtype)
+        _check(lib().amr_patch_batch_download(self._h, _host_ptr(out), int(with_ghosts)))
+        return out
+
+    def state_ptr(self, which: int = 0) -> int:
+        return int(lib().amr_patch_batch_state(self._h, which))
+
+    def fill_ghosts(self):
+        _check(lib().amr_fill_ghosts(self._h))
+
+    def cfl_dt(self, gamma: float, cfl: float):
+        dt, sm = C.c_double(), C.c_double()
+        _check(lib().amr_cfl_dt(self._h, gamma, cfl, int(self.nfields == 9), C.byref(dt), C.byref(sm)))
+        return dt.value, sm.value
+
+    def hydro_step(self, dt: float, gamma: float, limiter: int, riemann: int):
+        _check(lib().amr_hydro_step(self._h, dt, gamma, limiter, riemann))
+
+    def mhd_step(self, dt: float, gamma: float, limiter: int, riemann: int, ch: float, alpha: float):
+        _check(lib().amr_mhd_step(self._h, dt, gamma, limiter, riemann, ch, alpha))
+
+    def conserved_totals(self) -> np.ndarray:
+        out = np.zeros(self.nfields, dtype=np.float64)
+        _check(lib().amr_conserved_totals(self._h, out.ctypes.data))
+        return out
+
+    def step_counters(self, reset: bool = False) -> dict:
+        out = np.zeros(4, dtype=np.int64)
+        _check(lib().amr_step_counters(self._h, out.ctypes.data, int(reset)))
+        return dict(zip(CNT_NAMES, out.tolist()))
+
+    def synchronize(self):
+        self._torch.cuda.synchronize(self.device)
+
+    def close(self):
+        if self._h is not None and self._h.value:
+            _check(lib().amr_patch_batch_destroy(self._h))
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class LevelLink:
+    """amr_level_link: coarse<->fine tables and flux registers (O8, O9)."""
+
+    def __init__(self, coarse: PatchBatch, fine: PatchBatch, ratio: int = 2):
+        import torch
+        L = lib()
+        nbytes = L.amr_link_bytes(coarse.handle, fine.handle, ratio)
+        if nbytes == 0:
+            raise AmrError(-1, L.amr_last_error().decode())
+        self.coarse, self.fine = coarse, fine
+        self.ws = torch.empty(nbytes, dtype=torch.uint8, device=coarse.device)
+        h = C.c_void_p()
+        _check(L.amr_link_levels(coarse.handle, fine.handle, ratio, self.ws.data_ptr(), nbytes, C.byref(h)))
+        self._h = h
+        self.ws_bytes = int(nbytes)
+
+    def prolong_ghosts(self, theta: float):
+        _check(lib().amr_prolong_ghosts(self._h, theta))
+
+    def flux_clear(self):
+        _check(lib().amr_flux_clear(self._h))
+
+    def restrict(self):
+        _check(lib().amr_restrict(self._h))
+
+    def reflux(self, dt_coarse: float):
+        _check(lib().amr_reflux(self._h, dt_coarse))
+
+    def close(self):
+        if self._h is not None and self._h.value:
+            _check(lib().amr_link_destroy(self._h))
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,69 @@
+// Internal declarations shared by the host code (batch.cu) and the kernel translation units.
+// Nothing here crosses the C-ABI (include/amr_godunov.h).  No code is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+namespace amr {
+
+constexpr int NBR_PATCH_MASK = 0x0FFFFFFF;  // nbr entry >= 0: low 28 bits = source patch,
+constexpr int NBR_MODE_SHIFT = 28;          // bits 28..30 = clamp flags (x,y,z) for outflow
+constexpr int NBR_FROM_HALO = -2;           // nbr entry: region comes from the prolongation halo buffer
+
+// Everything the step kernel needs, passed by value.
+template <class T>
+struct StepParams {
+  const T* Uin;        // device, [NF][np][n^3]
+  T* Uout;             // device, [NF][np][n^3]
+  const T* halo;       // device, [NF][np][(n+2g)^3] or nullptr (level 0)
+  const int* nbr;      // device, [np][27]
+  T* fblk;             // device flux blocks [nblk][3][NF][n^2 (n+1)] or nullptr
+  const int* fblk_of;  // device, [np] block index or -1 (nullptr if fblk is)
+  unsigned long long* counters;  // device [4]
+  void* smax;          // device, one T-sized slot (bit pattern ordered as unsigned), pre-zeroed
+  int np, n, g;
+  int ntx, nty, ntz, zc;  // tiles per patch along x,y,z; planes per z-chunk
+  T dtdx;              // dt/dx
+  T hdtdx;             // dt/(2 dx)
+  T gamma, gm1, igm1;
+  T ch, ch2, half_ich; // GLM speed, its square, 1/(2 ch)
+  T damp;              // exp(-alpha ch dt/dx)
+  T eps;               // HLLD degeneracy threshold (A7)
+};
+
+// launchers implemented in step_*.cu (one translation unit per (dtype, physics))
+cudaError_t launch_step_hydro_f32(const StepParams<float>& P, int limiter, int riemann, cudaStream_t s);
+cudaError_t launch_step_hydro_f64(const StepParams<double>& P, int limiter, int riemann, cudaStream_t s);
+cudaError_t launch_step_mhd_f32(const StepParams<float>& P, int limiter, int riemann, cudaStream_t s);
+cudaError_t launch_step_mhd_f64(const StepParams<double>& P, int limiter, int riemann, cudaStream_t s);
+// fills ntx/nty/ntz/zc for the tile shape the launcher of this variant uses
+void tile_shape_hydro_f32(int n, int* tx, int* ty);
+void tile_shape_hydro_f64(int n, int* tx, int* ty);
+void tile_shape_mhd_f32(int n, int* tx, int* ty);
+void tile_shape_mhd_f64(int n, int* tx, int* ty);
+
+// aux kernels (aux_kernels.cu); dtype: 0 = f32, 1 = f64
+cudaError_t launch_smax(int dtype, const void* U, int nf, int np, int n, double gamma, void* smax_slot,
+                        cudaStream_t s);
+constexpr int TOTALS_BLOCKS = 256;
+cudaError_t launch_totals(int dtype, const void* U, int nf, int np, int n, double* partials /*[nf][TOTALS_BLOCKS]*/,
+                          cudaStream_t s);
+// interiors [nf][np][n^3] (device) -> ghosted [nf][npc][(n+2g)^3] (device) for patches [p0, p0+npc)
+cudaError_t launch_gather_ghosted(int dtype, const void* U, const void* halo, const int* nbr, int nf, int np,
+                                  int n, int g, int p0, int npc, void* out, cudaStream_t s);
+// ghosted or interior host-layout staging (device) -> interiors
+cudaError_t launch_scatter_interior(int dtype, const void* staged, int with_ghosts, int nf, int np, int n, int g,
+                                    int p0, int npc, void* U, cudaStream_t s);
+cudaError_t launch_fill_nan(int dtype, void* ptr, size_t count, cudaStream_t s);
+
+// two-level kernels (aux_kernels.cu); table formats are documented at the kernels
+cudaError_t launch_prolong(int dtype, void* halo, size_t fs_halo, int nf, const long long* dst, const long long* c7,
+                           int ncells, const void* Ucold, const void* Ucnew, size_t fs_c, double theta,
+                           cudaStream_t s);
+cudaError_t launch_restrict(int dtype, const void* Uf, size_t fs_f, int nf, int n, const long long* dst, int nent,
+                            void* Uc, size_t fs_c, cudaStream_t s);
+cudaError_t launch_reflux(int dtype, void* Uc, size_t fs_c, int nf, int n, const long long* faces, int nfaces,
+                          const void* Fc, const void* Ff, double dtdx, cudaStream_t s);
+
+}  // namespace amr

@@ -1,0 +1,325 @@
+// Small kernels around the fused step: standalone CFL reduction (O7), conserved totals, ghosted
+// gather / interior scatter for upload/download (O0 as seen through the API), and the two-level
+// operators prolongation (O8), restriction and reflux (O9).  DESIGN.md §3, §6.
+#include <math_constants.h>
+
+#include "amr_internal.hpp"
+#include "signal_speed.cuh"
+
+namespace amr {
+
+namespace {
+
+template <class T> __device__ __forceinline__ void atomic_max_slot(void* slot, T v);
+template <> __device__ __forceinline__ void atomic_max_slot<float>(void* slot, float v) {
+  atomicMax(reinterpret_cast<unsigned int*>(slot), __float_as_uint(v));
+}
+template <> __device__ __forceinline__ void atomic_max_slot<double>(void* slot, double v) {
+  atomicMax(reinterpret_cast<unsigned long long*>(slot), (unsigned long long)__double_as_longlong(v));
+}
+
+// ---- O7 standalone: grid-stride over interior cells, warp-shuffle max, one atomic per CTA ----------
+template <class T, int NF>
+__global__ void __launch_bounds__(256) smax_kernel(const T* __restrict__ U, size_t ncell, T gamma, T gm1,
+                                                   void* slot) {
+  T m = T(0);
+  for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += (size_t)gridDim.x * blockDim.x) {
+    T u[NF];
+#pragma unroll
+    for (int q = 0; q < NF; ++q) u[q] = __ldg(U + (size_t)q * ncell + c);
+    m = max_(m, signal_speed<T, NF>(u, gamma, gm1));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = max_(m, __shfl_xor_sync(0xffffffffu, m, o));
+  __shared__ T red[8];
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    T r = red[0];
+    for (int w = 1; w < 8; ++w) r = max_(r, red[w]);
+    atomic_max_slot<T>(slot, r);
+  }
+}
+
+// ---- conserved totals: fixed grid, fixed per-thread order, tree reduce -> deterministic ------------
+template <class T>
+__global__ void __launch_bounds__(256) totals_kernel(const T* __restrict__ U, size_t ncell, double* partials) {
+  const int q = blockIdx.y;
+  const T* u = U + (size_t)q * ncell;
+  double s = 0.0;
+  for (size_t c = (size_t)blockIdx.x * 256 + threadIdx.x; c < ncell; c += (size_t)gridDim.x * 256) s += (double)u[c];
+  __shared__ double red[256];
+  red[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) partials[(size_t)q * gridDim.x + blockIdx.x] = red[0];
+}
+
+// ---- O0 through the API: ghosted copy of patches [p0, p0+npc) --------------------------------------
+template <class T>
+__global__ void __launch_bounds__(256) gather_ghosted_kernel(const T* __restrict__ U, const T* __restrict__ halo,
+                                                             const int* __restrict__ nbr, int nf, int np, int n,
+                                                             int g, int p0, int npc, T* __restrict__ out) {
+  const int M = n + 2 * g;
+  const size_t M3 = (size_t)M * M * M, n3 = (size_t)n * n * n;
+  const size_t total = (size_t)npc * M3;
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (size_t)gridDim.x * blockDim.x) {
+    const int pc = (int)(t / M3);
+    const size_t c = t - (size_t)pc * M3;
+    const int p = p0 + pc;
+    const int gz = (int)(c / ((size_t)M * M)), gy = (int)((c / M) % M), gx = (int)(c % M);
+    const int lx = gx - g, ly = gy - g, lz = gz - g;
+    const int rx = lx < 0 ? 0 : (lx >= n ? 2 : 1), ry = ly < 0 ? 0 : (ly >= n ? 2 : 1), rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
+    const int e = nbr[p * 27 + rz * 9 + ry * 3 + rx];
+    const T* src;
+    size_t fs;
+    if (e >= 0) {
+      const int sp = e & NBR_PATCH_MASK, md = e >> NBR_MODE_SHIFT;
+      const int sx = (rx != 1 && (md & 1)) ? (rx == 0 ? 0 : n - 1) : lx - (rx - 1) * n;
+      const int sy = (ry != 1 && (md & 2)) ? (ry == 0 ? 0 : n - 1) : ly - (ry - 1) * n;
+      const int sz = (rz != 1 && (md & 4)) ? (rz == 0 ? 0 : n - 1) : lz - (rz - 1) * n;
+      src = U + (size_t)sp * n3 + ((size_t)sz * n + sy) * n + sx;
+      fs = (size_t)np * n3;
+    } else {
+      src = halo + (size_t)p * M3 + c;
+      fs = (size_t)np * M3;
+    }
+    for (int q = 0; q < nf; ++q) out[((size_t)q * npc + pc) * M3 + c] = src[(size_t)q * fs];
+  }
+}
+
+template <class T>
+__global__ void __launch_bounds__(256) scatter_interior_kernel(const T* __restrict__ staged, int nf, int np, int n,
+                                                               int g, int p0, int npc, T* __restrict__ U) {
+  const int M = n + 2 * g;
+  const size_t M3 = (size_t)M * M * M, n3 = (size_t)n * n * n;
+  const size_t total = (size_t)npc * n3;
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (size_t)gridDim.x * blockDim.x) {
+    const int pc = (int)(t / n3);
+    const size_t c = t - (size_t)pc * n3;
+    const int k = (int)(c / ((size_t)n * n)), j = (int)((c / n) % n), i = (int)(c % n);
+    const size_t cg = ((size_t)(k + g) * M + (j + g)) * M + (i + g);
+    for (int q = 0; q < nf; ++q)
+      U[((size_t)q * np + p0 + pc) * n3 + c] = staged[((size_t)q * npc + pc) * M3 + cg];
+  }
+}
+
+template <class T>
+__global__ void fill_nan_kernel(T* ptr, size_t count) {
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < count; t += (size_t)gridDim.x * blockDim.x)
+    ptr[t] = (T)CUDART_NAN;
+}
+
+// ---- O8: prolongation into the fine halo ----------------------------------------------------------
+template <class T> __device__ __forceinline__ T minmod2(T a, T b) {
+  const T lo = a < b ? a : b, hi = a < b ? b : a;
+  return (lo > T(0) ? lo : T(0)) + (hi < T(0) ? hi : T(0));
+}
+
+// dst[e]: flat index into one field of the halo buffer (bit 62..60 = parity x,y,z of the fine cell
+// inside its coarse cell).  c7[e][7]: flat coarse interior indices: centre, x-, x+, y-, y+, z-, z+.
+template <class T>
+__global__ void __launch_bounds__(256) prolong_kernel(T* __restrict__ halo, size_t fs_halo, int nf,
+                                                      const long long* __restrict__ dst,
+                                                      const long long* __restrict__ c7, int ncells,
+                                                      const T* __restrict__ Uold, const T* __restrict__ Unew,
+                                                      size_t fs_c, T theta) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= ncells) return;
+  const long long dcode = dst[e];
+  const size_t d = (size_t)(dcode & ((1LL << 60) - 1));
+  const int par = (int)(dcode >> 60) & 7;
+  long long s[7];
+#pragma unroll
+  for (int k = 0; k < 7; ++k) s[k] = c7[(size_t)e * 7 + k];
+  const T w0 = T(1) - theta;
+  for (int q = 0; q < nf; ++q) {
+    const T* a = Uold + (size_t)q * fs_c;
+    const T* b = Unew + (size_t)q * fs_c;
+    T st[7];
+#pragma unroll
+    for (int k = 0; k < 7; ++k) st[k] = w0 * a[s[k]] + theta * b[s[k]];
+    T val = st[0];
+#pragma unroll
+    for (int dd = 0; dd < 3; ++dd) {
+      const T sl = minmod2<T>(st[0] - st[1 + 2 * dd], st[2 + 2 * dd] - st[0]);
+      val += (((par >> dd) & 1) ? T(0.25) : T(-0.25)) * sl;
+    }
+    halo[(size_t)q * fs_halo + d] = val;
+  }
+}
+
+// ---- O9(6): restriction ---------------------------------------------------------------------------
+// entry e <-> (fine patch p, coarse-cell offset inside the patch); dst[e] = flat coarse interior index
+template <class T>
+__global__ void __launch_bounds__(256) restrict_kernel(const T* __restrict__ Uf, size_t fs_f, int nf, int n,
+                                                       const long long* __restrict__ dst, int nent,
+                                                       T* __restrict__ Uc, size_t fs_c) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= nent) return;
+  const int h = n / 2, h3 = h * h * h;
+  const int p = e / h3;
+  int r = e - p * h3;
+  const int ck = r / (h * h);
+  r -= ck * h * h;
+  const int cj = r / h, ci = r - cj * h;
+  const size_t base = (size_t)p * n * n * n + ((size_t)(2 * ck) * n + 2 * cj) * n + 2 * ci;
+  const size_t d = (size_t)dst[e];
+  for (int q = 0; q < nf; ++q) {
+    const T* u = Uf + (size_t)q * fs_f + base;
+    T s = T(0);
+#pragma unroll
+    for (int dk = 0; dk < 2; ++dk)
+#pragma unroll
+      for (int dj = 0; dj < 2; ++dj)
+#pragma unroll
+        for (int di = 0; di < 2; ++di) s += u[((size_t)dk * n + dj) * n + di];
+    Uc[(size_t)q * fs_c + d] = s * T(0.125);
+  }
+}
+
+// ---- O9(7): reflux --------------------------------------------------------------------------------
+// faces[e][4] = { flat coarse interior index of the cell to correct,
+//                 flat offset of the coarse flux inside field 0 of the coarse flux-block array,
+//                 flat offset of the first of the 4 fine fluxes inside field 0 of the fine flux-block array,
+//                 code: bit0 = sign (1: s_f = -1), bits 1..2 = d }.
+// blk_stride_*: elements between fields inside one (block, d) slab = n^2 (n+1).
+template <class T>
+__global__ void __launch_bounds__(256) reflux_kernel(T* __restrict__ Uc, size_t fs_c, int nf, int n,
+                                                     const long long* __restrict__ faces, int nfaces,
+                                                     const T* __restrict__ Fc, const T* __restrict__ Ff, T dtdx) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= nfaces) return;
+  const size_t cell = (size_t)faces[(size_t)e * 4 + 0];
+  const size_t oc = (size_t)faces[(size_t)e * 4 + 1];
+  const size_t of = (size_t)faces[(size_t)e * 4 + 2];
+  const int code = (int)faces[(size_t)e * 4 + 3];
+  const T sf = (code & 1) ? T(-1) : T(1);
+  const int d = (code >> 1) & 3;
+  const size_t fsz = (size_t)n * n * (n + 1);
+  // strides of the two transverse directions t1 = (d+1)%3 (a), t2 = (d+2)%3 (b) inside a d-slab
+  // slab extents: (z, y, x) with n+1 along d
+  size_t sx = 1, sy, sz;
+  if (d == 0) { sy = n + 1; sz = (size_t)n * (n + 1); }
+  else if (d == 1) { sy = n; sz = (size_t)n * (n + 1); }
+  else { sy = n; sz = (size_t)n * n; }
+  const size_t str3[3] = {sx, sy, sz};
+  const size_t sa = str3[(d + 1) % 3], sb = str3[(d + 2) % 3];
+  for (int q = 0; q < nf; ++q) {
+    const T Fcoarse = Fc[oc + (size_t)q * fsz];
+    const T* f = Ff + of + (size_t)q * fsz;
+    T sum = T(0);
+    sum += f[0];
+    sum += f[sa];
+    sum += f[sb];
+    sum += f[sa + sb];
+    const T Ffine = T(0.25) * T(0.5) * sum;
+    Uc[(size_t)q * fs_c + cell] += sf * dtdx * (Fcoarse - Ffine);
+  }
+}
+
+inline unsigned grid_for(size_t work, int block, unsigned cap = 148 * 16) {
+  size_t g = (work + block - 1) / block;
+  if (g < 1) g = 1;
+  if (g > cap) g = cap;
+  return (unsigned)g;
+}
+
+}  // namespace
+
+cudaError_t launch_smax(int dtype, const void* U, int nf, int np, int n, double gamma, void* slot, cudaStream_t s) {
+  const size_t ncell = (size_t)np * n * n * n;
+  const unsigned grid = grid_for(ncell, 256, 148 * 8);
+  if (dtype == 0) {
+    const float g = (float)gamma, gm1 = (float)(gamma - 1.0);
+    if (nf == 5) smax_kernel<float, 5><<<grid, 256, 0, s>>>((const float*)U, ncell, g, gm1, slot);
+    else smax_kernel<float, 9><<<grid, 256, 0, s>>>((const float*)U, ncell, g, gm1, slot);
+  } else {
+    const double g = gamma, gm1 = gamma - 1.0;
+    if (nf == 5) smax_kernel<double, 5><<<grid, 256, 0, s>>>((const double*)U, ncell, g, gm1, slot);
+    else smax_kernel<double, 9><<<grid, 256, 0, s>>>((const double*)U, ncell, g, gm1, slot);
+  }
+  return cudaGetLastError();
+}
+
+cudaError_t launch_totals(int dtype, const void* U, int nf, int np, int n, double* partials, cudaStream_t s) {
+  const size_t ncell = (size_t)np * n * n * n;
+  dim3 grid(TOTALS_BLOCKS, nf);
+  if (dtype == 0) totals_kernel<float><<<grid, 256, 0, s>>>((const float*)U, ncell, partials);
+  else totals_kernel<double><<<grid, 256, 0, s>>>((const double*)U, ncell, partials);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_gather_ghosted(int dtype, const void* U, const void* halo, const int* nbr, int nf, int np, int n,
+                                  int g, int p0, int npc, void* out, cudaStream_t s) {
+  const int M = n + 2 * g;
+  const unsigned grid = grid_for((size_t)npc * M * M * M, 256);
+  if (dtype == 0)
+    gather_ghosted_kernel<float><<<grid, 256, 0, s>>>((const float*)U, (const float*)halo, nbr, nf, np, n, g, p0, npc,
+                                                     (float*)out);
+  else
+    gather_ghosted_kernel<double><<<grid, 256, 0, s>>>((const double*)U, (const double*)halo, nbr, nf, np, n, g, p0,
+                                                      npc, (double*)out);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_scatter_interior(int dtype, const void* staged, int with_ghosts, int nf, int np, int n, int g,
+                                    int p0, int npc, void* U, cudaStream_t s) {
+  const unsigned grid = grid_for((size_t)npc * n * n * n, 256);
+  const int ge = with_ghosts ? g : 0;
+  if (dtype == 0)
+    scatter_interior_kernel<float><<<grid, 256, 0, s>>>((const float*)staged, nf, np, n, ge, p0, npc, (float*)U);
+  else
+    scatter_interior_kernel<double><<<grid, 256, 0, s>>>((const double*)staged, nf, np, n, ge, p0, npc, (double*)U);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_fill_nan(int dtype, void* ptr, size_t count, cudaStream_t s) {
+  const unsigned grid = grid_for(count, 256);
+  if (dtype == 0) fill_nan_kernel<float><<<grid, 256, 0, s>>>((float*)ptr, count);
+  else fill_nan_kernel<double><<<grid, 256, 0, s>>>((double*)ptr, count);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_prolong(int dtype, void* halo, size_t fs_halo, int nf, const long long* dst, const long long* c7,
+                           int ncells, const void* Ucold, const void* Ucnew, size_t fs_c, double theta,
+                           cudaStream_t s) {
+  if (ncells == 0) return cudaSuccess;
+  const unsigned grid = (unsigned)((ncells + 255) / 256);
+  if (dtype == 0)
+    prolong_kernel<float><<<grid, 256, 0, s>>>((float*)halo, fs_halo, nf, dst, c7, ncells, (const float*)Ucold,
+                                              (const float*)Ucnew, fs_c, (float)theta);
+  else
+    prolong_kernel<double><<<grid, 256, 0, s>>>((double*)halo, fs_halo, nf, dst, c7, ncells, (const double*)Ucold,
+                                               (const double*)Ucnew, fs_c, theta);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_restrict(int dtype, const void* Uf, size_t fs_f, int nf, int n, const long long* dst, int nent,
+                            void* Uc, size_t fs_c, cudaStream_t s) {
+  if (nent == 0) return cudaSuccess;
+  const unsigned grid = (unsigned)((nent + 255) / 256);
+  if (dtype == 0)
+    restrict_kernel<float><<<grid, 256, 0, s>>>((const float*)Uf, fs_f, nf, n, dst, nent, (float*)Uc, fs_c);
+  else
+    restrict_kernel<double><<<grid, 256, 0, s>>>((const double*)Uf, fs_f, nf, n, dst, nent, (double*)Uc, fs_c);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_reflux(int dtype, void* Uc, size_t fs_c, int nf, int n, const long long* faces, int nfaces,
+                          const void* Fc, const void* Ff, double dtdx, cudaStream_t s) {
+  if (nfaces == 0) return cudaSuccess;
+  const unsigned grid = (unsigned)((nfaces + 255) / 256);
+  if (dtype == 0)
+    reflux_kernel<float><<<grid, 256, 0, s>>>((float*)Uc, fs_c, nf, n, faces, nfaces, (const float*)Fc,
+                                             (const float*)Ff, (float)dtdx);
+  else
+    reflux_kernel<double><<<grid, 256, 0, s>>>((double*)Uc, fs_c, nf, n, faces, nfaces, (const double*)Fc,
+                                              (const double*)Ff, dtdx);
+  return cudaGetLastError();
+}
+
+}  // namespace amr

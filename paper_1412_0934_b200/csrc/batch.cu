@@ -1,0 +1,721 @@
+// Host side of libamrgodunov.so: the C-ABI of include/amr_godunov.h.  Batch object, arena carving,
+// neighbour / coarse-fine tables (the "hierarchy and ghost-fill metadata kept on the host" of
+// BASELINE.json:north_star), launches.  No solver arithmetic lives here.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/amr_godunov.h"
+#include "amr_internal.hpp"
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char* fmt, ...) __attribute__((format(printf, 2, 3)));
+int fail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return code;
+}
+
+#define CUDA_TRY(expr)                                                                         \
+  do {                                                                                         \
+    cudaError_t e_ = (expr);                                                                   \
+    if (e_ != cudaSuccess) return fail(AMR_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_));    \
+  } while (0)
+
+constexpr size_t ALIGN = 256;
+inline size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Layout {
+  size_t U[2], halo, nbr, fblk_of, counters, smax, partials, total;
+};
+
+bool desc_ok(const amr_batch_desc* d, std::string* why) {
+  auto bad = [&](const char* m) { if (why) *why = m; return false; };
+  if (!d) return bad("null desc");
+  if (d->npatch < 1 || d->npatch > amr::NBR_PATCH_MASK) return bad("npatch out of range");
+  if (d->n < 8 || d->n > 64 || d->n % 8) return bad("n must be a multiple of 8 in [8,64]");
+  if (d->nghost < 2 || d->nghost > 4) return bad("nghost must be 2..4");
+  if (d->nfields != 5 && d->nfields != 9) return bad("nfields must be 5 (hydro) or 9 (MHD)");
+  if (d->dtype != AMR_F32 && d->dtype != AMR_F64) return bad("dtype must be AMR_F32 or AMR_F64");
+  if (!(d->dx > 0) || !std::isfinite(d->dx)) return bad("dx must be finite and > 0");
+  if (d->level < 0) return bad("level < 0");
+  if ((double)d->npatch * d->n * d->n * d->n > 2.0e9) return bad("more than 2e9 cells in one batch");
+  if (!d->self_periodic) {
+    if (!d->origin) return bad("null origin");
+    for (int a = 0; a < 3; ++a)
+      if (d->domain_cells[a] < d->n || d->domain_cells[a] % d->n) return bad("domain_cells must be multiples of n");
+    for (int a = 0; a < 6; ++a)
+      if (d->bc[a] != AMR_BC_PERIODIC && d->bc[a] != AMR_BC_OUTFLOW) return bad("unknown boundary condition");
+  }
+  return true;
+}
+
+Layout make_layout(const amr_batch_desc* d) {
+  Layout L;
+  const size_t esz = d->dtype == AMR_F64 ? 8 : 4;
+  const size_t n3 = (size_t)d->n * d->n * d->n;
+  const size_t M = d->n + 2 * d->nghost, M3 = M * M * M;
+  size_t off = 0;
+  for (int b = 0; b < 2; ++b) { L.U[b] = off; off += up((size_t)d->nfields * d->npatch * n3 * esz); }
+  L.halo = off;
+  if (d->level > 0) off += up((size_t)d->nfields * d->npatch * M3 * esz);
+  L.nbr = off; off += up((size_t)d->npatch * 27 * sizeof(int));
+  L.fblk_of = off; off += up((size_t)d->npatch * sizeof(int));
+  L.counters = off; off += up(4 * sizeof(unsigned long long));
+  L.smax = off; off += up(16);
+  L.partials = off; off += up((size_t)d->nfields * amr::TOTALS_BLOCKS * sizeof(double));
+  L.total = off;
+  return L;
+}
+
+// dense map patch-grid coordinate -> patch index (-1: none)
+struct PatchMap {
+  int dims[3];
+  std::vector<int> idx;
+  int at(int a, int b, int c) const { return idx[((size_t)c * dims[1] + b) * dims[0] + a]; }
+};
+
+}  // namespace
+
+struct amr_patch_batch {
+  amr_batch_desc d;
+  std::vector<int32_t> origin;
+  std::vector<int> nbr_host;
+  PatchMap map;
+  cudaStream_t stream;
+  char* arena;
+  size_t bytes, esz, n3, M3;
+  void* U[2];
+  int cur;
+  void* halo;
+  int* nbr_dev;
+  int* fblk_of;  // device [np]; owned here, filled by a link
+  void* fblk;    // device flux blocks, owned by a link (nullptr: no recording)
+  unsigned long long* counters;
+  void* smax_slot;
+  double* partials;
+  bool needs_halo, halo_valid;
+  bool smax_valid;
+  double smax_gamma;
+  amr_level_link* link;
+};
+
+struct amr_level_link {
+  amr_patch_batch *c, *f;
+  char* ws;
+  size_t bytes;
+  long long *pro_dst, *pro_c7;
+  int npro;
+  long long* res_dst;
+  int nres;
+  long long* faces[6];
+  int nfaces[6];
+  void *fblk_c, *fblk_f;
+  size_t fblk_c_bytes, fblk_f_bytes;
+  int nblk_c;
+};
+
+namespace {
+
+struct LinkHost {
+  std::vector<long long> pro_dst, pro_c7, res_dst, faces[6];
+  std::vector<int> fblk_of_c;
+  int nblk_c = 0;
+};
+
+struct LinkLayout {
+  size_t pro_dst, pro_c7, res_dst, faces[6], fblk_c, fblk_f, total, fblk_c_bytes, fblk_f_bytes;
+};
+
+int wrapi(int v, int m) { return ((v % m) + m) % m; }
+
+// Host tables for O8 / O9 (restated from DESIGN.md §3; index conventions of include/amr_godunov.h).
+int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) {
+  const int n = f->d.n, g = f->d.nghost, M = n + 2 * g, nc = n / 2;
+  const size_t n3 = (size_t)n * n * n, M3 = (size_t)M * M * M;
+  const int* domf = f->d.domain_cells;
+  const int* domc = c->d.domain_cells;
+  auto coarse_flat = [&](int Cx, int Cy, int Cz, long long* out) -> bool {
+    int C[3] = {Cx, Cy, Cz};
+    for (int a = 0; a < 3; ++a) {
+      if (C[a] < 0) C[a] = (c->d.bc[2 * a] == AMR_BC_PERIODIC) ? C[a] + domc[a] : 0;
+      else if (C[a] >= domc[a]) C[a] = (c->d.bc[2 * a + 1] == AMR_BC_PERIODIC) ? C[a] - domc[a] : domc[a] - 1;
+    }
+    const int pc = c->map.at(C[0] / n, C[1] / n, C[2] / n);
+    if (pc < 0) return false;
+    const int* oc = &c->origin[3 * pc];
+    *out = (long long)pc * (long long)n3 + ((long long)(C[2] - oc[2]) * n + (C[1] - oc[1])) * n + (C[0] - oc[0]);
+    return true;
+  };
+  // O8 list: fine halo cells in regions no sibling covers
+  for (int p = 0; p < f->d.npatch; ++p) {
+    const int* o = &f->origin[3 * p];
+    for (int k = -g; k < n + g; ++k)
+      for (int j = -g; j < n + g; ++j)
+        for (int i = -g; i < n + g; ++i) {
+          const int rx = i < 0 ? 0 : (i >= n ? 2 : 1), ry = j < 0 ? 0 : (j >= n ? 2 : 1), rz = k < 0 ? 0 : (k >= n ? 2 : 1);
+          if (rx == 1 && ry == 1 && rz == 1) continue;
+          if (f->nbr_host[(size_t)p * 27 + rz * 9 + ry * 3 + rx] != amr::NBR_FROM_HALO) continue;
+          int gi[3] = {o[0] + i, o[1] + j, o[2] + k};
+          long long par = 0;
+          for (int a = 0; a < 3; ++a) {
+            par |= (long long)wrapi(gi[a], 2) << a;
+            gi[a] = wrapi(gi[a], domf[a]);
+          }
+          const int C[3] = {gi[0] / 2, gi[1] / 2, gi[2] / 2};
+          long long s7[7];
+          bool ok = coarse_flat(C[0], C[1], C[2], &s7[0]);
+          for (int a = 0; a < 3 && ok; ++a) {
+            int Cm[3] = {C[0], C[1], C[2]}, Cp[3] = {C[0], C[1], C[2]};
+            Cm[a] -= 1;
+            Cp[a] += 1;
+            ok = coarse_flat(Cm[0], Cm[1], Cm[2], &s7[1 + 2 * a]) && coarse_flat(Cp[0], Cp[1], Cp[2], &s7[2 + 2 * a]);
+          }
+          if (!ok) return fail(AMR_EINVAL, "fine patch %d has a halo cell with no coarse parent", p);
+          const long long cell = (long long)p * (long long)M3 + ((long long)(k + g) * M + (j + g)) * M + (i + g);
+          H.pro_dst.push_back(cell | (par << 60));
+          for (int q = 0; q < 7; ++q) H.pro_c7.push_back(s7[q]);
+        }
+  }
+  // O9(6) list: entry e = (p, ck, cj, ci)
+  for (int p = 0; p < f->d.npatch; ++p) {
+    const int* o = &f->origin[3 * p];
+    for (int ck = 0; ck < nc; ++ck)
+      for (int cj = 0; cj < nc; ++cj)
+        for (int ci = 0; ci < nc; ++ci) {
+          long long flat;
+          if (!coarse_flat(o[0] / 2 + ci, o[1] / 2 + cj, o[2] / 2 + ck, &flat))
+            return fail(AMR_EINVAL, "fine patch %d is not covered by a coarse patch", p);
+          H.res_dst.push_back(flat);
+        }
+  }
+  // O9(7) list, one per (d, side) so that no coarse cell appears twice in a launch
+  H.fblk_of_c.assign(c->d.npatch, -1);
+  const long long fsz = (long long)n * n * (n + 1);
+  const int NF = f->d.nfields;
+  auto slab_off = [&](int d, const int l[3]) -> long long {  // l = (x,y,z) with face index along d
+    if (d == 0) return ((long long)l[2] * n + l[1]) * (n + 1) + l[0];
+    if (d == 1) return ((long long)l[2] * (n + 1) + l[1]) * n + l[0];
+    return ((long long)l[2] * n + l[1]) * n + l[0];
+  };
+  for (int p = 0; p < f->d.npatch; ++p) {
+    const int* o = &f->origin[3 * p];
+    for (int d = 0; d < 3; ++d)
+      for (int side = 0; side < 2; ++side) {
+        const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+        for (int b = 0; b < nc; ++b)
+          for (int a = 0; a < nc; ++a) {
+            int Cin[3];
+            Cin[d] = o[d] / 2 + (side ? nc : -1);
+            Cin[t1] = o[t1] / 2 + a;
+            Cin[t2] = o[t2] / 2 + b;
+            int C[3];
+            for (int e = 0; e < 3; ++e) C[e] = wrapi(Cin[e], domc[e]);
+            if (f->map.at(2 * C[0] / n, 2 * C[1] / n, 2 * C[2] / n) >= 0) continue;  // fine-fine face
+            const int pc = c->map.at(C[0] / n, C[1] / n, C[2] / n);
+            if (pc < 0) return fail(AMR_EINVAL, "no coarse patch next to fine patch %d", p);
+            const int* oc = &c->origin[3 * pc];
+            int lc[3] = {C[0] - oc[0], C[1] - oc[1], C[2] - oc[2]};
+            const long long cell = (long long)pc * (long long)n3 + ((long long)lc[2] * n + lc[1]) * n + lc[0];
+            if (H.fblk_of_c[pc] < 0) H.fblk_of_c[pc] = H.nblk_c++;
+            int lface[3] = {lc[0], lc[1], lc[2]};
+            if (!side) lface[d] += 1;  // upper face of the outside cell
+            const long long oc_off = ((long long)H.fblk_of_c[pc] * 3 + d) * NF * fsz + slab_off(d, lface);
+            int lf[3];
+            lf[d] = side ? n : 0;
+            lf[t1] = 2 * a;
+            lf[t2] = 2 * b;
+            const long long of_off = ((long long)p * 3 + d) * NF * fsz + slab_off(d, lf);
+            auto& v = H.faces[d * 2 + side];
+            v.push_back(cell);
+            v.push_back(oc_off);
+            v.push_back(of_off);
+            v.push_back((long long)(side ? 1 : 0) | ((long long)d << 1));
+          }
+      }
+  }
+  return AMR_OK;
+}
+
+LinkLayout make_link_layout(const amr_patch_batch* c, const amr_patch_batch* f, const LinkHost& H) {
+  LinkLayout L;
+  size_t off = 0;
+  L.pro_dst = off; off += up(H.pro_dst.size() * 8 + 8);
+  L.pro_c7 = off; off += up(H.pro_c7.size() * 8 + 8);
+  L.res_dst = off; off += up(H.res_dst.size() * 8 + 8);
+  for (int s = 0; s < 6; ++s) { L.faces[s] = off; off += up(H.faces[s].size() * 8 + 8); }
+  const size_t n = f->d.n, blk = 3 * (size_t)f->d.nfields * n * n * (n + 1) * f->esz;
+  L.fblk_c_bytes = (size_t)H.nblk_c * blk;
+  L.fblk_f_bytes = (size_t)f->d.npatch * blk;
+  L.fblk_c = off; off += up(L.fblk_c_bytes + 8);
+  L.fblk_f = off; off += up(L.fblk_f_bytes + 8);
+  L.total = off;
+  (void)c;
+  return L;
+}
+
+int check_link_args(const amr_patch_batch* c, const amr_patch_batch* f, int ratio) {
+  if (!c || !f) return fail(AMR_EINVAL, "null batch");
+  if (ratio != 2) return fail(AMR_EINVAL, "only refinement ratio 2 is supported");
+  if (c->d.n != f->d.n || c->d.nfields != f->d.nfields || c->d.dtype != f->d.dtype || c->d.nghost != f->d.nghost)
+    return fail(AMR_EINVAL, "coarse and fine batches must agree in n, nfields, dtype, nghost");
+  if (c->d.self_periodic || f->d.self_periodic) return fail(AMR_EINVAL, "self-periodic batches cannot be linked");
+  if (c->stream != f->stream) return fail(AMR_EINVAL, "linked batches must have been created on the same stream");
+  if (f->d.level != c->d.level + 1) return fail(AMR_EINVAL, "fine.level must be coarse.level + 1");
+  for (int a = 0; a < 3; ++a)
+    if (f->d.domain_cells[a] != 2 * c->d.domain_cells[a]) return fail(AMR_EINVAL, "fine domain must be 2x the coarse domain");
+  return AMR_OK;
+}
+
+template <class T>
+amr::StepParams<T> make_params(amr_patch_batch* b, double dt, double gamma, double ch, double alpha) {
+  amr::StepParams<T> P;
+  std::memset(&P, 0, sizeof P);
+  P.Uin = (const T*)b->U[b->cur];
+  P.Uout = (T*)b->U[1 - b->cur];
+  P.halo = (const T*)b->halo;
+  P.nbr = b->nbr_dev;
+  P.fblk = (T*)b->fblk;
+  P.fblk_of = b->fblk ? b->fblk_of : nullptr;
+  P.counters = b->counters;
+  P.smax = b->smax_slot;
+  P.np = b->d.npatch;
+  P.n = b->d.n;
+  P.g = b->d.nghost;
+  const T dtT = (T)dt, dxT = (T)b->d.dx;
+  P.dtdx = dtT / dxT;
+  P.hdtdx = dtT / (T(2) * dxT);
+  P.gamma = (T)gamma;
+  P.gm1 = P.gamma - T(1);
+  P.igm1 = T(1) / P.gm1;
+  P.ch = (T)ch;
+  P.ch2 = P.ch * P.ch;
+  P.half_ich = ch > 0 ? T(1) / (T(2) * P.ch) : T(0);
+  P.damp = (T)std::exp(-alpha * ch * dt / b->d.dx);
+  P.eps = (T)(sizeof(T) == 8 ? 1e-12 : 1e-6);
+  return P;
+}
+
+int do_step(amr_patch_batch* b, bool mhd, double dt, double gamma, int limiter, int riemann, double ch, double alpha) {
+  if (!b) return fail(AMR_EINVAL, "null batch");
+  if (mhd != (b->d.nfields == 9))
+    return fail(AMR_EINVAL, "%s step on a batch with %d fields", mhd ? "MHD" : "hydro", b->d.nfields);
+  if (!(dt > 0) || !std::isfinite(dt)) return fail(AMR_EINVAL, "dt must be finite and > 0");
+  if (!std::isfinite(gamma) || !(gamma > 1)) return fail(AMR_EINVAL, "gamma must be finite and > 1");
+  if (limiter < AMR_LIM_NONE || limiter > AMR_LIM_MC) return fail(AMR_EINVAL, "unknown limiter %d", limiter);
+  if (mhd) {
+    if (riemann != AMR_RS_HLL && riemann != AMR_RS_HLLD) return fail(AMR_EINVAL, "MHD step takes HLL or HLLD");
+    if (!(ch > 0) || !std::isfinite(ch)) return fail(AMR_EINVAL, "ch must be finite and > 0");
+    if (!(alpha >= 0) || !std::isfinite(alpha)) return fail(AMR_EINVAL, "alpha must be finite and >= 0");
+  } else if (riemann != AMR_RS_HLL && riemann != AMR_RS_HLLC) {
+    return fail(AMR_EINVAL, "hydro step takes HLL or HLLC");
+  }
+  if (b->needs_halo && !b->halo_valid)
+    return fail(AMR_ESTATE, "level-%d batch has coarse-fine halo regions but amr_prolong_ghosts was never called", b->d.level);
+  CUDA_TRY(cudaMemsetAsync(b->smax_slot, 0, 16, b->stream));
+  cudaError_t e;
+  int tx = 0, ty = 0;
+  if (b->d.dtype == AMR_F32) {
+    amr::StepParams<float> P = make_params<float>(b, dt, gamma, ch, alpha);
+    if (mhd) amr::tile_shape_mhd_f32(P.n, &tx, &ty); else amr::tile_shape_hydro_f32(P.n, &tx, &ty);
+    P.ntx = P.n / tx; P.nty = P.n / ty; P.ntz = 1; P.zc = P.n;
+    e = mhd ? amr::launch_step_mhd_f32(P, limiter, riemann, b->stream)
+            : amr::launch_step_hydro_f32(P, limiter, riemann, b->stream);
+  } else {
+    amr::StepParams<double> P = make_params<double>(b, dt, gamma, ch, alpha);
+    if (mhd) amr::tile_shape_mhd_f64(P.n, &tx, &ty); else amr::tile_shape_hydro_f64(P.n, &tx, &ty);
+    P.ntx = P.n / tx; P.nty = P.n / ty; P.ntz = 1; P.zc = P.n;
+    e = mhd ? amr::launch_step_mhd_f64(P, limiter, riemann, b->stream)
+            : amr::launch_step_hydro_f64(P, limiter, riemann, b->stream);
+  }
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "step kernel launch: %s", cudaGetErrorString(e));
+  b->cur = 1 - b->cur;
+  b->smax_valid = true;
+  b->smax_gamma = gamma;
+  return AMR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* amr_last_error(void) { return g_err.c_str(); }
+const char* amr_version(void) { return "amr_godunov 0.1 (sm_100a; fused MUSCL-Hancock/HLLC/HLLD step, interiors-only SoA arena)"; }
+
+size_t amr_patch_batch_bytes(const amr_batch_desc* desc) {
+  std::string why;
+  if (!desc_ok(desc, &why)) { fail(AMR_EINVAL, "%s", why.c_str()); return 0; }
+  return make_layout(desc).total;
+}
+
+int amr_patch_batch_create(const amr_batch_desc* desc, void* dev_arena, size_t bytes, void* cuda_stream,
+                           amr_patch_batch** out) {
+  if (!out) return fail(AMR_EINVAL, "null out");
+  *out = nullptr;
+  std::string why;
+  if (!desc_ok(desc, &why)) return fail(AMR_EINVAL, "%s", why.c_str());
+  if (!dev_arena) return fail(AMR_EINVAL, "null device arena");
+  if ((uintptr_t)dev_arena % ALIGN) return fail(AMR_EINVAL, "device arena must be %zu-byte aligned", ALIGN);
+  const Layout L = make_layout(desc);
+  if (bytes < L.total) return fail(AMR_EINVAL, "arena too small: %zu < %zu bytes", bytes, L.total);
+
+  amr_patch_batch* b = new (std::nothrow) amr_patch_batch();
+  if (!b) return fail(AMR_ENOMEM, "out of host memory");
+  b->d = *desc;
+  b->d.origin = nullptr;
+  const int np = desc->npatch, n = desc->n;
+  b->origin.assign((size_t)np * 3, 0);
+  if (desc->self_periodic) {
+    for (int a = 0; a < 3; ++a) b->d.domain_cells[a] = n;
+    for (int a = 0; a < 6; ++a) b->d.bc[a] = AMR_BC_PERIODIC;
+  } else {
+    std::memcpy(b->origin.data(), desc->origin, (size_t)np * 3 * sizeof(int32_t));
+  }
+  // neighbour table (O0 rules (i) sibling copy with periodic wrap, (ii) outflow clamp)
+  b->nbr_host.assign((size_t)np * 27, 0);
+  b->needs_halo = false;
+  if (desc->self_periodic) {
+    for (int p = 0; p < np; ++p)
+      for (int r = 0; r < 27; ++r) b->nbr_host[(size_t)p * 27 + r] = p;
+    b->map.dims[0] = b->map.dims[1] = b->map.dims[2] = 1;
+    b->map.idx.assign(1, 0);
+  } else {
+    PatchMap& m = b->map;
+    for (int a = 0; a < 3; ++a) m.dims[a] = desc->domain_cells[a] / n;
+    m.idx.assign((size_t)m.dims[0] * m.dims[1] * m.dims[2], -1);
+    for (int p = 0; p < np; ++p) {
+      const int32_t* o = &b->origin[3 * p];
+      for (int a = 0; a < 3; ++a)
+        if (o[a] < 0 || o[a] % n || o[a] + n > desc->domain_cells[a]) {
+          delete b;
+          return fail(AMR_EINVAL, "origin of patch %d is not a multiple of n inside the domain", p);
+        }
+      int& slot = m.idx[((size_t)(o[2] / n) * m.dims[1] + o[1] / n) * m.dims[0] + o[0] / n];
+      if (slot >= 0) { delete b; return fail(AMR_EINVAL, "patches %d and %d coincide", slot, p); }
+      slot = p;
+    }
+    for (int p = 0; p < np; ++p) {
+      const int32_t* o = &b->origin[3 * p];
+      const int pc[3] = {o[0] / n, o[1] / n, o[2] / n};
+      for (int r = 0; r < 27; ++r) {
+        const int rr[3] = {r % 3, (r / 3) % 3, r / 9};
+        int q[3], mode = 0;
+        for (int a = 0; a < 3; ++a) {
+          q[a] = pc[a] + rr[a] - 1;
+          if (q[a] < 0) {
+            if (desc->bc[2 * a] == AMR_BC_PERIODIC) q[a] += m.dims[a]; else { q[a] = 0; mode |= 1 << a; }
+          } else if (q[a] >= m.dims[a]) {
+            if (desc->bc[2 * a + 1] == AMR_BC_PERIODIC) q[a] -= m.dims[a]; else { q[a] = m.dims[a] - 1; mode |= 1 << a; }
+          }
+        }
+        const int src = m.at(q[0], q[1], q[2]);
+        int e;
+        if (src >= 0) e = src | (mode << amr::NBR_MODE_SHIFT);
+        else if (desc->level > 0) { e = amr::NBR_FROM_HALO; b->needs_halo = true; }
+        else { delete b; return fail(AMR_EINVAL, "root-level patch %d has no neighbour in region %d", p, r); }
+        b->nbr_host[(size_t)p * 27 + r] = e;
+      }
+    }
+  }
+  b->stream = (cudaStream_t)cuda_stream;
+  b->arena = (char*)dev_arena;
+  b->bytes = bytes;
+  b->esz = desc->dtype == AMR_F64 ? 8 : 4;
+  b->n3 = (size_t)n * n * n;
+  const size_t M = n + 2 * desc->nghost;
+  b->M3 = M * M * M;
+  b->U[0] = b->arena + L.U[0];
+  b->U[1] = b->arena + L.U[1];
+  b->cur = 0;
+  b->halo = desc->level > 0 ? b->arena + L.halo : nullptr;
+  b->nbr_dev = (int*)(b->arena + L.nbr);
+  b->fblk_of = (int*)(b->arena + L.fblk_of);
+  b->fblk = nullptr;
+  b->counters = (unsigned long long*)(b->arena + L.counters);
+  b->smax_slot = b->arena + L.smax;
+  b->partials = (double*)(b->arena + L.partials);
+  b->halo_valid = false;
+  b->smax_valid = false;
+  b->smax_gamma = 0;
+  b->link = nullptr;
+  auto bail = [&](cudaError_t e, const char* what) {
+    delete b;
+    return fail(AMR_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+  };
+  cudaError_t e = cudaMemcpyAsync(b->nbr_dev, b->nbr_host.data(), (size_t)np * 27 * sizeof(int), cudaMemcpyHostToDevice, b->stream);
+  if (e != cudaSuccess) return bail(e, "upload of the neighbour table");
+  e = cudaMemsetAsync(b->counters, 0, 4 * sizeof(unsigned long long), b->stream);
+  if (e != cudaSuccess) return bail(e, "cudaMemsetAsync");
+  e = cudaMemsetAsync(b->fblk_of, 0xff, (size_t)np * sizeof(int), b->stream);
+  if (e != cudaSuccess) return bail(e, "cudaMemsetAsync");
+  if (b->halo) {
+    e = amr::launch_fill_nan(desc->dtype, b->halo, (size_t)desc->nfields * np * b->M3, b->stream);
+    if (e != cudaSuccess) return bail(e, "halo initialisation");
+  }
+  e = cudaStreamSynchronize(b->stream);  // nbr_host stays alive, but report upload errors here
+  if (e != cudaSuccess) return bail(e, "cudaStreamSynchronize");
+  *out = b;
+  return AMR_OK;
+}
+
+int amr_patch_batch_destroy(amr_patch_batch* b) {
+  if (!b) return AMR_OK;
+  if (b->link) return fail(AMR_ESTATE, "batch is still linked; call amr_link_destroy first");
+  cudaStreamSynchronize(b->stream);
+  delete b;
+  return AMR_OK;
+}
+
+void* amr_patch_batch_state(amr_patch_batch* b, int which) {
+  if (!b || which < 0 || which > 1) { fail(AMR_EINVAL, "bad arguments"); return nullptr; }
+  return b->U[which == 0 ? b->cur : 1 - b->cur];
+}
+
+int amr_patch_batch_upload(amr_patch_batch* b, const void* host, int with_ghosts) {
+  if (!b || !host) return fail(AMR_EINVAL, "null pointer");
+  const int nf = b->d.nfields, np = b->d.npatch;
+  const size_t state_bytes = (size_t)nf * np * b->n3 * b->esz;
+  if (!with_ghosts) {
+    CUDA_TRY(cudaMemcpyAsync(b->U[b->cur], host, state_bytes, cudaMemcpyHostToDevice, b->stream));
+  } else {
+    const size_t per_patch = (size_t)nf * b->M3 * b->esz;
+    int chunk = (int)std::max<size_t>(1, std::min<size_t>((size_t)np, ((size_t)512 << 20) / per_patch));
+    void* stage = nullptr;
+    CUDA_TRY(cudaMalloc(&stage, (size_t)chunk * per_patch));
+    for (int p0 = 0; p0 < np; p0 += chunk) {
+      const int npc = std::min(chunk, np - p0);
+      for (int q = 0; q < nf; ++q) {
+        cudaError_t e = cudaMemcpyAsync((char*)stage + (size_t)q * npc * b->M3 * b->esz,
+                                        (const char*)host + ((size_t)q * np + p0) * b->M3 * b->esz,
+                                        (size_t)npc * b->M3 * b->esz, cudaMemcpyHostToDevice, b->stream);
+        if (e != cudaSuccess) { cudaFree(stage); return fail(AMR_ECUDA, "upload: %s", cudaGetErrorString(e)); }
+      }
+      cudaError_t e = amr::launch_scatter_interior(b->d.dtype, stage, 1, nf, np, b->d.n, b->d.nghost, p0, npc,
+                                                   b->U[b->cur], b->stream);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(b->stream);
+      if (e != cudaSuccess) { cudaFree(stage); return fail(AMR_ECUDA, "upload: %s", cudaGetErrorString(e)); }
+    }
+    cudaFree(stage);
+  }
+  // both buffers hold the uploaded state, so that "previous state" is defined before the first step
+  CUDA_TRY(cudaMemcpyAsync(b->U[1 - b->cur], b->U[b->cur], state_bytes, cudaMemcpyDeviceToDevice, b->stream));
+  CUDA_TRY(cudaStreamSynchronize(b->stream));
+  b->smax_valid = false;
+  return AMR_OK;
+}
+
+int amr_patch_batch_download(amr_patch_batch* b, void* host, int with_ghosts) {
+  if (!b || !host) return fail(AMR_EINVAL, "null pointer");
+  const int nf = b->d.nfields, np = b->d.npatch;
+  if (!with_ghosts) {
+    CUDA_TRY(cudaMemcpyAsync(host, b->U[b->cur], (size_t)nf * np * b->n3 * b->esz, cudaMemcpyDeviceToHost, b->stream));
+    CUDA_TRY(cudaStreamSynchronize(b->stream));
+    return AMR_OK;
+  }
+  const size_t per_patch = (size_t)nf * b->M3 * b->esz;
+  int chunk = (int)std::max<size_t>(1, std::min<size_t>((size_t)np, ((size_t)512 << 20) / per_patch));
+  void* stage = nullptr;
+  CUDA_TRY(cudaMalloc(&stage, (size_t)chunk * per_patch));
+  for (int p0 = 0; p0 < np; p0 += chunk) {
+    const int npc = std::min(chunk, np - p0);
+    cudaError_t e = amr::launch_gather_ghosted(b->d.dtype, b->U[b->cur], b->halo, b->nbr_dev, nf, np, b->d.n,
+                                               b->d.nghost, p0, npc, stage, b->stream);
+    for (int q = 0; q < nf && e == cudaSuccess; ++q)
+      e = cudaMemcpyAsync((char*)host + ((size_t)q * np + p0) * b->M3 * b->esz,
+                          (const char*)stage + (size_t)q * npc * b->M3 * b->esz, (size_t)npc * b->M3 * b->esz,
+                          cudaMemcpyDeviceToHost, b->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(b->stream);
+    if (e != cudaSuccess) { cudaFree(stage); return fail(AMR_ECUDA, "download: %s", cudaGetErrorString(e)); }
+  }
+  cudaFree(stage);
+  return AMR_OK;
+}
+
+int amr_fill_ghosts(amr_patch_batch* b) {
+  if (!b) return fail(AMR_EINVAL, "null batch");
+  return AMR_OK;
+}
+
+int amr_cfl_dt(amr_patch_batch* b, double gamma, double cfl, int mhd, double* dt_out, double* smax_out) {
+  if (!b) return fail(AMR_EINVAL, "null batch");
+  if ((mhd != 0) != (b->d.nfields == 9)) return fail(AMR_EINVAL, "mhd flag does not match nfields = %d", b->d.nfields);
+  if (!std::isfinite(gamma) || !(gamma > 1)) return fail(AMR_EINVAL, "gamma must be finite and > 1");
+  if (!(cfl > 0) || !std::isfinite(cfl)) return fail(AMR_EINVAL, "cfl must be finite and > 0");
+  if (!(b->smax_valid && b->smax_gamma == gamma)) {
+    CUDA_TRY(cudaMemsetAsync(b->smax_slot, 0, 16, b->stream));
+    cudaError_t e = amr::launch_smax(b->d.dtype, b->U[b->cur], b->d.nfields, b->d.npatch, b->d.n, gamma, b->smax_slot, b->stream);
+    if (e != cudaSuccess) return fail(AMR_ECUDA, "smax kernel launch: %s", cudaGetErrorString(e));
+    b->smax_valid = true;
+    b->smax_gamma = gamma;
+  }
+  double smax;
+  if (b->d.dtype == AMR_F32) {
+    float v = 0;
+    CUDA_TRY(cudaMemcpyAsync(&v, b->smax_slot, 4, cudaMemcpyDeviceToHost, b->stream));
+    CUDA_TRY(cudaStreamSynchronize(b->stream));
+    smax = v;
+  } else {
+    CUDA_TRY(cudaMemcpyAsync(&smax, b->smax_slot, 8, cudaMemcpyDeviceToHost, b->stream));
+    CUDA_TRY(cudaStreamSynchronize(b->stream));
+  }
+  if (smax_out) *smax_out = smax;
+  if (dt_out) *dt_out = cfl * b->d.dx / smax;
+  return AMR_OK;
+}
+
+int amr_hydro_step(amr_patch_batch* b, double dt, double gamma, int limiter, int riemann) {
+  return do_step(b, false, dt, gamma, limiter, riemann, 0.0, 0.0);
+}
+
+int amr_mhd_step(amr_patch_batch* b, double dt, double gamma, int limiter, int riemann, double ch, double alpha) {
+  return do_step(b, true, dt, gamma, limiter, riemann, ch, alpha);
+}
+
+int amr_conserved_totals(amr_patch_batch* b, double* totals) {
+  if (!b || !totals) return fail(AMR_EINVAL, "null pointer");
+  const int nf = b->d.nfields;
+  cudaError_t e = amr::launch_totals(b->d.dtype, b->U[b->cur], nf, b->d.npatch, b->d.n, b->partials, b->stream);
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "totals kernel launch: %s", cudaGetErrorString(e));
+  std::vector<double> h((size_t)nf * amr::TOTALS_BLOCKS);
+  CUDA_TRY(cudaMemcpyAsync(h.data(), b->partials, h.size() * sizeof(double), cudaMemcpyDeviceToHost, b->stream));
+  CUDA_TRY(cudaStreamSynchronize(b->stream));
+  for (int q = 0; q < nf; ++q) {
+    long double s = 0;
+    for (int k = 0; k < amr::TOTALS_BLOCKS; ++k) s += (long double)h[(size_t)q * amr::TOTALS_BLOCKS + k];
+    totals[q] = (double)s;
+  }
+  return AMR_OK;
+}
+
+int amr_step_counters(amr_patch_batch* b, long long* counters, int reset) {
+  if (!b || !counters) return fail(AMR_EINVAL, "null pointer");
+  CUDA_TRY(cudaMemcpyAsync(counters, b->counters, 4 * sizeof(long long), cudaMemcpyDeviceToHost, b->stream));
+  if (reset) CUDA_TRY(cudaMemsetAsync(b->counters, 0, 4 * sizeof(long long), b->stream));
+  CUDA_TRY(cudaStreamSynchronize(b->stream));
+  return AMR_OK;
+}
+
+// ---- two-level -------------------------------------------------------------------------------------
+
+size_t amr_link_bytes(const amr_patch_batch* coarse, const amr_patch_batch* fine, int ratio) {
+  if (check_link_args(coarse, fine, ratio) != AMR_OK) return 0;
+  LinkHost H;
+  if (build_link(coarse, fine, H) != AMR_OK) return 0;
+  return make_link_layout(coarse, fine, H).total;
+}
+
+int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, void* dev_ws, size_t bytes,
+                    amr_level_link** out) {
+  if (!out) return fail(AMR_EINVAL, "null out");
+  *out = nullptr;
+  int rc = check_link_args(coarse, fine, ratio);
+  if (rc != AMR_OK) return rc;
+  if (coarse->link || fine->link) return fail(AMR_ESTATE, "batch already linked");
+  if (!dev_ws || (uintptr_t)dev_ws % ALIGN) return fail(AMR_EINVAL, "workspace must be a %zu-byte aligned device pointer", ALIGN);
+  LinkHost H;
+  rc = build_link(coarse, fine, H);
+  if (rc != AMR_OK) return rc;
+  const LinkLayout L = make_link_layout(coarse, fine, H);
+  if (bytes < L.total) return fail(AMR_EINVAL, "workspace too small: %zu < %zu bytes", bytes, L.total);
+  amr_level_link* l = new (std::nothrow) amr_level_link();
+  if (!l) return fail(AMR_ENOMEM, "out of host memory");
+  l->c = coarse; l->f = fine; l->ws = (char*)dev_ws; l->bytes = bytes;
+  l->pro_dst = (long long*)(l->ws + L.pro_dst);
+  l->pro_c7 = (long long*)(l->ws + L.pro_c7);
+  l->res_dst = (long long*)(l->ws + L.res_dst);
+  l->npro = (int)H.pro_dst.size();
+  l->nres = (int)H.res_dst.size();
+  for (int s = 0; s < 6; ++s) { l->faces[s] = (long long*)(l->ws + L.faces[s]); l->nfaces[s] = (int)(H.faces[s].size() / 4); }
+  l->fblk_c = l->ws + L.fblk_c; l->fblk_f = l->ws + L.fblk_f;
+  l->fblk_c_bytes = L.fblk_c_bytes; l->fblk_f_bytes = L.fblk_f_bytes;
+  l->nblk_c = H.nblk_c;
+  cudaStream_t s = coarse->stream;
+  auto h2d = [&](void* dst, const void* src, size_t nb) {
+    return nb ? cudaMemcpyAsync(dst, src, nb, cudaMemcpyHostToDevice, s) : cudaSuccess;
+  };
+  cudaError_t e = h2d(l->pro_dst, H.pro_dst.data(), H.pro_dst.size() * 8);
+  if (e == cudaSuccess) e = h2d(l->pro_c7, H.pro_c7.data(), H.pro_c7.size() * 8);
+  if (e == cudaSuccess) e = h2d(l->res_dst, H.res_dst.data(), H.res_dst.size() * 8);
+  for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = h2d(l->faces[k], H.faces[k].data(), H.faces[k].size() * 8);
+  if (e == cudaSuccess) e = h2d(coarse->fblk_of, H.fblk_of_c.data(), H.fblk_of_c.size() * sizeof(int));
+  std::vector<int> idf(fine->d.npatch);
+  for (int p = 0; p < fine->d.npatch; ++p) idf[p] = p;
+  if (e == cudaSuccess) e = h2d(fine->fblk_of, idf.data(), idf.size() * sizeof(int));
+  if (e == cudaSuccess) e = cudaMemsetAsync(l->fblk_c, 0, L.fblk_c_bytes + 8, s);
+  if (e == cudaSuccess) e = cudaMemsetAsync(l->fblk_f, 0, L.fblk_f_bytes + 8, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) { delete l; return fail(AMR_ECUDA, "link upload: %s", cudaGetErrorString(e)); }
+  coarse->fblk = l->nblk_c ? l->fblk_c : nullptr;
+  fine->fblk = l->fblk_f;
+  coarse->link = fine->link = l;
+  *out = l;
+  return AMR_OK;
+}
+
+int amr_link_destroy(amr_level_link* l) {
+  if (!l) return AMR_OK;
+  cudaStreamSynchronize(l->c->stream);
+  cudaStreamSynchronize(l->f->stream);
+  l->c->fblk = nullptr; l->f->fblk = nullptr;
+  l->c->link = nullptr; l->f->link = nullptr;
+  delete l;
+  return AMR_OK;
+}
+
+int amr_prolong_ghosts(amr_level_link* l, double theta) {
+  if (!l) return fail(AMR_EINVAL, "null link");
+  if (!(theta >= 0 && theta <= 1)) return fail(AMR_EINVAL, "theta must be in [0,1]");
+  amr_patch_batch *c = l->c, *f = l->f;
+  cudaError_t e = amr::launch_prolong(f->d.dtype, f->halo, (size_t)f->d.npatch * f->M3, f->d.nfields, l->pro_dst, l->pro_c7,
+                                      l->npro, c->U[1 - c->cur], c->U[c->cur], (size_t)c->d.npatch * c->n3, theta, f->stream);
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "prolong kernel launch: %s", cudaGetErrorString(e));
+  f->halo_valid = true;
+  return AMR_OK;
+}
+
+int amr_flux_clear(amr_level_link* l) {
+  if (!l) return fail(AMR_EINVAL, "null link");
+  if (l->fblk_c_bytes) CUDA_TRY(cudaMemsetAsync(l->fblk_c, 0, l->fblk_c_bytes, l->c->stream));
+  if (l->fblk_f_bytes) CUDA_TRY(cudaMemsetAsync(l->fblk_f, 0, l->fblk_f_bytes, l->f->stream));
+  return AMR_OK;
+}
+
+int amr_restrict(amr_level_link* l) {
+  if (!l) return fail(AMR_EINVAL, "null link");
+  amr_patch_batch *c = l->c, *f = l->f;
+  cudaError_t e = amr::launch_restrict(f->d.dtype, f->U[f->cur], (size_t)f->d.npatch * f->n3, f->d.nfields, f->d.n, l->res_dst,
+                                       l->nres, c->U[c->cur], (size_t)c->d.npatch * c->n3, c->stream);
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "restrict kernel launch: %s", cudaGetErrorString(e));
+  c->smax_valid = false;
+  return AMR_OK;
+}
+
+int amr_reflux(amr_level_link* l, double dt_coarse) {
+  if (!l) return fail(AMR_EINVAL, "null link");
+  if (!(dt_coarse > 0) || !std::isfinite(dt_coarse)) return fail(AMR_EINVAL, "dt_coarse must be finite and > 0");
+  amr_patch_batch* c = l->c;
+  for (int s = 0; s < 6; ++s) {
+    cudaError_t e = amr::launch_reflux(c->d.dtype, c->U[c->cur], (size_t)c->d.npatch * c->n3, c->d.nfields, c->d.n,
+                                       l->faces[s], l->nfaces[s], l->fblk_c, l->fblk_f, dt_coarse / c->d.dx, c->stream);
+    if (e != cudaSuccess) return fail(AMR_ECUDA, "reflux kernel launch: %s", cudaGetErrorString(e));
+  }
+  c->smax_valid = false;
+  return AMR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,49 @@
+// O7 (reading A9): max over directions of |v_d| + c_d for one cell, from its conserved state.
+// Used by the fused epilogue of the step kernel and by the standalone reduction (amr_cfl_dt); written
+// with explicitly rounded intrinsics (no FMA contraction) so that both kernels give bitwise the same
+// number for the same stored state (pin P15).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace amr {
+
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ float div_rn(float a, float b) { return __fdiv_rn(a, b); }
+__device__ __forceinline__ double div_rn(double a, double b) { return __ddiv_rn(a, b); }
+__device__ __forceinline__ float sqrt_rn(float a) { return __fsqrt_rn(a); }
+__device__ __forceinline__ double sqrt_rn(double a) { return __dsqrt_rn(a); }
+__device__ __forceinline__ float max_(float a, float b) { return fmaxf(a, b); }
+__device__ __forceinline__ double max_(double a, double b) { return fmax(a, b); }
+__device__ __forceinline__ float abs_(float a) { return fabsf(a); }
+__device__ __forceinline__ double abs_(double a) { return fabs(a); }
+
+template <class T, int NF>
+__device__ __forceinline__ T signal_speed(const T* u, T gamma, T gm1) {
+  const T rho = u[0];
+  const T vx = div_rn(u[1], rho), vy = div_rn(u[2], rho), vz = div_rn(u[3], rho);
+  const T v2 = add_rn(add_rn(mul_rn(vx, vx), mul_rn(vy, vy)), mul_rn(vz, vz));
+  const T ke = mul_rn(mul_rn(T(0.5), rho), v2);
+  const T vmax = max_(max_(abs_(vx), abs_(vy)), abs_(vz));
+  if (NF == 5) {
+    const T pr = mul_rn(gm1, add_rn(u[4], -ke));
+    const T c = sqrt_rn(div_rn(mul_rn(gamma, pr), rho));
+    return add_rn(vmax, c);  // c is the same in all directions
+  } else {
+    const T bx2 = mul_rn(u[5], u[5]), by2 = mul_rn(u[6], u[6]), bz2 = mul_rn(u[7], u[7]);
+    const T B2 = add_rn(add_rn(bx2, by2), bz2);
+    const T pr = mul_rn(gm1, add_rn(add_rn(u[4], -ke), -mul_rn(T(0.5), B2)));
+    const T gp = mul_rn(gamma, pr);
+    const T a = div_rn(add_rn(gp, B2), rho);
+    const T a2 = mul_rn(a, a);
+    const T k = div_rn(mul_rn(T(4), gp), mul_rn(rho, rho));  // 4 gamma p / rho^2
+    const T cx = sqrt_rn(mul_rn(T(0.5), add_rn(a, sqrt_rn(max_(add_rn(a2, -mul_rn(k, bx2)), T(0))))));
+    const T cy = sqrt_rn(mul_rn(T(0.5), add_rn(a, sqrt_rn(max_(add_rn(a2, -mul_rn(k, by2)), T(0))))));
+    const T cz = sqrt_rn(mul_rn(T(0.5), add_rn(a, sqrt_rn(max_(add_rn(a2, -mul_rn(k, bz2)), T(0))))));
+    return max_(max_(add_rn(abs_(vx), cx), add_rn(abs_(vy), cy)), add_rn(abs_(vz), cz));
+  }
+}
+
+}  // namespace amr

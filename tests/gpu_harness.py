@@ -1,0 +1,79 @@
+"""Sequencing helpers for the -m gpu parity tests: drive the CUDA path through the Python binding
+exactly as oracle.api.advance / two_level_step sequence the oracle (same order of calls), and the
+error norm of reading A18.  No arithmetic of the method lives here."""
+import numpy as np
+
+import paper_1412_0934_b200 as amr
+
+
+def gpu_dtype(np_dtype):
+    return amr.AMR_F64 if np.dtype(np_dtype) == np.float64 else amr.AMR_F32
+
+
+def gpu_step(b, wl, dt, ch, limiter=None, riemann=None):
+    lim = wl.limiter if limiter is None else limiter
+    rs = wl.riemann if riemann is None else riemann
+    if wl.mhd:
+        b.mhd_step(dt, wl.gamma, lim, rs, ch, wl.alpha)
+    else:
+        b.hydro_step(dt, wl.gamma, lim, rs)
+
+
+def gpu_advance(level, wl, nsteps, np_dtype=np.float64, dt_fixed=None, limiter=None, riemann=None):
+    """Every step: amr_cfl_dt (O7; fused value after the first step) -> dt = cfl dx / smax, c_h = smax
+    -> amr_*_step (O0..O6).  Returns dict(U, dts, smaxs, counters, batch)."""
+    b = amr.PatchBatch.from_level(level, gpu_dtype(np_dtype))
+    dts, smaxs = [], []
+    for _ in range(nsteps):
+        dt, sm = b.cfl_dt(wl.gamma, wl.cfl)
+        if dt_fixed is not None:
+            dt = dt_fixed
+        gpu_step(b, wl, dt, sm, limiter, riemann)
+        dts.append(dt)
+        smaxs.append(sm)
+    return dict(U=b.download(), dts=dts, smaxs=smaxs, counters=b.step_counters(), batch=b)
+
+
+def gpu_two_level_step(wl, np_dtype=np.float64, do_reflux=True):
+    """O9 in the order of oracle.api.two_level_step."""
+    lc, lf = wl.levels
+    dt_ = gpu_dtype(np_dtype)
+    bc = amr.PatchBatch.from_level(lc, dt_)
+    bf = amr.PatchBatch.from_level(lf, dt_)
+    link = amr.LevelLink(bc, bf)
+    _, s0 = bc.cfl_dt(wl.gamma, wl.cfl)
+    _, s1 = bf.cfl_dt(wl.gamma, wl.cfl)
+    sm = max(s0, s1)
+    dt0 = wl.cfl * lc.dx / sm
+    link.flux_clear()
+    gpu_step(bc, wl, dt0, sm)
+    for theta in (0.0, 0.5):
+        link.prolong_ghosts(theta)
+        gpu_step(bf, wl, 0.5 * dt0, sm)
+    link.restrict()
+    if do_reflux:
+        link.reflux(dt0)
+    out = dict(Uc=bc.download(), Uf=bf.download(), dt0=dt0, smax=sm, coarse=bc, fine=bf, link=link)
+    return out
+
+
+def field_groups(nf):
+    """A18: momentum and B are normalised by the max over their three components."""
+    g = [[0], [1, 2, 3], [4]]
+    if nf == 9:
+        g += [[5, 6, 7], [8]]
+    return g
+
+
+def rel_err(got, ref, psi_scale=None):
+    """Per field group: max|got-ref| / max|ref| (psi: / psi_scale when given, since it starts at 0)."""
+    got = np.asarray(got, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    errs = []
+    for grp in field_groups(ref.shape[0]):
+        num = np.abs(got[grp] - ref[grp]).max()
+        den = np.abs(ref[grp]).max()
+        if grp == [8] and psi_scale is not None:
+            den = max(den, psi_scale)
+        errs.append(num / max(den, 1e-300))
+    return np.array(errs)

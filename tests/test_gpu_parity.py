@@ -1,0 +1,277 @@
+"""-m gpu parity tests proper: the CUDA path (through the C-ABI, via the Python binding) against the
+CPU oracle, element by element on the same seeded inputs.  Tolerances: BASELINE.json:north_star
+(fp64 <= 1e-12 per step, <= 1e-10 after 20 steps; fp32 <= 1e-5; conserved totals 1e-13), error norm
+of reading A18 (tests/gpu_harness.rel_err)."""
+import numpy as np
+import pytest
+
+import workloads as wk
+
+pytestmark = pytest.mark.gpu
+
+TOL64_STEP, TOL64_MULTI, TOL32 = 1e-12, 1e-10, 1e-5
+
+
+@pytest.fixture(scope="module")
+def H():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device (there is no CPU fallback)")
+    from tests import gpu_harness
+    return gpu_harness
+
+
+def _psi_scale(ref, ch):
+    return ch * np.abs(ref[5:8]).max()
+
+
+def test_config1_sod_20_steps_fp64(oracle, H):
+    """Config 1: one 32^3 patch, outflow, minmod + HLLC, cfl 0.4, 20 steps, dt from amr_cfl_dt."""
+    wl = wk.config1_sod()
+    lev = wl.levels[0]
+    ref1 = oracle.advance(lev, wl, 1)
+    got1 = H.gpu_advance(lev, wl, 1)
+    assert H.rel_err(got1["U"], ref1["U"]).max() <= TOL64_STEP
+    ref = oracle.advance(lev, wl, 20)
+    got = H.gpu_advance(lev, wl, 20)
+    assert np.allclose(got["dts"], ref["dts"], rtol=1e-12, atol=0)
+    assert H.rel_err(got["U"], ref["U"]).max() <= TOL64_MULTI
+    # P3 on the GPU: j/k invariance bitwise, no transverse momentum
+    U = got["U"][:, 0]
+    assert np.array_equal(U, np.broadcast_to(U[:, :1, :1, :], U.shape))
+    assert not U[2].any() and not U[3].any()
+    # P1/P2: against the exact Riemann solution (tests/golden/sod_exact.txt is used by the oracle pin;
+    # here the same L1 bound is asserted on the GPU profile through the oracle's agreement)
+    assert np.abs(U[0, 0, 0] - ref["U"][0, 0, 0, 0]).max() < 1e-12
+
+
+def test_config2_random_patches_fp64(oracle, H):
+    """Config 2: 512 self-periodic 16^3 patches, MC + HLLC, one step at the CFL-reduced dt."""
+    wl = wk.config2_random_patches()
+    lev = wl.levels[0]
+    ref = oracle.advance(lev, wl, 1)
+    got = H.gpu_advance(lev, wl, 1)
+    assert abs(got["smaxs"][0] - ref["smaxs"][0]) <= 1e-14 * ref["smaxs"][0]
+    assert H.rel_err(got["U"], ref["U"]).max() <= TOL64_STEP
+    # conserved totals: GPU reduction vs oracle long-double sums, and conservation itself (P5)
+    b = got["batch"]
+    tot = b.conserved_totals()
+    tref = oracle.totals(oracle.ghosted(ref["U"], lev.g), lev.g)
+    absn = np.abs(ref["U"]).sum(axis=(1, 2, 3, 4))
+    assert (np.abs(tot - tref) / absn).max() <= 1e-13
+    t0 = oracle.totals(oracle.ghosted(lev.U, lev.g), lev.g)
+    assert (np.abs(tot - t0) / absn).max() <= 1e-13
+
+
+@pytest.mark.parametrize("np_dtype", [np.float64, np.float32])
+def test_config3_orszag_tang_small(oracle, H, np_dtype):
+    """Config 3 at 64^3 (64 patches of 16^3, Morton order): MC + HLLD + GLM, 5 steps."""
+    wl = wk.config3_orszag_tang(N=64)
+    lev = wl.levels[0]
+    lev.U = lev.U.astype(np_dtype).astype(np.float64)     # A17: oracle starts from the rounded data
+    ref = oracle.advance(lev, wl, 5)
+    got = H.gpu_advance(lev, wl, 5, np_dtype=np_dtype)
+    tol = TOL64_MULTI if np_dtype == np.float64 else TOL32
+    err = H.rel_err(got["U"], ref["U"], psi_scale=_psi_scale(ref["U"], ref["smaxs"][-1]))
+    assert err.max() <= tol, err
+    if np_dtype == np.float64:
+        got1 = H.gpu_advance(lev, wl, 1)
+        ref1 = oracle.advance(lev, wl, 1)
+        e1 = H.rel_err(got1["U"], ref1["U"], psi_scale=_psi_scale(ref1["U"], ref1["smaxs"][-1]))
+        assert e1.max() <= TOL64_STEP, e1
+        tot = got["batch"].conserved_totals()
+        t0 = oracle.totals(oracle.ghosted(lev.U, lev.g), lev.g)
+        absn = np.abs(lev.U).sum(axis=(1, 2, 3, 4))
+        assert (np.abs(tot - t0)[:8] / absn[:8]).max() <= 1e-13
+
+
+@pytest.mark.parametrize("np_dtype", [np.float64, np.float32])
+def test_config5_turbulence_small(oracle, H, np_dtype):
+    """Config 5 recipe at 64^3 as 8 patches of 32^3 (several tiles per patch, Mach 3, beta = 100)."""
+    G = wk.configs.turbulence_state(64)
+    wl = wk.uniform_grid_workload("config5_small", G, 32, 5.0 / 3.0, True, wk.configs.LIM_MC, wk.configs.RS_HLLD, 0.3, 3)
+    lev = wl.levels[0]
+    lev.U = lev.U.astype(np_dtype).astype(np.float64)
+    ref = oracle.advance(lev, wl, 3)
+    got = H.gpu_advance(lev, wl, 3, np_dtype=np_dtype)
+    tol = TOL64_MULTI if np_dtype == np.float64 else TOL32
+    err = H.rel_err(got["U"], ref["U"], psi_scale=_psi_scale(ref["U"], ref["smaxs"][-1]))
+    assert err.max() <= tol, err
+
+
+def _random_level(nf, n, npx, seed, outflow=False, np_dtype=np.float64):
+    rng = np.random.default_rng([wk.SEED, 99, seed])
+    N = n * npx
+    rho = np.exp(0.4 * rng.standard_normal((N, N, N)))
+    v = 0.8 * rng.standard_normal((3, N, N, N))
+    p = np.exp(0.3 * rng.standard_normal((N, N, N)))
+    B = 0.7 * rng.standard_normal((3, N, N, N)) if nf == 9 else None
+    G = wk.primitive_to_conserved(rho, v, p, 5.0 / 3.0, B=B)
+    if nf == 9:
+        G[8] = 0.1 * rng.standard_normal((N, N, N))
+    bc = (wk.configs.BC_OUTFLOW,) * 6 if outflow else (wk.configs.BC_PERIODIC,) * 6
+    wl = wk.uniform_grid_workload("random", G, n, 5.0 / 3.0, nf == 9, wk.configs.LIM_MC,
+                                  wk.configs.RS_HLLD if nf == 9 else wk.configs.RS_HLLC, 0.3, 1, bc=bc)
+    wl.levels[0].U = wl.levels[0].U.astype(np_dtype).astype(np.float64)
+    return wl
+
+
+@pytest.mark.parametrize("nf", [5, 9])
+@pytest.mark.parametrize("limiter", [0, 1, 2])
+@pytest.mark.parametrize("rs_exact", [False, True])
+@pytest.mark.parametrize("n", [8, 16])
+def test_every_limiter_and_solver_fp64(oracle, H, nf, limiter, rs_exact, n):
+    """One step of every (limiter x Riemann solver) on rough random data (white noise: shocks at every
+    face, all HLLD regions, positivity fallbacks), periodic 2x2x2 patches; n=8 runs the 8x8 tile."""
+    wl = _random_level(nf, n, 2, seed=nf * 10 + n)
+    lev = wl.levels[0]
+    rs = (wk.configs.RS_HLLD if nf == 9 else wk.configs.RS_HLLC) if rs_exact else wk.configs.RS_HLL
+    ref = oracle.advance(lev, wl, 1, limiter=limiter, riemann_solver=rs)
+    got = H.gpu_advance(lev, wl, 1, limiter=limiter, riemann=rs)
+    err = H.rel_err(got["U"], ref["U"], psi_scale=_psi_scale(ref["U"], ref["smaxs"][0]) if nf == 9 else None)
+    assert err.max() <= TOL64_STEP, err
+    if n == 16:  # tile == patch: the event counters count the same cells/faces as the oracle
+        assert got["counters"] == ref["counters"][0]
+
+
+@pytest.mark.parametrize("nf", [5, 9])
+def test_every_solver_fp32(oracle, H, nf):
+    wl = _random_level(nf, 16, 2, seed=7 + nf, np_dtype=np.float32)
+    lev = wl.levels[0]
+    ref = oracle.advance(lev, wl, 2)
+    got = H.gpu_advance(lev, wl, 2, np_dtype=np.float32)
+    err = H.rel_err(got["U"], ref["U"], psi_scale=_psi_scale(ref["U"], ref["smaxs"][0]) if nf == 9 else None)
+    assert err.max() <= TOL32, err
+
+
+@pytest.mark.parametrize("nf", [5, 9])
+def test_outflow_multi_patch(oracle, H, nf):
+    """O0 (ii): outflow clamp on a 2x2x2-patch domain (edge and corner regions clamp into siblings)."""
+    wl = _random_level(nf, 16, 2, seed=3, outflow=True)
+    lev = wl.levels[0]
+    ref = oracle.advance(lev, wl, 2)
+    got = H.gpu_advance(lev, wl, 2)
+    err = H.rel_err(got["U"], ref["U"], psi_scale=_psi_scale(ref["U"], ref["smaxs"][0]) if nf == 9 else None)
+    assert err.max() <= TOL64_MULTI, err
+
+
+@pytest.mark.parametrize("outflow", [False, True])
+def test_ghost_cells_seen_through_the_api(oracle, H, outflow):
+    """amr_patch_batch_download(with_ghosts=1) == oracle O0 fill, all three layers, bit for bit."""
+    import paper_1412_0934_b200 as amr
+    wl = _random_level(9, 16, 2, seed=11, outflow=outflow)
+    lev = wl.levels[0]
+    b = amr.PatchBatch.from_level(lev, amr.AMR_F64)
+    b.fill_ghosts()
+    got = b.download(with_ghosts=True)
+    ref = oracle.ghosted(lev.U, lev.g)
+    oracle.fill_ghosts(ref, lev.g, lev.origin, lev.domain_cells, lev.bc, lev.self_periodic)
+    assert np.array_equal(got, ref)
+    # upload with ghosts ignores the ghost layer
+    junk = ref.copy()
+    junk[:, :, :3] = -7.0
+    b.upload(junk, with_ghosts=True)
+    assert np.array_equal(b.download(), lev.U)
+
+
+def test_cfl_fused_equals_standalone(oracle, H):
+    """P15 on the GPU: the smax fused into the step epilogue is bitwise the standalone reduction's."""
+    import paper_1412_0934_b200 as amr
+    for nf, npd in ((5, np.float64), (9, np.float64), (5, np.float32), (9, np.float32)):
+        wl = _random_level(nf, 16, 2, seed=21 + nf, np_dtype=npd)
+        lev = wl.levels[0]
+        r = H.gpu_advance(lev, wl, 1, np_dtype=npd)
+        b = r["batch"]
+        _, fused = b.cfl_dt(wl.gamma, wl.cfl)
+        b2 = amr.PatchBatch(lev.npatch, lev.n, nf, H.gpu_dtype(npd), lev.dx, origin=lev.origin,
+                            domain_cells=lev.domain_cells, bc=lev.bc)
+        b2.upload(r["U"])
+        _, alone = b2.cfl_dt(wl.gamma, wl.cfl)
+        assert fused == alone
+        ref = oracle.smax(oracle.ghosted(r["U"].astype(np.float64), lev.g), lev.g, wl.gamma)
+        assert abs(alone - ref) <= (1e-14 if npd == np.float64 else 1e-6) * ref
+
+
+def test_uniform_state_is_preserved_bitwise(H):
+    """P4 on the GPU: flux differences cancel exactly; psi only decays by exp(-alpha ch dt/dx)."""
+    import paper_1412_0934_b200 as amr
+    n, npx = 16, 2
+    G = np.empty((9, 32, 32, 32))
+    prim = wk.primitive_to_conserved(np.full((32, 32, 32), 1.3), (np.full((32, 32, 32), 0.4),) * 3,
+                                     np.full((32, 32, 32), 0.7), 5.0 / 3.0,
+                                     B=(np.full((32, 32, 32), 0.3), np.full((32, 32, 32), -0.2), np.full((32, 32, 32), 0.5)))
+    G[:] = prim
+    G[8] = 0.25
+    wl = wk.uniform_grid_workload("uniform", G, n, 5.0 / 3.0, True, 2, 2, 0.3, 1)
+    lev = wl.levels[0]
+    b = amr.PatchBatch.from_level(lev, amr.AMR_F64)
+    dt, sm = b.cfl_dt(wl.gamma, wl.cfl)
+    b.mhd_step(dt, wl.gamma, 2, 2, sm, 0.4)
+    U = b.download()
+    assert np.array_equal(U[:8], lev.U[:8])
+    assert np.allclose(U[8], 0.25 * np.exp(-0.4 * sm * dt / lev.dx), rtol=1e-15)
+
+
+@pytest.mark.parametrize("mhd", [False, True])
+def test_two_level_step_fp64(oracle, H, mhd):
+    """Config 4 at 64^3 fine index space: O9 (coarse step, two fine substeps with prolonged halos,
+    restriction, reflux) against the oracle, and composite conservation (P13) on the GPU result."""
+    wl = wk.config4_two_level(mhd, nfine=64, threshold=3.0)
+    lc, lf = wl.levels
+    ref = oracle.two_level_step(wl)
+    got = H.gpu_two_level_step(wl)
+    assert abs(got["dt0"] - ref["dt0"]) <= 1e-13 * ref["dt0"]
+    ps = ref["smax"] * max(np.abs(ref["Uc"][5:8]).max(), 1e-300) if mhd else None
+    ec = H.rel_err(got["Uc"], ref["Uc"], psi_scale=ps)
+    ef = H.rel_err(got["Uf"], ref["Uf"], psi_scale=ps)
+    assert ec.max() <= 2 * TOL64_STEP and ef.max() <= 2 * TOL64_STEP, (ec, ef)
+    tot = oracle.composite_totals(oracle.ghosted(got["Uc"], lc.g), lc, oracle.ghosted(got["Uf"], lf.g), lf)
+    nfc = 8 if mhd else 5
+    absn = np.array([np.abs(lc.U[f]).sum() * lc.dx ** 3 for f in range(lc.nfields)])
+    assert (np.abs(tot - ref["totals_before"])[:nfc] / absn[:nfc]).max() <= 1e-13
+
+
+def test_prolonged_halo_seen_through_the_api(oracle, H):
+    """O8 through the API: after amr_prolong_ghosts the fine ghosts equal the oracle's (theta = 0.5)."""
+    import paper_1412_0934_b200 as amr
+    wl = wk.config4_two_level(False, nfine=64, threshold=3.0)
+    lc, lf = wl.levels
+    bc = amr.PatchBatch.from_level(lc, amr.AMR_F64)
+    bf = amr.PatchBatch.from_level(lf, amr.AMR_F64)
+    link = amr.LevelLink(bc, bf)
+    dt, sm = bc.cfl_dt(wl.gamma, wl.cfl)
+    bc.hydro_step(dt, wl.gamma, wl.limiter, wl.riemann)
+    link.prolong_ghosts(0.5)
+    got = bf.download(with_ghosts=True)
+    g = lc.g
+    Uc = oracle.ghosted(lc.U, g)
+    oracle.fill_ghosts(Uc, g, lc.origin, lc.domain_cells, lc.bc, False)
+    Ucn = oracle.step(Uc, g, dt, lc.dx, wl.gamma, wl.limiter, wl.riemann)["U"]
+    oracle.fill_ghosts(Ucn, g, lc.origin, lc.domain_cells, lc.bc, False)
+    Uf = oracle.ghosted(lf.U, g)
+    mask = oracle.fill_ghosts(Uf, g, lf.origin, lf.domain_cells, lf.bc, False)
+    oracle.prolong_ghosts(Uf, mask, lf, Uc, Ucn, lc, 0.5)
+    assert (mask == 2).any()
+    assert H.rel_err(got, Uf).max() <= TOL64_STEP
+
+
+def test_api_rejects_bad_arguments(H):
+    import paper_1412_0934_b200 as amr
+    with pytest.raises(amr.AmrError):
+        amr.PatchBatch(1, 12, 5, amr.AMR_F64, 0.1, self_periodic=True)          # n not a multiple of 8
+    with pytest.raises(amr.AmrError):
+        amr.PatchBatch(1, 16, 7, amr.AMR_F64, 0.1, self_periodic=True)          # nfields
+    with pytest.raises(amr.AmrError):
+        amr.PatchBatch(2, 16, 5, amr.AMR_F64, 0.1, origin=[[0, 0, 0], [0, 0, 0]], domain_cells=(32, 16, 16))
+    b = amr.PatchBatch(1, 16, 5, amr.AMR_F64, 0.1, self_periodic=True)
+    b.upload(np.ones((5, 1, 16, 16, 16)))
+    for args in ((0.0, 1.4, 1, 1), (1e-3, 1.0, 1, 1), (1e-3, float("nan"), 1, 1), (1e-3, 1.4, 5, 1), (1e-3, 1.4, 1, 2)):
+        with pytest.raises(amr.AmrError):
+            b.hydro_step(*args)
+    with pytest.raises(amr.AmrError):
+        b.mhd_step(1e-3, 1.4, 1, 2, 1.0, 0.4)                                   # MHD step on 5 fields
+    m = amr.PatchBatch(1, 16, 9, amr.AMR_F32, 0.1, self_periodic=True)
+    with pytest.raises(amr.AmrError):
+        m.mhd_step(1e-3, 1.4, 1, 1, 1.0, 0.4)                                   # HLLC in the MHD step
+    with pytest.raises(amr.AmrError):
+        m.mhd_step(1e-3, 1.4, 1, 2, 0.0, 0.4)                                   # ch <= 0
