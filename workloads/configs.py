@@ -407,3 +407,71 @@ def smooth_wave_patchset(kind: str, N: int, axis: int = 0, t: float = 0.0, n: in
                               0.3, 0)
     w.levels[0].dx = 1.0 / N
     return w
+
+
+# --------------------------------------------------------------------------------------
+# device-side generator for the full-size config 5 (512^3): same recipe (A21) evaluated with
+# torch.fft on the GPU from a seeded torch.Generator, because 512^3 float64 FFTs on the host
+# would dominate the benchmark's run time (SURVEY.md §8(d) allows exactly this).  Data only.
+# --------------------------------------------------------------------------------------
+
+def morton_permutation(npx: int, npy: int, npz: int) -> np.ndarray:
+    """perm[m] = raster index (pz*npy + py)*npx + px of the m-th patch along the Morton curve."""
+    pz, py, px = np.meshgrid(np.arange(npz), np.arange(npy), np.arange(npx), indexing="ij")
+    px, py, pz = px.ravel(), py.ravel(), pz.ravel()
+    return np.argsort(morton_key(px, py, pz), kind="stable")
+
+
+def turbulence_patches_torch(N: int, n: int, device, mach: float = 3.0, beta: float = 100.0,
+                             index: float = -11.0 / 3.0, config: int = 5):
+    """Config-5 state on an N^3 grid, built on `device` in float32: rho=1, p=1, v = Gaussian random
+    fields with P(k) ~ k^index scaled to sqrt<v.v> = mach*sqrt(gamma); B = solenoidally projected
+    field of the same spectrum, zero mean, <B.B> = 2p/beta; psi = 0.  Returns (U, origin) with U a
+    torch float32 tensor [9, npatch, n, n, n] in Morton patch order and origin int32 [npatch, 3]."""
+    import torch
+    gamma = 5.0 / 3.0
+    gen = torch.Generator(device=device)
+    gen.manual_seed(SEED * 10 + config)
+    kf = torch.fft.fftfreq(N, device=device) * N
+    kx = torch.fft.rfftfreq(N, device=device) * N
+    KZ, KY, KX = torch.meshgrid(kf, kf, kx, indexing="ij")
+    k2 = KX * KX + KY * KY + KZ * KZ
+    k = torch.sqrt(k2)
+    amp = torch.where((k > 0) & (k <= N / 2), torch.clamp(k, min=1.0) ** (index / 2.0), torch.zeros_like(k))
+    del k
+
+    def filtered_hat():
+        w = torch.randn((N, N, N), generator=gen, device=device, dtype=torch.float32)
+        return torch.fft.rfftn(w) * amp
+
+    v = []
+    for _ in range(3):
+        f = torch.fft.irfftn(filtered_hat(), s=(N, N, N))
+        f -= f.mean()
+        f /= f.std()
+        v.append(f)
+    norm = torch.sqrt((v[0] ** 2 + v[1] ** 2 + v[2] ** 2).mean())
+    v = [c * (mach * np.sqrt(gamma) / norm) for c in v]
+    hats = [filtered_hat() for _ in range(3)]
+    kdotb = (KX * hats[0] + KY * hats[1] + KZ * hats[2]) / torch.clamp(k2, min=1.0)
+    hats = [hats[0] - KX * kdotb, hats[1] - KY * kdotb, hats[2] - KZ * kdotb]
+    del kdotb
+    B = []
+    for h in hats:
+        f = torch.fft.irfftn(h, s=(N, N, N))
+        f -= f.mean()
+        B.append(f)
+    del hats
+    bn = torch.sqrt((B[0] ** 2 + B[1] ** 2 + B[2] ** 2).mean())
+    B = [c * (np.sqrt(2.0 / beta) / bn) for c in B]
+    rho = torch.ones((N, N, N), device=device, dtype=torch.float32)
+    E = 1.0 / (gamma - 1.0) + 0.5 * rho * (v[0] ** 2 + v[1] ** 2 + v[2] ** 2) + 0.5 * (B[0] ** 2 + B[1] ** 2 + B[2] ** 2)
+    fields = [rho, rho * v[0], rho * v[1], rho * v[2], E, B[0], B[1], B[2], torch.zeros_like(rho)]
+    npd = N // n
+    perm = torch.as_tensor(morton_permutation(npd, npd, npd), device=device)
+    out = torch.empty((9, npd ** 3, n, n, n), device=device, dtype=torch.float32)
+    for q, f in enumerate(fields):
+        t = f.reshape(npd, n, npd, n, npd, n).permute(0, 2, 4, 1, 3, 5).reshape(npd ** 3, n, n, n)
+        out[q] = t.index_select(0, perm)
+    origin = morton_patch_origins(npd, npd, npd, n)
+    return out, origin
