@@ -42,7 +42,7 @@ UNIT = "cell-updates/s"
 BYTES_PER_CELL = {("hydro", "f32"): 40, ("hydro", "f64"): 80, ("mhd", "f32"): 72, ("mhd", "f64"): 144}
 # algorithmic floating-point operations per cell-update (add/sub/mul/min/max/abs/compare = 1,
 # fma = 2, div and sqrt = 1; each face once, no halo recomputation), MC limiter, HLLC / HLLD+GLM
-FLOPS_PER_CELL = {"hydro": 640, "mhd": 1730}
+FLOPS_PER_CELL = {"hydro": 600, "mhd": 1700}
 
 
 def peaks():
