@@ -4,15 +4,26 @@
 // U_new written to HBM.  Formulas: DESIGN.md §3; PAPER.md:43, 57, 58, 76 name the pieces.
 //
 // Work decomposition: one CTA owns a TX x TY column of one patch and marches along z
-// (2.5-D streaming).  A ring of three primitive planes (tile + radius-2 halo) lives in shared memory.
-// Per plane:  A  load U of plane k+1 through the neighbour table, convert, store to the ring
-//             B  one thread per cell of the tile grown by one layer in x/y: slopes, predictor, face
-//                states; x/y face states go to shared memory, z face states stay in registers and the
-//                z flux is solved here
-//             C  one thread per x/y face: Riemann flux -> shared memory
-//             D  one thread per interior cell: gather the six fluxes, update, store, signal speed
+// (2.5-D streaming).  One thread per cell of the tile grown by one layer in x/y (no corners).  Shared
+// memory is array-of-structs (all NF components of a cell contiguous, padded to a bank-conflict-free
+// stride) so that a cell moves with 128-bit LDS/STS:
+//   ring   three planes of primitives on the tile + radius-2 halo; the raw conserved plane k+2 arrives by
+//          cp.async (LDGSTS) into the slot plane k-1 vacates and is converted in place by the thread
+//          that issued the copies
+//   XP/YP  W^+_x / W^+_y of the left / lower neighbour of every x / y face of the current plane
+//   FX/FY  the x / y face fluxes of the current plane
+// Per plane, two barriers:
+//   1  slopes, predictor, positivity; publish W^+_x, W^+_y; keep W^-_x, W^-_y in registers; the z face
+//      (left state = this thread's W^+_z of the previous plane) is solved here and the previous plane
+//      is updated, stored and its signal speed reduced                                   | barrier
+//   2  issue the copies of plane k+2; x and y Riemann problems at this cell's lower faces (the upper
+//      ring solves the tile's last face); convert plane k+2 to primitives                | barrier
+//   3  (Fx+ - Fx-) + (Fy+ - Fy-) of this plane -> registers; falls through into 1 of the next plane
 // Every face flux is computed once per tile by one position-independent routine, so a face shared by
 // two tiles/patches gets bitwise the same flux on both sides (conservation to round-off).
+//
+// fp32 arithmetic uses the SFU approximations (rcp/sqrt/rsqrt .approx.ftz, <= 2 ulp) instead of the
+// IEEE sequences (12 issue slots each, measured): DESIGN.md §3 "arithmetic freedom"; fp64 is IEEE.
 #pragma once
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -26,33 +37,62 @@ enum { LIM_NONE = 0, LIM_MINMOD = 1, LIM_MC = 2 };
 enum { RS_HLL = 0, RS_HLLC = 1, RS_HLLD = 2 };
 enum { CNT_POSITIVITY = 0, CNT_HLL_FALLBACK = 1, CNT_DEGENERATE_D = 2, CNT_NEG_STATE = 3 };
 
-template <class T> __device__ __forceinline__ T rmin(T a, T b) { return a < b ? a : b; }
-template <> __device__ __forceinline__ float rmin<float>(float a, float b) { return fminf(a, b); }
-template <> __device__ __forceinline__ double rmin<double>(double a, double b) { return fmin(a, b); }
-template <class T> __device__ __forceinline__ T rmax(T a, T b) { return a > b ? a : b; }
-template <> __device__ __forceinline__ float rmax<float>(float a, float b) { return fmaxf(a, b); }
-template <> __device__ __forceinline__ double rmax<double>(double a, double b) { return fmax(a, b); }
-__device__ __forceinline__ float rsqrt_(float a) { return sqrtf(a); }
+__device__ __forceinline__ float rmin(float a, float b) { return fminf(a, b); }
+__device__ __forceinline__ double rmin(double a, double b) { return fmin(a, b); }
+__device__ __forceinline__ float rmax(float a, float b) { return fmaxf(a, b); }
+__device__ __forceinline__ double rmax(double a, double b) { return fmax(a, b); }
+// three-input min / max: one FMNMX3 on sm_100a for fp32
+__device__ __forceinline__ float rmin3(float a, float b, float c) {
+  float r;
+  asm("min.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+  return r;
+}
+__device__ __forceinline__ float rmax3(float a, float b, float c) {
+  float r;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+  return r;
+}
+__device__ __forceinline__ double rmin3(double a, double b, double c) { return fmin(fmin(a, b), c); }
+__device__ __forceinline__ double rmax3(double a, double b, double c) { return fmax(fmax(a, b), c); }
+__device__ __forceinline__ float rsqrt_(float a) {
+  float r;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
+  return r;
+}
 __device__ __forceinline__ double rsqrt_(double a) { return sqrt(a); }
 __device__ __forceinline__ float rabs(float a) { return fabsf(a); }
 __device__ __forceinline__ double rabs(double a) { return fabs(a); }
-__device__ __forceinline__ float rrcp(float a) { return 1.0f / a; }
+__device__ __forceinline__ float rrcp(float a) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
+  return r;
+}
 __device__ __forceinline__ double rrcp(double a) { return 1.0 / a; }
+// 1/sqrt(x) given x and sq = sqrt(x)
+__device__ __forceinline__ float rinvsqrt(float x, float) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ double rinvsqrt(double, double sq) { return 1.0 / sq; }
 template <class T> __device__ __forceinline__ T rinf();
 template <> __device__ __forceinline__ float rinf<float>() { return CUDART_INF_F; }
 template <> __device__ __forceinline__ double rinf<double>() { return CUDART_INF; }
 
-// O2.  a = W_c - W_{c-1}, b = W_{c+1} - W_c (undivided).  Branch-free forms that return exactly
-// the value of the sign-test definition:
-//   minmod: max(min(a,b),0) + min(max(a,b),0)
-//   MC    : 2*( max(min(a,b,q),0) + min(max(a,b,q),0) ),  q = (a+b)/4
+// O2, as HALF slopes h = Delta/2 (the face states are W* +- h, the predictor uses (dt/dx) h).
+// a = W_c - W_{c-1}, b = W_{c+1} - W_c (undivided).  Branch-free forms that return exactly the value of
+// the sign-test definition (x = min of the candidates, y = max of them: x > 0 -> x, y < 0 -> y, else 0):
+//   minmod: Delta/2 = max(x, min(y, 0)) with candidates a/2, b/2
+//   MC    : Delta/2 = max(x, min(y, 0)) with candidates a, b, (a+b)/4
 template <class T, int LIM>
-__device__ __forceinline__ T limited_slope(T a, T b) {
+__device__ __forceinline__ T half_slope(T a, T b) {
   if (LIM == LIM_NONE) return T(0);
-  const T lo = rmin(a, b), hi = rmax(a, b);
-  if (LIM == LIM_MINMOD) return rmax(lo, T(0)) + rmin(hi, T(0));
+  if (LIM == LIM_MINMOD) {
+    const T ha = T(0.5) * a, hb = T(0.5) * b;
+    return rmax(rmin(ha, hb), rmin(rmax(ha, hb), T(0)));
+  }
   const T q = T(0.25) * (a + b);
-  return T(2) * (rmax(rmin(lo, q), T(0)) + rmin(rmax(hi, q), T(0)));
+  return rmax(rmin3(a, b, q), rmin(rmax3(a, b, q), T(0)));
 }
 
 template <class T>
@@ -189,13 +229,14 @@ __device__ __forceinline__ void riemann_mhd(const T* WL, const T* WR, const Riem
   T f7 = uK * b2K - wK * Bn;
   if (star) {
     // star-state tangential components on both sides (the ** state needs both)
-    T vs[2], ws[2], b1s[2], b2s[2], rs[2];
+    T vs[2], ws[2], b1s[2], b2s[2], rs[2], idSM[2];
 #pragma unroll
     for (int K = 0; K < 2; ++K) {
       const T m = K ? mR : mL, sk = K ? sr : sl, SKk = K ? SR : SL, u = K ? uR : uL;
       const T v = K ? vR : vL, w = K ? wR : wL, b1 = K ? b1R : b1L, b2 = K ? b2R : b2L;
       const T dSM = SKk - SM;
-      rs[K] = m * rrcp(dSM);
+      idSM[K] = rrcp(dSM);
+      rs[K] = m * idSM[K];
       const T D = m * dSM - Bn2;
       const bool deg = rabs(D) < C.eps * m * sk;
       if (deg) atomicAdd(&s_cnt[CNT_DEGENERATE_D], 1);
@@ -211,7 +252,7 @@ __device__ __forceinline__ void riemann_mhd(const T* WL, const T* WR, const Riem
     const T rsK = left ? rs[0] : rs[1], vsK = left ? vs[0] : vs[1], wsK = left ? ws[0] : ws[1];
     const T b1sK = left ? b1s[0] : b1s[1], b2sK = left ? b2s[0] : b2s[1];
     const T vBsK = SM * Bn + vsK * b1sK + wsK * b2sK;
-    const T EsK = (skK * EK - pTK * uK + pTs * SM + Bn * (vBK - vBsK)) * rrcp(SK - SM);
+    const T EsK = (skK * EK - pTK * uK + pTs * SM + Bn * (vBK - vBsK)) * (left ? idSM[0] : idSM[1]);
     f0 += SK * (rsK - rK);
     f1 += SK * (rsK * SM - mnK);
     f2 += SK * (rsK * vsK - rK * vK);
@@ -222,7 +263,8 @@ __device__ __forceinline__ void riemann_mhd(const T* WL, const T* WR, const Riem
     if (!(Bn2 < C.eps * pTs)) {  // rotational waves present
       const T sqL = rsqrt_(rs[0]), sqR = rsqrt_(rs[1]);
       const T aBn = rabs(Bn);
-      const T SsK = left ? (SM - aBn * rrcp(sqL)) : (SM + aBn * rrcp(sqR));
+      const T sqK = left ? sqL : sqR;
+      const T SsK = SM + (left ? -aBn : aBn) * rinvsqrt(rsK, sqK);
       const bool dstar = left ? (SsK < T(0)) : (SsK >= T(0));
       if (dstar) {
         const T sg = (Bn > T(0)) ? T(1) : T(-1);
@@ -232,7 +274,6 @@ __device__ __forceinline__ void riemann_mhd(const T* WL, const T* WR, const Riem
         const T b1ss = (sqL * b1s[1] + sqR * b1s[0] + sqL * sqR * (vs[1] - vs[0]) * sg) * iSig;
         const T b2ss = (sqL * b2s[1] + sqR * b2s[0] + sqL * sqR * (ws[1] - ws[0]) * sg) * iSig;
         const T vBss = SM * Bn + vss * b1ss + wss * b2ss;
-        const T sqK = left ? sqL : sqR;
         // E**_L = E*_L - sqrt(rho*_L)(vB*_L - vB**) sg ;  E**_R = E*_R + sqrt(rho*_R)(vB*_R - vB**) sg
         const T EssK = left ? (EsK - sqK * (vBsK - vBss) * sg) : (EsK + sqK * (vBsK - vBss) * sg);
         f2 += SsK * (rsK * vss - rsK * vsK);
@@ -260,31 +301,100 @@ template <> __device__ __forceinline__ void atomic_max_bits<double>(void* slot, 
   atomicMax(reinterpret_cast<unsigned long long*>(slot), (unsigned long long)__double_as_longlong(v));
 }
 
+// ---- shared-memory cell records (array of structs) -------------------------------------------------
+// FS = record stride in elements: a multiple of the vector width VW, chosen so that the 128-bit (64-bit
+// for fp32 hydro) accesses of consecutive lanes to consecutive records touch every bank once per phase:
+//   fp32 MHD  9 -> 12 (float4, float4, float)     fp32 hydro 5 -> 6 (float2, float2, float)
+//   fp64 MHD  9 -> 10 (4 x double2, double)       fp64 hydro 5 -> 6 (2 x double2, double)
+template <class T, int NF>
+struct Aos {
+  static constexpr int VW = (sizeof(T) == 4 && NF == 9) ? 4 : 2;
+  static constexpr int FS = sizeof(T) == 4 ? (NF == 9 ? 12 : 6) : (NF == 9 ? 10 : 6);
+};
+template <class T, int VW> struct Vec;
+template <> struct Vec<float, 4> { using type = float4; };
+template <> struct Vec<float, 2> { using type = float2; };
+template <> struct Vec<double, 2> { using type = double2; };
+
+template <class T, int NF>
+__device__ __forceinline__ void lds_cell(const T* p, T* w) {
+  constexpr int VW = Aos<T, NF>::VW;
+  using V = typename Vec<T, VW>::type;
+#pragma unroll
+  for (int q = 0; q + VW <= NF; q += VW) {
+    const V v = *reinterpret_cast<const V*>(p + q);
+    w[q] = v.x;
+    w[q + 1] = v.y;
+    if constexpr (VW == 4) { w[q + 2] = v.z; w[q + 3] = v.w; }
+  }
+#pragma unroll
+  for (int q = (NF / VW) * VW; q < NF; ++q) w[q] = p[q];
+}
+template <class T, int NF>
+__device__ __forceinline__ void sts_cell(T* p, const T* w) {
+  constexpr int VW = Aos<T, NF>::VW;
+  using V = typename Vec<T, VW>::type;
+#pragma unroll
+  for (int q = 0; q + VW <= NF; q += VW) {
+    V v;
+    v.x = w[q];
+    v.y = w[q + 1];
+    if constexpr (VW == 4) { v.z = w[q + 2]; v.w = w[q + 3]; }
+    *reinterpret_cast<V*>(p + q) = v;
+  }
+#pragma unroll
+  for (int q = (NF / VW) * VW; q < NF; ++q) p[q] = w[q];
+}
+
+// LDGSTS: one element, global -> shared, asynchronously
+template <class T>
+__device__ __forceinline__ void cp_async_elem(T* smem_dst, const T* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  if constexpr (sizeof(T) == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
+  else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 template <class T, int NF, int TX, int TY>
 struct TileGeom {
+  static constexpr int FS = Aos<T, NF>::FS;
   static constexpr int RW = TX + 4, RH = TY + 4, RP = RW * RH;   // ring plane (tile + radius-2 halo)
   static constexpr int NXF = (TX + 1) * TY, NYF = TX * (TY + 1);  // x / y faces per plane
   static constexpr int NCELL = TX * TY;
-  static constexpr int NBC = NCELL + 2 * TY + 2 * TX;             // cells that need face states
-  static constexpr size_t smem_elems = (size_t)3 * NF * RP + (size_t)3 * NF * NXF + (size_t)3 * NF * NYF;
+  static constexpr int NBC = NCELL + 2 * TY + 2 * TX;             // cells that need the predictor
+  static constexpr size_t smem_elems = (size_t)FS * (3 * RP + 2 * NXF + 2 * NYF);
   static constexpr size_t smem_bytes = smem_elems * sizeof(T);
 };
+
+// rotated component order handed to the 1-D Riemann routine: x -> (x,y,z), y -> (y,z,x), z -> (z,x,y)
+template <class T, int NF, int D>
+__device__ __forceinline__ void rotate_in(const T* w, T* r) {
+  constexpr int qn = 1 + D, q1 = 1 + (D + 1) % 3, q2 = 1 + (D + 2) % 3;
+  r[0] = w[0]; r[1] = w[qn]; r[2] = w[q1]; r[3] = w[q2]; r[4] = w[4];
+  if (NF == 9) { r[5] = w[4 + qn]; r[6] = w[4 + q1]; r[7] = w[4 + q2]; r[8] = w[8]; }
+}
+template <class T, int NF, int D>
+__device__ __forceinline__ void rotate_out(const T* r, T* f) {
+  constexpr int qn = 1 + D, q1 = 1 + (D + 1) % 3, q2 = 1 + (D + 2) % 3;
+  f[0] = r[0]; f[qn] = r[1]; f[q1] = r[2]; f[q2] = r[3]; f[4] = r[4];
+  if (NF == 9) { f[4 + qn] = r[5]; f[4 + q1] = r[6]; f[4 + q2] = r[7]; f[8] = r[8]; }
+}
 
 template <class T, int NF, int LIM, int RS, int TX, int TY, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB) godunov_step_kernel(const __grid_constant__ StepParams<T> P) {
   using G = TileGeom<T, NF, TX, TY>;
-  constexpr int RW = G::RW, RP = G::RP, NXF = G::NXF, NYF = G::NYF, NCELL = G::NCELL, NBC = G::NBC;
+  constexpr int FS = G::FS, RW = G::RW, RP = G::RP, NXF = G::NXF, NYF = G::NYF, NCELL = G::NCELL, NBC = G::NBC;
+  constexpr int LC = (RP + NT - 1) / NT;  // ring cells per thread in the plane loader
   static_assert(NT >= NBC, "one thread per predictor cell");
   static_assert(NT % 32 == 0, "whole warps");
+  static_assert(LC <= 8, "loader mask");
 
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* ring = reinterpret_cast<T*>(smem_raw);          // [3][NF][RP]
-  T* XL = ring + 3 * NF * RP;                        // [NF][NXF]  W^+_x of the cell left of the face
-  T* XR = XL + NF * NXF;                             // [NF][NXF]  W^-_x of the cell right of the face
-  T* FX = XR + NF * NXF;                             // [NF][NXF]
-  T* YL = FX + NF * NXF;                             // [NF][NYF]
-  T* YR = YL + NF * NYF;
-  T* FY = YR + NF * NYF;
+  T* const ring = reinterpret_cast<T*>(smem_raw);  // [3][RP][FS]   primitives
+  T* const XP = ring + 3 * RP * FS;                // [NXF][FS]     W^+_x of the cell left of the face
+  T* const YP = XP + NXF * FS;                     // [NYF][FS]     W^+_y of the cell below the face
+  T* const FX = YP + NYF * FS;                     // [NXF][FS]     x face fluxes
+  T* const FY = FX + NXF * FS;                     // [NYF][FS]     y face fluxes
   __shared__ int s_nbr[27];
   __shared__ int s_cnt[4];
   __shared__ T s_red[NT / 32];
@@ -304,7 +414,8 @@ __global__ void __launch_bounds__(NT, MINB) godunov_step_kernel(const __grid_con
   if (tid < 4) s_cnt[tid] = 0;
   __syncthreads();
 
-  const size_t n3 = (size_t)n * n * n;
+  const int n2 = n * n;
+  const size_t n3 = (size_t)n2 * n;
   const size_t fs_int = (size_t)P.np * n3;
   const int M = n + 2 * P.g;
   const size_t fs_halo = (size_t)P.np * M * M * M;
@@ -313,267 +424,283 @@ __global__ void __launch_bounds__(NT, MINB) godunov_step_kernel(const __grid_con
   RC.gamma = P.gamma; RC.igm1 = P.igm1; RC.ch2 = P.ch2; RC.half_ch = T(0.5) * P.ch; RC.half_ich = P.half_ich;
   RC.eps = P.eps;
 
-  // ---- phase A: one plane of U -> primitives -> ring slot -----------------------------------
-  auto load_plane = [&](int lz, int slot) {
-    const int rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
-    T* dst = ring + (size_t)slot * NF * RP;
-    for (int c = tid; c < RP; c += NT) {
+  // ---- plane loader (O0): raw U of plane lz -> ring slot, asynchronously ----------------------------
+  // ring cell c = ry*RW + rx  <->  patch-local (lx, ly) = (x0 + rx - 2, y0 + ry - 2); cells outside the
+  // stencil footprint (corners) are never touched.
+  unsigned lmask = 0;  // bit l: this thread's l-th loader cell exists
+#pragma unroll
+  for (int l = 0; l < LC; ++l) {
+    const int c = tid + l * NT;
+    if (c < RP) {
       const int ry = c / RW, rx = c - ry * RW;
       const int hx = rx < 2 ? 2 - rx : (rx >= TX + 2 ? rx - (TX + 1) : 0);
       const int hy = ry < 2 ? 2 - ry : (ry >= TY + 2 ? ry - (TY + 1) : 0);
-      if (hx + hy > 2) continue;  // outside the stencil footprint
-      const int lx = x0 + rx - 2, ly = y0 + ry - 2;
-      const int gx = lx < 0 ? 0 : (lx >= n ? 2 : 1), gy = ly < 0 ? 0 : (ly >= n ? 2 : 1);
-      const int e = s_nbr[rz * 9 + gy * 3 + gx];
-      const T* src;
-      size_t fs;
-      if (e >= 0) {
-        const int sp = e & NBR_PATCH_MASK, md = e >> NBR_MODE_SHIFT;
-        const int sx = (gx != 1 && (md & 1)) ? (gx == 0 ? 0 : n - 1) : lx - (gx - 1) * n;
-        const int sy = (gy != 1 && (md & 2)) ? (gy == 0 ? 0 : n - 1) : ly - (gy - 1) * n;
-        const int sz = (rz != 1 && (md & 4)) ? (rz == 0 ? 0 : n - 1) : lz - (rz - 1) * n;
-        src = P.Uin + (size_t)sp * n3 + ((size_t)sz * n + sy) * n + sx;
-        fs = fs_int;
-      } else {
-        src = P.halo + (size_t)p * M * M * M + ((size_t)(lz + P.g) * M + (ly + P.g)) * M + (lx + P.g);
-        fs = fs_halo;
-      }
-      T u[NF];
+      if (hx + hy <= 2) lmask |= 1u << l;
+    }
+  }
+  auto issue_plane = [&](int lz, T* dst) {
+    const int rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
 #pragma unroll
-      for (int q = 0; q < NF; ++q) u[q] = __ldg(src + q * fs);
-      const T ir = rrcp(u[0]);
-      const T vx = u[1] * ir, vy = u[2] * ir, vz = u[3] * ir;
-      T e_int = u[4] - T(0.5) * u[0] * (vx * vx + vy * vy + vz * vz);
-      if (NF == 9) e_int -= T(0.5) * (u[5] * u[5] + u[6] * u[6] + u[7] * u[7]);
-      dst[0 * RP + c] = u[0];
-      dst[1 * RP + c] = vx;
-      dst[2 * RP + c] = vy;
-      dst[3 * RP + c] = vz;
-      dst[4 * RP + c] = P.gm1 * e_int;
-      if (NF == 9) {
-        dst[5 * RP + c] = u[5]; dst[6 * RP + c] = u[6]; dst[7 * RP + c] = u[7]; dst[8 * RP + c] = u[8];
+    for (int l = 0; l < LC; ++l) {
+      if (lmask & (1u << l)) {
+        const int c = tid + l * NT;
+        const int ry = c / RW, rx = c - ry * RW;
+        const int lx = x0 + rx - 2, ly = y0 + ry - 2;
+        const int gx = lx < 0 ? 0 : (lx >= n ? 2 : 1), gy = ly < 0 ? 0 : (ly >= n ? 2 : 1);
+        const int e = s_nbr[rz * 9 + gy * 3 + gx];
+        const T* src;
+        size_t fs;
+        if (e >= 0) {
+          const int sp = e & NBR_PATCH_MASK, md = e >> NBR_MODE_SHIFT;
+          const int sx = (gx != 1 && (md & 1)) ? (gx == 0 ? 0 : n - 1) : lx - (gx - 1) * n;
+          const int sy = (gy != 1 && (md & 2)) ? (gy == 0 ? 0 : n - 1) : ly - (gy - 1) * n;
+          const int sz = (rz != 1 && (md & 4)) ? (rz == 0 ? 0 : n - 1) : lz - (rz - 1) * n;
+          src = P.Uin + ((size_t)sp * n3 + (size_t)((sz * n + sy) * n + sx));
+          fs = fs_int;
+        } else {
+          src = P.halo + ((size_t)p * M * M * M + (size_t)(((lz + P.g) * M + (ly + P.g)) * M + (lx + P.g)));
+          fs = fs_halo;
+        }
+        T* d = dst + c * FS;
+#pragma unroll
+        for (int q = 0; q < NF; ++q) cp_async_elem<T>(d + q, src + q * fs);
+      }
+    }
+  };
+  // O1 in place: conserved -> primitive, each thread on the cells it copied
+  auto convert_plane = [&](T* dst) {
+#pragma unroll
+    for (int l = 0; l < LC; ++l) {
+      if (lmask & (1u << l)) {
+        T* d = dst + (tid + l * NT) * FS;
+        T u[NF];
+        lds_cell<T, NF>(d, u);
+        const T ir = rrcp(u[0]);
+        const T vx = u[1] * ir, vy = u[2] * ir, vz = u[3] * ir;
+        T e_int = u[4] - T(0.5) * u[0] * (vx * vx + vy * vy + vz * vz);
+        if (NF == 9) e_int -= T(0.5) * (u[5] * u[5] + u[6] * u[6] + u[7] * u[7]);
+        u[1] = vx; u[2] = vy; u[3] = vz; u[4] = P.gm1 * e_int;
+        sts_cell<T, NF>(d, u);
       }
     }
   };
 
-  // per-thread role in phase B
-  const bool interior_thread = tid < NCELL;
-  int bi, bj;  // tile-local cell coordinates of this thread's predictor cell
+  // ---- per-thread role: one cell (bi, bj) of the tile grown by one layer, no corners ----------------
+  //   [0, NCELL)            interior cell: predictor, lower x/y/z faces, update
+  //   + TY, + TX            upper ring (bi = TX | bj = TY): predictor, the tile's last x | y face
+  //   + TY, + TX            lower ring (bi = -1 | bj = -1): predictor, publishes W^+_x | W^+_y
+  int bi, bj;
   if (tid < NCELL) { bj = tid / TX; bi = tid - bj * TX; }
-  else if (tid < NCELL + 2 * TY) { const int r = tid - NCELL; bj = r >> 1; bi = (r & 1) ? TX : -1; }
-  else { const int r = tid - NCELL - 2 * TY; bi = r >> 1; bj = (r & 1) ? TY : -1; }
-  const int bc = (bj + 2) * RW + (bi + 2);
+  else if (tid < NCELL + TY) { bi = TX; bj = tid - NCELL; }
+  else if (tid < NCELL + TY + TX) { bi = tid - (NCELL + TY); bj = TY; }
+  else if (tid < NCELL + 2 * TY + TX) { bi = -1; bj = tid - (NCELL + TY + TX); }
+  else { bi = tid - (NCELL + 2 * TY + TX); bj = -1; }
+  const bool interior = tid < NCELL;
+  const bool pred = tid < NBC;
+  const bool in_x = bi >= 0 && bi < TX, in_y = bj >= 0 && bj < TY;
+  const bool pub_x = pred && in_y && bi < TX;     // W^+_x feeds face bi+1 of row bj
+  const bool pub_y = pred && in_x && bj < TY;     // W^+_y feeds face bj+1 of column bi
+  const bool do_x = pred && in_y && bi >= 0;      // solves x face bi of row bj (interior, or bi = TX)
+  const bool do_y = pred && in_x && bj >= 0;      // solves y face bj of column bi
+  const int bc = pred ? (bj + 2) * RW + (bi + 2) : 0;
+  const int xf = do_x ? bj * (TX + 1) + bi : 0;   // x face to the left of this cell
+  const int yf = do_y ? bj * TX + bi : 0;         // y face below this cell
+  const size_t cell0 = (size_t)p * n3 + (size_t)((interior ? (y0 + bj) * n + (x0 + bi) : 0));
 
-  T zl[NF];    // W^+_z of the previous plane (left state of the next z face)
-  T fz[NF];    // flux through the lower z face of the current plane
-  T fzlo[NF];  // flux through the lower z face of the plane being accumulated
-  T acc[NF];   // (Fx+ - Fx-) + (Fy+ - Fy-) of the plane being accumulated
+  T zl[NF];     // W^+_z of the previous plane (left state of the next z face)
+  T fzlo[NF];   // flux through the lower z face of the plane whose update is pending
+  T acc[NF];    // (Fx+ - Fx-) + (Fy+ - Fy-) of the plane whose update is pending
+  T wmx[NF];    // W^-_x of the current plane (right state of this cell's lower x face)
+  T wmy[NF];    // W^-_y
   T smax_loc = T(0);
 #pragma unroll
-  for (int q = 0; q < NF; ++q) { zl[q] = T(0); fz[q] = T(0); fzlo[q] = T(0); acc[q] = T(0); }
+  for (int q = 0; q < NF; ++q) { zl[q] = T(0); fzlo[q] = T(0); acc[q] = T(0); wmx[q] = T(0); wmy[q] = T(0); }
 
-  load_plane(z0 - 2, 0);
-  load_plane(z0 - 1, 1);
+  T* Wm = ring;
+  T* Wc = ring + RP * FS;
+  T* Wp = ring + 2 * RP * FS;
+  issue_plane(z0 - 2, Wm);
+  issue_plane(z0 - 1, Wc);
+  issue_plane(z0, Wp);
+  cp_async_wait_all();
+  convert_plane(Wm);
+  convert_plane(Wc);
+  convert_plane(Wp);
+  __syncthreads();
+
+  const int blk = (P.fblk != nullptr) ? P.fblk_of[p] : -1;  // flux-register block of this patch
+  const size_t fsz = (size_t)n2 * (n + 1);
 
   for (int t = 0; t <= zc + 1; ++t) {
-    const int kk = z0 - 1 + t;  // plane being predicted
+    const int kk = z0 - 1 + t;               // plane being predicted
     const bool mid = (t >= 1) && (t <= zc);  // kk is a plane of this tile (x/y fluxes needed)
-    load_plane(kk + 1, (t + 2) % 3);
-    __syncthreads();
 
-    // ---- phase B ---------------------------------------------------------------------------
-    if (tid < (mid ? NBC : NCELL)) {
-      const T* Wm = ring + (size_t)(t % 3) * NF * RP;
-      const T* Wc = ring + (size_t)((t + 1) % 3) * NF * RP;
-      const T* Wp = ring + (size_t)((t + 2) % 3) * NF * RP;
-      T w[NF], Dx[NF], Dy[NF], Dz[NF];
+    // ---- phase 1: slopes, predictor, face states; z face; update of plane kk-1 ---------------------
+    if (mid ? pred : interior) {
+      T w[NF], hx[NF], hy[NF], hz[NF];
+      {
+        const T* cc = Wc + bc * FS;
+        T a[NF], b[NF];
+        lds_cell<T, NF>(cc, w);
+        lds_cell<T, NF>(cc - FS, a);
+        lds_cell<T, NF>(cc + FS, b);
 #pragma unroll
-      for (int q = 0; q < NF; ++q) {
-        const T c0 = Wc[q * RP + bc];
-        w[q] = c0;
-        Dx[q] = limited_slope<T, LIM>(c0 - Wc[q * RP + bc - 1], Wc[q * RP + bc + 1] - c0);
-        Dy[q] = limited_slope<T, LIM>(c0 - Wc[q * RP + bc - RW], Wc[q * RP + bc + RW] - c0);
-        Dz[q] = limited_slope<T, LIM>(c0 - Wm[q * RP + bc], Wp[q * RP + bc] - c0);
+        for (int q = 0; q < NF; ++q) hx[q] = half_slope<T, LIM>(w[q] - a[q], b[q] - w[q]);
+        lds_cell<T, NF>(cc - RW * FS, a);
+        lds_cell<T, NF>(cc + RW * FS, b);
+#pragma unroll
+        for (int q = 0; q < NF; ++q) hy[q] = half_slope<T, LIM>(w[q] - a[q], b[q] - w[q]);
+        lds_cell<T, NF>(Wm + bc * FS, a);
+        lds_cell<T, NF>(Wp + bc * FS, b);
+#pragma unroll
+        for (int q = 0; q < NF; ++q) hz[q] = half_slope<T, LIM>(w[q] - a[q], b[q] - w[q]);
       }
-      // O3 predictor
-      const T s = P.hdtdx;
+      // O3 predictor with half slopes: W* = W - (dt/dx) sum_d A_d h_d
+      const T s = P.dtdx;
       const T rho = w[0], pr = w[4];
       const T ir = rrcp(rho);
       T ws[NF];
-#define ADV(q) (w[1] * Dx[q] + w[2] * Dy[q] + w[3] * Dz[q])
-      const T divv = Dx[1] + Dy[2] + Dz[3];
+#define ADV(q) (w[1] * hx[q] + w[2] * hy[q] + w[3] * hz[q])
+      const T divv = hx[1] + hy[2] + hz[3];
       ws[0] = rho - s * (ADV(0) + rho * divv);
       if (NF == 5) {
-        ws[1] = w[1] - s * (ADV(1) + Dx[4] * ir);
-        ws[2] = w[2] - s * (ADV(2) + Dy[4] * ir);
-        ws[3] = w[3] - s * (ADV(3) + Dz[4] * ir);
+        ws[1] = w[1] - s * (ADV(1) + hx[4] * ir);
+        ws[2] = w[2] - s * (ADV(2) + hy[4] * ir);
+        ws[3] = w[3] - s * (ADV(3) + hz[4] * ir);
         ws[4] = pr - s * (ADV(4) + P.gamma * pr * divv);
       } else {
-#define BGRAD(q) (w[5] * Dx[q] + w[6] * Dy[q] + w[7] * Dz[q])
-        const T divB = Dx[5] + Dy[6] + Dz[7];
+#define BGRAD(q) (w[5] * hx[q] + w[6] * hy[q] + w[7] * hz[q])
+        const T divB = hx[5] + hy[6] + hz[7];
         const T vB = w[1] * w[5] + w[2] * w[6] + w[3] * w[7];
-        const T BdBx = w[5] * Dx[5] + w[6] * Dx[6] + w[7] * Dx[7];
-        const T BdBy = w[5] * Dy[5] + w[6] * Dy[6] + w[7] * Dy[7];
-        const T BdBz = w[5] * Dz[5] + w[6] * Dz[6] + w[7] * Dz[7];
-        ws[1] = w[1] - s * (ADV(1) + ((Dx[4] + BdBx) - (BGRAD(5) + w[5] * divB)) * ir);
-        ws[2] = w[2] - s * (ADV(2) + ((Dy[4] + BdBy) - (BGRAD(6) + w[6] * divB)) * ir);
-        ws[3] = w[3] - s * (ADV(3) + ((Dz[4] + BdBz) - (BGRAD(7) + w[7] * divB)) * ir);
-        ws[5] = w[5] - s * (ADV(5) + w[5] * divv - BGRAD(1) - w[1] * divB + Dx[8]);
-        ws[6] = w[6] - s * (ADV(6) + w[6] * divv - BGRAD(2) - w[2] * divB + Dy[8]);
-        ws[7] = w[7] - s * (ADV(7) + w[7] * divv - BGRAD(3) - w[3] * divB + Dz[8]);
+        const T BdBx = w[5] * hx[5] + w[6] * hx[6] + w[7] * hx[7];
+        const T BdBy = w[5] * hy[5] + w[6] * hy[6] + w[7] * hy[7];
+        const T BdBz = w[5] * hz[5] + w[6] * hz[6] + w[7] * hz[7];
+        ws[1] = w[1] - s * (ADV(1) + ((hx[4] + BdBx) - (BGRAD(5) + w[5] * divB)) * ir);
+        ws[2] = w[2] - s * (ADV(2) + ((hy[4] + BdBy) - (BGRAD(6) + w[6] * divB)) * ir);
+        ws[3] = w[3] - s * (ADV(3) + ((hz[4] + BdBz) - (BGRAD(7) + w[7] * divB)) * ir);
+        ws[5] = w[5] - s * (ADV(5) + w[5] * divv - BGRAD(1) - w[1] * divB + hx[8]);
+        ws[6] = w[6] - s * (ADV(6) + w[6] * divv - BGRAD(2) - w[2] * divB + hy[8]);
+        ws[7] = w[7] - s * (ADV(7) + w[7] * divv - BGRAD(3) - w[3] * divB + hz[8]);
         ws[4] = pr - s * (ADV(4) + P.gamma * pr * divv + P.gm1 * (vB * divB - BGRAD(8)));
         ws[8] = w[8] - s * P.ch2 * divB;
 #undef BGRAD
       }
 #undef ADV
       // O4 positivity: the smallest/largest of the six face values of rho and p
-      const T hr = T(0.5) * rmax(rmax(rabs(Dx[0]), rabs(Dy[0])), rabs(Dz[0]));
-      const T hp = T(0.5) * rmax(rmax(rabs(Dx[4]), rabs(Dy[4])), rabs(Dz[4]));
+      const T hr = rmax3(rabs(hx[0]), rabs(hy[0]), rabs(hz[0]));
+      const T hp = rmax3(rabs(hx[4]), rabs(hy[4]), rabs(hz[4]));
       const bool ok = (ws[0] - hr > T(0)) && (ws[4] - hp > T(0)) && (ws[0] + hr < rinf<T>()) &&
                       (ws[4] + hp < rinf<T>());
       if (!ok) {
         atomicAdd(&s_cnt[CNT_POSITIVITY], 1);
 #pragma unroll
-        for (int q = 0; q < NF; ++q) { ws[q] = w[q]; Dx[q] = T(0); Dy[q] = T(0); Dz[q] = T(0); }
+        for (int q = 0; q < NF; ++q) { ws[q] = w[q]; hx[q] = T(0); hy[q] = T(0); hz[q] = T(0); }
       }
       if (mid) {
-        // publish x / y face states: face fi lies between cells fi-1 and fi
-        if (bj >= 0 && bj < TY) {
-          const int row = bj * (TX + 1);
+        T fs_[NF];
+        if (pub_x) {
 #pragma unroll
-          for (int q = 0; q < NF; ++q) {
-            if (bi < TX) XL[q * NXF + row + bi + 1] = ws[q] + T(0.5) * Dx[q];
-            if (bi >= 0) XR[q * NXF + row + bi] = ws[q] - T(0.5) * Dx[q];
-          }
+          for (int q = 0; q < NF; ++q) fs_[q] = ws[q] + hx[q];
+          sts_cell<T, NF>(XP + (bj * (TX + 1) + bi + 1) * FS, fs_);
         }
-        if (bi >= 0 && bi < TX) {
+        if (pub_y) {
 #pragma unroll
-          for (int q = 0; q < NF; ++q) {
-            if (bj < TY) YL[q * NYF + (bj + 1) * TX + bi] = ws[q] + T(0.5) * Dy[q];
-            if (bj >= 0) YR[q * NYF + bj * TX + bi] = ws[q] - T(0.5) * Dy[q];
-          }
+          for (int q = 0; q < NF; ++q) fs_[q] = ws[q] + hy[q];
+          sts_cell<T, NF>(YP + ((bj + 1) * TX + bi) * FS, fs_);
         }
+#pragma unroll
+        for (int q = 0; q < NF; ++q) { wmx[q] = ws[q] - hx[q]; wmy[q] = ws[q] - hy[q]; }
       }
-      if (interior_thread) {
-        if (t >= 1) {  // z face between planes kk-1 and kk; rotated order (z, x, y)
-          T WL[NF], WR[NF], Fr[NF];
-          WL[0] = zl[0]; WL[1] = zl[3]; WL[2] = zl[1]; WL[3] = zl[2]; WL[4] = zl[4];
-          WR[0] = ws[0] - T(0.5) * Dz[0]; WR[1] = ws[3] - T(0.5) * Dz[3]; WR[2] = ws[1] - T(0.5) * Dz[1];
-          WR[3] = ws[2] - T(0.5) * Dz[2]; WR[4] = ws[4] - T(0.5) * Dz[4];
-          if (NF == 9) {
-            WL[5] = zl[7]; WL[6] = zl[5]; WL[7] = zl[6]; WL[8] = zl[8];
-            WR[5] = ws[7] - T(0.5) * Dz[7]; WR[6] = ws[5] - T(0.5) * Dz[5]; WR[7] = ws[6] - T(0.5) * Dz[6];
-            WR[8] = ws[8] - T(0.5) * Dz[8];
-          }
-          riemann<T, NF, RS>(WL, WR, RC, Fr, s_cnt);
-          fz[0] = Fr[0]; fz[3] = Fr[1]; fz[1] = Fr[2]; fz[2] = Fr[3]; fz[4] = Fr[4];
-          if (NF == 9) { fz[7] = Fr[5]; fz[5] = Fr[6]; fz[6] = Fr[7]; fz[8] = Fr[8]; }
-        }
+      if (interior) {
+        if (t >= 1) {  // z face between planes kk-1 and kk
+          T fz[NF];
+          {
+            T wr[NF], WL[NF], WR[NF], Fr[NF];
 #pragma unroll
-        for (int q = 0; q < NF; ++q) zl[q] = ws[q] + T(0.5) * Dz[q];
-      }
-    }
-    __syncthreads();
-
-    // ---- phase C: x and y faces of plane kk -----------------------------------------------
-    if (mid) {
-      for (int f = tid; f < NXF + NYF; f += NT) {
-        const int d = f >= NXF ? 1 : 0;
-        const int ff = f - d * NXF;
-        const int stride = d ? NYF : NXF;
-        const T* L = d ? YL : XL;
-        const T* R = d ? YR : XR;
-        T* Fo = d ? FY : FX;
-        const int qn = 1 + d, q1 = 1 + (d + 1) % 3, q2 = 1 + (d + 2) % 3;
-        T WL[NF], WR[NF], Fr[NF];
-        WL[0] = L[ff]; WR[0] = R[ff];
-        WL[1] = L[qn * stride + ff]; WR[1] = R[qn * stride + ff];
-        WL[2] = L[q1 * stride + ff]; WR[2] = R[q1 * stride + ff];
-        WL[3] = L[q2 * stride + ff]; WR[3] = R[q2 * stride + ff];
-        WL[4] = L[4 * stride + ff]; WR[4] = R[4 * stride + ff];
-        if (NF == 9) {
-          WL[5] = L[(4 + qn) * stride + ff]; WR[5] = R[(4 + qn) * stride + ff];
-          WL[6] = L[(4 + q1) * stride + ff]; WR[6] = R[(4 + q1) * stride + ff];
-          WL[7] = L[(4 + q2) * stride + ff]; WR[7] = R[(4 + q2) * stride + ff];
-          WL[8] = L[8 * stride + ff]; WR[8] = R[8 * stride + ff];
-        }
-        riemann<T, NF, RS>(WL, WR, RC, Fr, s_cnt);
-        Fo[ff] = Fr[0];
-        Fo[qn * stride + ff] = Fr[1];
-        Fo[q1 * stride + ff] = Fr[2];
-        Fo[q2 * stride + ff] = Fr[3];
-        Fo[4 * stride + ff] = Fr[4];
-        if (NF == 9) {
-          Fo[(4 + qn) * stride + ff] = Fr[5];
-          Fo[(4 + q1) * stride + ff] = Fr[6];
-          Fo[(4 + q2) * stride + ff] = Fr[7];
-          Fo[8 * stride + ff] = Fr[8];
-        }
-        if (P.fblk != nullptr) {  // record x / y face fluxes for the reflux
-          const int blk = P.fblk_of[p];
-          if (blk >= 0) {
-            const int a = d ? ff % TX : ff % (TX + 1), b = d ? ff / TX : ff / (TX + 1);
-            // a,b: tile-local (face or cell) coordinates along x and y
-            const bool owned = d ? (b < TY || y0 + TY == n) : (a < TX || x0 + TX == n);
-            if (owned) {
-              const size_t fsz = (size_t)n * n * (n + 1);
-              const size_t off = d ? (((size_t)kk * (n + 1) + (y0 + b)) * n + (x0 + a))
-                                   : (((size_t)kk * n + (y0 + b)) * (n + 1) + (x0 + a));
-              T* dstF = P.fblk + ((size_t)blk * 3 + d) * NF * fsz + off;
-              dstF[0] += Fr[0];
-              dstF[(size_t)qn * fsz] += Fr[1];
-              dstF[(size_t)q1 * fsz] += Fr[2];
-              dstF[(size_t)q2 * fsz] += Fr[3];
-              dstF[(size_t)4 * fsz] += Fr[4];
-              if (NF == 9) {
-                dstF[(size_t)(4 + qn) * fsz] += Fr[5];
-                dstF[(size_t)(4 + q1) * fsz] += Fr[6];
-                dstF[(size_t)(4 + q2) * fsz] += Fr[7];
-                dstF[(size_t)8 * fsz] += Fr[8];
-              }
+            for (int q = 0; q < NF; ++q) wr[q] = ws[q] - hz[q];
+            rotate_in<T, NF, 2>(zl, WL);
+            rotate_in<T, NF, 2>(wr, WR);
+            riemann<T, NF, RS>(WL, WR, RC, Fr, s_cnt);
+            rotate_out<T, NF, 2>(Fr, fz);
+          }
+          if (blk >= 0 && (t <= zc || z0 + zc == n)) {
+            T* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)kk * n2 + (size_t)((y0 + bj) * n + (x0 + bi)));
+#pragma unroll
+            for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += fz[q];
+          }
+          if (t >= 2) {  // O6 for plane kk-1, GLM damping, O7 of the new state
+            const size_t cell = cell0 + (size_t)(kk - 1) * n2;
+            T un[NF];
+#pragma unroll
+            for (int q = 0; q < NF; ++q) {
+              const T u = __ldg(P.Uin + q * fs_int + cell);
+              un[q] = u - P.dtdx * (acc[q] + (fz[q] - fzlo[q]));
             }
+            if (NF == 9) un[8] *= P.damp;
+#pragma unroll
+            for (int q = 0; q < NF; ++q) P.Uout[q * fs_int + cell] = un[q];
+            if (!(un[0] > T(0))) atomicAdd(&s_cnt[CNT_NEG_STATE], 1);
+            smax_loc = rmax(smax_loc, signal_speed<T, NF>(un, P.gamma, P.gm1));
           }
+#pragma unroll
+          for (int q = 0; q < NF; ++q) fzlo[q] = fz[q];
         }
+#pragma unroll
+        for (int q = 0; q < NF; ++q) zl[q] = ws[q] + hz[q];
       }
     }
+    if (t == zc + 1) break;
     __syncthreads();
 
-    // ---- phase D: finish plane kk-1, start accumulating plane kk ----------------------------
-    if (interior_thread) {
-      if (t >= 1 && P.fblk != nullptr) {  // z face flux (lower face of plane kk)
-        const int blk = P.fblk_of[p];
-        if (blk >= 0 && (t <= zc || z0 + zc == n)) {
-          const size_t fsz = (size_t)n * n * (n + 1);
-          T* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)kk * n + (y0 + bj)) * n + (x0 + bi);
+    // ---- phase 2: copies of plane kk+2; x / y Riemann problems of plane kk; convert plane kk+2 ------
+    issue_plane(kk + 2, Wm);
+    if (mid) {
+      if (do_x) {
+        T wl[NF], WL[NF], WR[NF], Fr[NF], f[NF];
+        lds_cell<T, NF>(XP + xf * FS, wl);
+        rotate_in<T, NF, 0>(wl, WL);
+        rotate_in<T, NF, 0>(wmx, WR);
+        riemann<T, NF, RS>(WL, WR, RC, Fr, s_cnt);
+        rotate_out<T, NF, 0>(Fr, f);
+        sts_cell<T, NF>(FX + xf * FS, f);
+        if (blk >= 0 && (bi < TX || x0 + TX == n)) {  // record the flux for the reflux
+          T* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + bj)) * (n + 1) + (x0 + bi));
 #pragma unroll
-          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += fz[q];
+          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += f[q];
         }
       }
-      if (t >= 2) {
-        const size_t cell = (size_t)p * n3 + ((size_t)(kk - 1) * n + (y0 + bj)) * n + (x0 + bi);
-        T un[NF];
+      if (do_y) {
+        T wl[NF], WL[NF], WR[NF], Fr[NF], f[NF];
+        lds_cell<T, NF>(YP + yf * FS, wl);
+        rotate_in<T, NF, 1>(wl, WL);
+        rotate_in<T, NF, 1>(wmy, WR);
+        riemann<T, NF, RS>(WL, WR, RC, Fr, s_cnt);
+        rotate_out<T, NF, 1>(Fr, f);
+        sts_cell<T, NF>(FY + yf * FS, f);
+        if (blk >= 0 && (bj < TY || y0 + TY == n)) {
+          T* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + (y0 + bj)) * n + (x0 + bi));
 #pragma unroll
-        for (int q = 0; q < NF; ++q) {
-          const T u = __ldg(P.Uin + q * fs_int + cell);
-          un[q] = u - P.dtdx * (acc[q] + (fz[q] - fzlo[q]));
-        }
-        if (NF == 9) un[8] *= P.damp;
-#pragma unroll
-        for (int q = 0; q < NF; ++q) P.Uout[q * fs_int + cell] = un[q];
-        if (!(un[0] > T(0))) atomicAdd(&s_cnt[CNT_NEG_STATE], 1);
-        smax_loc = rmax(smax_loc, signal_speed<T, NF>(un, P.gamma, P.gm1));
-      }
-      if (mid) {
-        const int xr = bj * (TX + 1) + bi, yr = bj * TX + bi;
-#pragma unroll
-        for (int q = 0; q < NF; ++q) {
-          acc[q] = (FX[q * NXF + xr + 1] - FX[q * NXF + xr]) + (FY[q * NYF + yr + TX] - FY[q * NYF + yr]);
-          fzlo[q] = fz[q];
+          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += f[q];
         }
       }
     }
-    // no barrier needed here: the next writers of FX/FY (phase C) and of the ring slot read by this
-    // iteration's phase B sit behind the barrier that follows the next load_plane
+    cp_async_wait_all();
+    convert_plane(Wm);
+    __syncthreads();
+
+    // ---- phase 3: x/y flux differences of plane kk -> registers ------------------------------------
+    if (interior && mid) {
+      T a[NF], b[NF], c[NF], d[NF];
+      lds_cell<T, NF>(FX + xf * FS, a);
+      lds_cell<T, NF>(FX + (xf + 1) * FS, b);
+      lds_cell<T, NF>(FY + yf * FS, c);
+      lds_cell<T, NF>(FY + (yf + TX) * FS, d);
+#pragma unroll
+      for (int q = 0; q < NF; ++q) acc[q] = (b[q] - a[q]) + (d[q] - c[q]);
+    }
+    T* tmp = Wm; Wm = Wc; Wc = Wp; Wp = tmp;
+    // no barrier here: the next writers of XP/YP (phase 1) are ordered behind this iteration's second
+    // barrier, FX/FY are next written behind the next iteration's first barrier
   }
 
   // ---- epilogue: max signal speed of the new state (O7), event counters -----------------------
