@@ -54,7 +54,10 @@ bool desc_ok(const amr_batch_desc* d, std::string* why) {
   if (d->dtype != AMR_F32 && d->dtype != AMR_F64) return bad("dtype must be AMR_F32 or AMR_F64");
   if (!(d->dx > 0) || !std::isfinite(d->dx)) return bad("dx must be finite and > 0");
   if (d->level < 0) return bad("level < 0");
-  if ((double)d->npatch * d->n * d->n * d->n > 2.0e9) return bad("more than 2e9 cells in one batch");
+  {  // the step kernel keeps per-field element offsets (interiors and ghosted halo buffer) in 32 bits
+    const double M = d->n + 2.0 * d->nghost;
+    if ((double)d->npatch * M * M * M > 2.0e9) return bad("more than 2e9 (ghosted) cells in one batch");
+  }
   if (!d->self_periodic) {
     if (!d->origin) return bad("null origin");
     for (int a = 0; a < 3; ++a)

@@ -25,6 +25,7 @@
 // fp32 arithmetic uses the SFU approximations (rcp/sqrt/rsqrt .approx.ftz, <= 2 ulp) instead of the
 // IEEE sequences (12 issue slots each, measured): DESIGN.md §3 "arithmetic freedom"; fp64 is IEEE.
 #pragma once
+#include <cstdio>
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
@@ -353,7 +354,9 @@ __device__ __forceinline__ void cp_async_elem(T* smem_dst, const T* gsrc) {
   if constexpr (sizeof(T) == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
   else asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
 }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 template <class T, int NF, int TX, int TY>
 struct TileGeom {
@@ -362,7 +365,8 @@ struct TileGeom {
   static constexpr int NXF = (TX + 1) * TY, NYF = TX * (TY + 1);  // x / y faces per plane
   static constexpr int NCELL = TX * TY;
   static constexpr int NBC = NCELL + 2 * TY + 2 * TX;             // cells that need the predictor
-  static constexpr size_t smem_elems = (size_t)FS * (3 * RP + 2 * NXF + 2 * NYF);
+  static constexpr int NSLOT = 4;                                 // ring planes: k-1, k, k+1 and k+2 in flight
+  static constexpr size_t smem_elems = (size_t)FS * (NSLOT * RP + NXF + NYF) + (size_t)2 * 4 * NCELL;
   static constexpr size_t smem_bytes = smem_elems * sizeof(T);
 };
 
@@ -380,21 +384,20 @@ __device__ __forceinline__ void rotate_out(const T* r, T* f) {
   if (NF == 9) { f[4 + qn] = r[5]; f[4 + q1] = r[6]; f[4 + q2] = r[7]; f[8] = r[8]; }
 }
 
-template <class T, int NF, int LIM, int RS, int TX, int TY, int NT, int MINB>
-__global__ void __launch_bounds__(NT, MINB) godunov_step_kernel(const __grid_constant__ StepParams<T> P) {
+template <class T, int NF, int LIM, int RS, int TX, int TY, int NT, int MAXR>
+__global__ void __maxnreg__(MAXR) godunov_step_kernel(const __grid_constant__ StepParams<T> P) {
   using G = TileGeom<T, NF, TX, TY>;
   constexpr int FS = G::FS, RW = G::RW, RP = G::RP, NXF = G::NXF, NYF = G::NYF, NCELL = G::NCELL, NBC = G::NBC;
   constexpr int LC = (RP + NT - 1) / NT;  // ring cells per thread in the plane loader
   static_assert(NT >= NBC, "one thread per predictor cell");
   static_assert(NT % 32 == 0, "whole warps");
-  static_assert(LC <= 8, "loader mask");
+  static_assert(LC <= 8, "loader masks");
 
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  T* const ring = reinterpret_cast<T*>(smem_raw);  // [3][RP][FS]   primitives
-  T* const XP = ring + 3 * RP * FS;                // [NXF][FS]     W^+_x of the cell left of the face
-  T* const YP = XP + NXF * FS;                     // [NYF][FS]     W^+_y of the cell below the face
-  T* const FX = YP + NYF * FS;                     // [NXF][FS]     x face fluxes
-  T* const FY = FX + NXF * FS;                     // [NYF][FS]     y face fluxes
+  T* const ring = reinterpret_cast<T*>(smem_raw);  // [4][RP][FS]   primitives (raw U while in flight)
+  T* const XF = ring + G::NSLOT * RP * FS;         // [NXF][FS]     W^+_x of the cell left of the face, then the x flux
+  T* const YF = XF + NXF * FS;                     // [NYF][FS]     W^+_y of the cell below the face, then the y flux
+  T* const UO = YF + NYF * FS;                     // [2][NCELL][4] (m_x, m_y, m_z, E) of the cell awaiting its update
   __shared__ int s_nbr[27];
   __shared__ int s_cnt[4];
   __shared__ T s_red[NT / 32];
@@ -415,10 +418,11 @@ __global__ void __launch_bounds__(NT, MINB) godunov_step_kernel(const __grid_con
   __syncthreads();
 
   const int n2 = n * n;
-  const size_t n3 = (size_t)n2 * n;
+  const int n3 = n2 * n;                     // host guarantees np * (n+2g)^3 < 2^31
   const size_t fs_int = (size_t)P.np * n3;
   const int M = n + 2 * P.g;
-  const size_t fs_halo = (size_t)P.np * M * M * M;
+  const int M2 = M * M;
+  const size_t fs_halo = (size_t)P.np * M2 * M;
 
   RiemannConst<T> RC;
   RC.gamma = P.gamma; RC.igm1 = P.igm1; RC.ch2 = P.ch2; RC.half_ch = T(0.5) * P.ch; RC.half_ich = P.half_ich;
@@ -426,7 +430,10 @@ __global__ void __launch_bounds__(NT, MINB) godunov_step_kernel(const __grid_con
 
   // ---- plane loader (O0): raw U of plane lz -> ring slot, asynchronously ----------------------------
   // ring cell c = ry*RW + rx  <->  patch-local (lx, ly) = (x0 + rx - 2, y0 + ry - 2); cells outside the
-  // stencil footprint (corners) are never touched.
+  // stencil footprint (corners) are never touched.  Per z region (below / inside / above the patch) the
+  // source of a cell is fixed up to the z term, so its offset is resolved once per region:
+  //   goff[l]  element offset of (source patch, z = 0, sy, sx)      hmask  source is the prolongation halo
+  //   zmask    the z index is clamped (outflow)
   unsigned lmask = 0;  // bit l: this thread's l-th loader cell exists
 #pragma unroll
   for (int l = 0; l < LC; ++l) {
@@ -438,30 +445,48 @@ __global__ void __launch_bounds__(NT, MINB) godunov_step_kernel(const __grid_con
       if (hx + hy <= 2) lmask |= 1u << l;
     }
   }
-  auto issue_plane = [&](int lz, T* dst) {
-    const int rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
+  int goff[LC];
+  unsigned hmask = 0, zmask = 0;
+  int cur_rz = -1;
+  auto setup_region = [&](int rz) {
+    hmask = 0; zmask = 0;
 #pragma unroll
     for (int l = 0; l < LC; ++l) {
+      goff[l] = 0;
       if (lmask & (1u << l)) {
         const int c = tid + l * NT;
         const int ry = c / RW, rx = c - ry * RW;
         const int lx = x0 + rx - 2, ly = y0 + ry - 2;
         const int gx = lx < 0 ? 0 : (lx >= n ? 2 : 1), gy = ly < 0 ? 0 : (ly >= n ? 2 : 1);
         const int e = s_nbr[rz * 9 + gy * 3 + gx];
-        const T* src;
-        size_t fs;
         if (e >= 0) {
           const int sp = e & NBR_PATCH_MASK, md = e >> NBR_MODE_SHIFT;
           const int sx = (gx != 1 && (md & 1)) ? (gx == 0 ? 0 : n - 1) : lx - (gx - 1) * n;
           const int sy = (gy != 1 && (md & 2)) ? (gy == 0 ? 0 : n - 1) : ly - (gy - 1) * n;
-          const int sz = (rz != 1 && (md & 4)) ? (rz == 0 ? 0 : n - 1) : lz - (rz - 1) * n;
-          src = P.Uin + ((size_t)sp * n3 + (size_t)((sz * n + sy) * n + sx));
-          fs = fs_int;
+          if (rz != 1 && (md & 4)) zmask |= 1u << l;
+          goff[l] = sp * n3 + sy * n + sx;
         } else {
-          src = P.halo + ((size_t)p * M * M * M + (size_t)(((lz + P.g) * M + (ly + P.g)) * M + (lx + P.g)));
-          fs = fs_halo;
+          hmask |= 1u << l;
+          goff[l] = p * (M2 * M) + (ly + P.g) * M + (lx + P.g);
         }
-        T* d = dst + c * FS;
+      }
+    }
+    cur_rz = rz;
+  };
+  auto issue_plane = [&](int lz, T* dst) {
+    const int rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
+    if (rz != cur_rz) setup_region(rz);
+    const int zt_int = (lz - (rz - 1) * n) * n2;
+    const int zt_clamp = (rz == 0 ? 0 : n - 1) * n2;
+    const int zt_halo = (lz + P.g) * M2;
+#pragma unroll
+    for (int l = 0; l < LC; ++l) {
+      if (lmask & (1u << l)) {
+        const bool fh = hmask & (1u << l);
+        const int off = goff[l] + (fh ? zt_halo : ((zmask & (1u << l)) ? zt_clamp : zt_int));
+        const T* src = (fh ? P.halo : P.Uin) + off;
+        const size_t fs = fh ? fs_halo : fs_int;
+        T* d = dst + (tid + l * NT) * FS;
 #pragma unroll
         for (int q = 0; q < NF; ++q) cp_async_elem<T>(d + q, src + q * fs);
       }
@@ -503,26 +528,30 @@ __global__ void __launch_bounds__(NT, MINB) godunov_step_kernel(const __grid_con
   const bool do_x = pred && in_y && bi >= 0;      // solves x face bi of row bj (interior, or bi = TX)
   const bool do_y = pred && in_x && bj >= 0;      // solves y face bj of column bi
   const int bc = pred ? (bj + 2) * RW + (bi + 2) : 0;
-  const int xf = do_x ? bj * (TX + 1) + bi : 0;   // x face to the left of this cell
-  const int yf = do_y ? bj * TX + bi : 0;         // y face below this cell
-  const size_t cell0 = (size_t)p * n3 + (size_t)((interior ? (y0 + bj) * n + (x0 + bi) : 0));
+  T* const xfp = XF + (do_x ? bj * (TX + 1) + bi : 0) * FS;   // x face to the left of this cell
+  T* const yfp = YF + (do_y ? bj * TX + bi : 0) * FS;         // y face below this cell
+  const int cell0 = interior ? p * n3 + (y0 + bj) * n + (x0 + bi) : 0;
+  T* const uo = UO + (interior ? tid * 4 : 0);
 
   T zl[NF];     // W^+_z of the previous plane (left state of the next z face)
-  T fzlo[NF];   // flux through the lower z face of the plane whose update is pending
-  T acc[NF];    // (Fx+ - Fx-) + (Fy+ - Fy-) of the plane whose update is pending
-  T wmx[NF];    // W^-_x of the current plane (right state of this cell's lower x face)
-  T wmy[NF];    // W^-_y
+  T dU[NF];     // flux sum of the plane whose update is pending: ((Fx+ - Fx-) + (Fy+ - Fy-)) - Fz-
+  T wmx[NF];    // W^-_x of the current plane (right state of this cell's lower x face), then its x flux
+  T wmy[NF];    // W^-_y, then the y flux
   T smax_loc = T(0);
 #pragma unroll
-  for (int q = 0; q < NF; ++q) { zl[q] = T(0); fzlo[q] = T(0); acc[q] = T(0); wmx[q] = T(0); wmy[q] = T(0); }
+  for (int q = 0; q < NF; ++q) { zl[q] = T(0); dU[q] = T(0); wmx[q] = T(0); wmy[q] = T(0); }
 
   T* Wm = ring;
   T* Wc = ring + RP * FS;
   T* Wp = ring + 2 * RP * FS;
+  T* Wn = ring + 3 * RP * FS;
   issue_plane(z0 - 2, Wm);
   issue_plane(z0 - 1, Wc);
   issue_plane(z0, Wp);
-  cp_async_wait_all();
+  cp_async_commit();
+  issue_plane(z0 + 1, Wn);
+  cp_async_commit();
+  cp_async_wait_group<1>();
   convert_plane(Wm);
   convert_plane(Wc);
   convert_plane(Wp);
@@ -601,23 +630,24 @@ __global__ void __launch_bounds__(NT, MINB) godunov_step_kernel(const __grid_con
         if (pub_x) {
 #pragma unroll
           for (int q = 0; q < NF; ++q) fs_[q] = ws[q] + hx[q];
-          sts_cell<T, NF>(XP + (bj * (TX + 1) + bi + 1) * FS, fs_);
+          sts_cell<T, NF>(XF + (bj * (TX + 1) + bi + 1) * FS, fs_);
         }
         if (pub_y) {
 #pragma unroll
           for (int q = 0; q < NF; ++q) fs_[q] = ws[q] + hy[q];
-          sts_cell<T, NF>(YP + ((bj + 1) * TX + bi) * FS, fs_);
+          sts_cell<T, NF>(YF + ((bj + 1) * TX + bi) * FS, fs_);
         }
 #pragma unroll
         for (int q = 0; q < NF; ++q) { wmx[q] = ws[q] - hx[q]; wmy[q] = ws[q] - hy[q]; }
       }
       if (interior) {
+        T wr[NF], zn[NF];
+#pragma unroll
+        for (int q = 0; q < NF; ++q) { wr[q] = ws[q] - hz[q]; zn[q] = ws[q] + hz[q]; }
         if (t >= 1) {  // z face between planes kk-1 and kk
           T fz[NF];
           {
-            T wr[NF], WL[NF], WR[NF], Fr[NF];
-#pragma unroll
-            for (int q = 0; q < NF; ++q) wr[q] = ws[q] - hz[q];
+            T WL[NF], WR[NF], Fr[NF];
             rotate_in<T, NF, 2>(zl, WL);
             rotate_in<T, NF, 2>(wr, WR);
             riemann<T, NF, RS>(WL, WR, RC, Fr, s_cnt);
@@ -629,78 +659,99 @@ __global__ void __launch_bounds__(NT, MINB) godunov_step_kernel(const __grid_con
             for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += fz[q];
           }
           if (t >= 2) {  // O6 for plane kk-1, GLM damping, O7 of the new state
-            const size_t cell = cell0 + (size_t)(kk - 1) * n2;
+            // U_old: rho, B, psi are the ring record of plane kk-1 (conversion leaves them untouched),
+            // m and E were staged two iterations ago
             T un[NF];
-#pragma unroll
-            for (int q = 0; q < NF; ++q) {
-              const T u = __ldg(P.Uin + q * fs_int + cell);
-              un[q] = u - P.dtdx * (acc[q] + (fz[q] - fzlo[q]));
+            const T* om = Wm + bc * FS;
+            un[0] = om[0];
+            if (NF == 9) { un[5] = om[5]; un[6] = om[6]; un[7] = om[7]; un[8] = om[8]; }
+            {
+              const T* ou = uo + ((t & 1) ? 4 * NCELL : 0);
+              using V = typename Vec<T, Aos<T, 9>::VW>::type;
+              if constexpr (sizeof(T) == 4) {
+                const V v = *reinterpret_cast<const V*>(ou);
+                un[1] = v.x; un[2] = v.y; un[3] = v.z; un[4] = v.w;
+              } else {
+                const V v0 = *reinterpret_cast<const V*>(ou), v1 = *reinterpret_cast<const V*>(ou + 2);
+                un[1] = v0.x; un[2] = v0.y; un[3] = v1.x; un[4] = v1.y;
+              }
             }
-            if (NF == 9) un[8] *= P.damp;
 #pragma unroll
-            for (int q = 0; q < NF; ++q) P.Uout[q * fs_int + cell] = un[q];
+            for (int q = 0; q < NF; ++q) un[q] = un[q] - P.dtdx * (dU[q] + fz[q]);
+            if (NF == 9) un[8] *= P.damp;
+            T* out = P.Uout + (cell0 + (kk - 1) * n2);
+#pragma unroll
+            for (int q = 0; q < NF; ++q) out[q * fs_int] = un[q];
             if (!(un[0] > T(0))) atomicAdd(&s_cnt[CNT_NEG_STATE], 1);
             smax_loc = rmax(smax_loc, signal_speed<T, NF>(un, P.gamma, P.gm1));
           }
 #pragma unroll
-          for (int q = 0; q < NF; ++q) fzlo[q] = fz[q];
+          for (int q = 0; q < NF; ++q) dU[q] = -fz[q];
         }
 #pragma unroll
-        for (int q = 0; q < NF; ++q) zl[q] = ws[q] + hz[q];
+        for (int q = 0; q < NF; ++q) zl[q] = zn[q];
       }
     }
     if (t == zc + 1) break;
     __syncthreads();
 
-    // ---- phase 2: copies of plane kk+2; x / y Riemann problems of plane kk; convert plane kk+2 ------
-    issue_plane(kk + 2, Wm);
+    // ---- phase 2: copies of plane kk+3 and of (m, E) of plane kk+1; x / y Riemann problems of plane kk;
+    //      convert plane kk+2 (its copies were issued one iteration ago) ---------------------------------
+    if (t <= zc - 1) {
+      issue_plane(kk + 3, Wm);
+      if (interior) {
+        const T* src = P.Uin + (cell0 + (kk + 1) * n2);
+        T* d = uo + ((t & 1) ? 4 * NCELL : 0);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) cp_async_elem<T>(d + q, src + (q + 1) * fs_int);
+      }
+    }
+    cp_async_commit();
     if (mid) {
       if (do_x) {
-        T wl[NF], WL[NF], WR[NF], Fr[NF], f[NF];
-        lds_cell<T, NF>(XP + xf * FS, wl);
+        T wl[NF], WL[NF], WR[NF], Fr[NF];
+        lds_cell<T, NF>(xfp, wl);
         rotate_in<T, NF, 0>(wl, WL);
         rotate_in<T, NF, 0>(wmx, WR);
         riemann<T, NF, RS>(WL, WR, RC, Fr, s_cnt);
-        rotate_out<T, NF, 0>(Fr, f);
-        sts_cell<T, NF>(FX + xf * FS, f);
+        rotate_out<T, NF, 0>(Fr, wmx);
+        sts_cell<T, NF>(xfp, wmx);
         if (blk >= 0 && (bi < TX || x0 + TX == n)) {  // record the flux for the reflux
           T* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + bj)) * (n + 1) + (x0 + bi));
 #pragma unroll
-          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += f[q];
+          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += wmx[q];
         }
       }
       if (do_y) {
-        T wl[NF], WL[NF], WR[NF], Fr[NF], f[NF];
-        lds_cell<T, NF>(YP + yf * FS, wl);
+        T wl[NF], WL[NF], WR[NF], Fr[NF];
+        lds_cell<T, NF>(yfp, wl);
         rotate_in<T, NF, 1>(wl, WL);
         rotate_in<T, NF, 1>(wmy, WR);
         riemann<T, NF, RS>(WL, WR, RC, Fr, s_cnt);
-        rotate_out<T, NF, 1>(Fr, f);
-        sts_cell<T, NF>(FY + yf * FS, f);
+        rotate_out<T, NF, 1>(Fr, wmy);
+        sts_cell<T, NF>(yfp, wmy);
         if (blk >= 0 && (bj < TY || y0 + TY == n)) {
           T* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + (y0 + bj)) * n + (x0 + bi));
 #pragma unroll
-          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += f[q];
+          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += wmy[q];
         }
       }
     }
-    cp_async_wait_all();
-    convert_plane(Wm);
+    cp_async_wait_group<1>();
+    convert_plane(Wn);
     __syncthreads();
 
     // ---- phase 3: x/y flux differences of plane kk -> registers ------------------------------------
+    // (own fluxes are in wmx / wmy; the upper ones are read from the slots this very thread overwrites
+    // with its W^+ in the next phase 1, so no barrier is needed before that)
     if (interior && mid) {
-      T a[NF], b[NF], c[NF], d[NF];
-      lds_cell<T, NF>(FX + xf * FS, a);
-      lds_cell<T, NF>(FX + (xf + 1) * FS, b);
-      lds_cell<T, NF>(FY + yf * FS, c);
-      lds_cell<T, NF>(FY + (yf + TX) * FS, d);
+      T b[NF], d[NF];
+      lds_cell<T, NF>(xfp + FS, b);
+      lds_cell<T, NF>(yfp + TX * FS, d);
 #pragma unroll
-      for (int q = 0; q < NF; ++q) acc[q] = (b[q] - a[q]) + (d[q] - c[q]);
+      for (int q = 0; q < NF; ++q) dU[q] = ((b[q] - wmx[q]) + (d[q] - wmy[q])) + dU[q];
     }
-    T* tmp = Wm; Wm = Wc; Wc = Wp; Wp = tmp;
-    // no barrier here: the next writers of XP/YP (phase 1) are ordered behind this iteration's second
-    // barrier, FX/FY are next written behind the next iteration's first barrier
+    T* tmp = Wm; Wm = Wc; Wc = Wp; Wp = Wn; Wn = tmp;
   }
 
   // ---- epilogue: max signal speed of the new state (O7), event counters -----------------------
@@ -718,11 +769,11 @@ __global__ void __launch_bounds__(NT, MINB) godunov_step_kernel(const __grid_con
   if (tid < 4 && s_cnt[tid] != 0) atomicAdd(P.counters + tid, (unsigned long long)s_cnt[tid]);
 }
 
-// host-side launcher for one (T, NF, TX, TY, NT, MINB) tile configuration
-template <class T, int NF, int LIM, int RS, int TX, int TY, int NT, int MINB>
+// host-side launcher for one (T, NF, TX, TY, NT, MAXR) tile configuration
+template <class T, int NF, int LIM, int RS, int TX, int TY, int NT, int MAXR>
 cudaError_t launch_variant(const StepParams<T>& P, cudaStream_t s) {
   using G = TileGeom<T, NF, TX, TY>;
-  auto kern = godunov_step_kernel<T, NF, LIM, RS, TX, TY, NT, MINB>;
+  auto kern = godunov_step_kernel<T, NF, LIM, RS, TX, TY, NT, MAXR>;
   static bool configured = false;  // per instantiation; attribute is per device function
   if (!configured) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
@@ -731,14 +782,21 @@ cudaError_t launch_variant(const StepParams<T>& P, cudaStream_t s) {
   }
   const long long grid = (long long)P.np * P.ntx * P.nty * P.ntz;
   kern<<<(unsigned)grid, NT, G::smem_bytes, s>>>(P);
-  return cudaGetLastError();
+  cudaError_t le = cudaGetLastError();
+  if (le != cudaSuccess) {
+    cudaFuncAttributes fa;
+    if (cudaFuncGetAttributes(&fa, kern) == cudaSuccess)
+      fprintf(stderr, "amr: step kernel launch failed: %d threads, %d regs/thread, %zu B dynamic + %zu B static smem, maxThreadsPerBlock %d\n",
+              NT, fa.numRegs, (size_t)G::smem_bytes, fa.sharedSizeBytes, fa.maxThreadsPerBlock);
+  }
+  return le;
 }
 
-template <class T, int NF, int TX, int TY, int NT, int MINB>
+template <class T, int NF, int TX, int TY, int NT, int MAXR>
 cudaError_t launch_dispatch(const StepParams<T>& P, int limiter, int riemann, cudaStream_t s) {
   constexpr int RSX = (NF == 5) ? RS_HLLC : RS_HLLD;
 #define AMR_CASE(L, R) \
-  if (limiter == L && riemann == R) return launch_variant<T, NF, L, R, TX, TY, NT, MINB>(P, s);
+  if (limiter == L && riemann == R) return launch_variant<T, NF, L, R, TX, TY, NT, MAXR>(P, s);
   AMR_CASE(LIM_NONE, RS_HLL)
   AMR_CASE(LIM_MINMOD, RS_HLL)
   AMR_CASE(LIM_MC, RS_HLL)

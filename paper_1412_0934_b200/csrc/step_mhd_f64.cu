@@ -12,8 +12,8 @@ void tile_shape_mhd_f64(int n, int* tx, int* ty) {
 cudaError_t launch_step_mhd_f64(const StepParams<double>& P, int limiter, int riemann, cudaStream_t s) {
   using C = TileCfg_mhd_f64;
   if (P.n % C::TX == 0 && P.n % C::TY == 0)
-    return launch_dispatch<double, 9, C::TX, C::TY, C::NT, C::MINB>(P, limiter, riemann, s);
-  return launch_dispatch<double, 9, 8, 8, 96, 2>(P, limiter, riemann, s);
+    return launch_dispatch<double, 9, C::TX, C::TY, C::NT, C::MAXR>(P, limiter, riemann, s);
+  return launch_dispatch<double, 9, 8, 8, 96, 255>(P, limiter, riemann, s);
 }
 
 }  // namespace amr
