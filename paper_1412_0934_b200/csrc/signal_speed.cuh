@@ -1,9 +1,14 @@
 // O7 (reading A9): max over directions of |v_d| + c_d for one cell, from its conserved state.
-// Used by the fused epilogue of the step kernel and by the standalone reduction (amr_cfl_dt); written
-// with explicitly rounded intrinsics (no FMA contraction) so that both kernels give bitwise the same
-// number for the same stored state (pin P15).
+// Used by the fused epilogue of the step kernels and by the standalone reduction (amr_cfl_dt); written
+// with explicitly rounded intrinsics (no FMA contraction) so that all kernels give bitwise the same
+// number for the same stored state (pin P15).  T = double: IEEE divide and square root.  T = float and
+// T = x2::F2 (two cells at once): the SFU reciprocal and square root (<= 2 ulp each, deterministic), like
+// the rest of the fp32 path; the packed *_rn operations round exactly like the scalar ones, so the F2
+// instantiation gives the float one's bits in each half.
 #pragma once
 #include <cuda_runtime.h>
+
+#include "pair_math.cuh"
 
 namespace amr {
 
@@ -11,14 +16,20 @@ __device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, 
 __device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
 __device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
 __device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
-__device__ __forceinline__ float div_rn(float a, float b) { return __fdiv_rn(a, b); }
+__device__ __forceinline__ float div_rn(float a, float b) { return __fmul_rn(a, x2::rcpf(b)); }
 __device__ __forceinline__ double div_rn(double a, double b) { return __ddiv_rn(a, b); }
-__device__ __forceinline__ float sqrt_rn(float a) { return __fsqrt_rn(a); }
+__device__ __forceinline__ float sqrt_rn(float a) { return x2::sqrtf_(a); }
 __device__ __forceinline__ double sqrt_rn(double a) { return __dsqrt_rn(a); }
 __device__ __forceinline__ float max_(float a, float b) { return fmaxf(a, b); }
 __device__ __forceinline__ double max_(double a, double b) { return fmax(a, b); }
 __device__ __forceinline__ float abs_(float a) { return fabsf(a); }
 __device__ __forceinline__ double abs_(double a) { return fabs(a); }
+__device__ __forceinline__ x2::F2 mul_rn(x2::F2 a, x2::F2 b) { return a * b; }
+__device__ __forceinline__ x2::F2 add_rn(x2::F2 a, x2::F2 b) { return a + b; }
+__device__ __forceinline__ x2::F2 div_rn(x2::F2 a, x2::F2 b) { return a * x2::rcp2(b); }
+__device__ __forceinline__ x2::F2 sqrt_rn(x2::F2 a) { return x2::sqrt2(a); }
+__device__ __forceinline__ x2::F2 max_(x2::F2 a, x2::F2 b) { return x2::max2(a, b); }
+__device__ __forceinline__ x2::F2 abs_(x2::F2 a) { return x2::abs2(a); }
 
 template <class T, int NF>
 __device__ __forceinline__ T signal_speed(const T* u, T gamma, T gm1) {

@@ -1,11 +1,25 @@
-// Tile shapes of the fused step kernel per (physics, dtype): TX x TY interior cells per CTA column,
-// NT threads (>= TX*TY + 2*TX + 2*TY, whole warps), MAXR = register cap per thread (__maxnreg__), which
-// with NT and the shared-memory footprint fixes the CTAs per SM.
-// Chosen from ptxas -v (registers / spills) and the shared-memory budget.
+// Tile shapes of the fused step kernels per (physics, dtype): TX x TY interior cells per CTA column,
+// NT threads (whole warps), MAXR = register cap per thread (__maxnreg__), which with NT and the
+// shared-memory footprint fixes the CTAs per SM.  Chosen from ptxas -v (registers / spills), the
+// shared-memory budget and measured step times.
+//   fp32: two cells per thread (godunov_step_x2.cuh): TX/2*TY interior pair threads (whole warps) plus the
+//         aux warps (ring pairs + loader), NT >= TX/2*TY + 2*TY + TX; W = tile for n % 32 == 0, S = tile for
+//         the other multiples of 16; test-size patches (n = 8) run the scalar 8x8 tile
+//   fp64: one cell per thread (godunov_step.cuh), NT >= TX*TY + 2*TX + 2*TY
+// The AMR_TUNE_* macros exist for tuning sweeps only (one -D per value); the defaults are the product.
 #pragma once
+#ifndef AMR_TUNE_F32_WTX
+#define AMR_TUNE_F32_WTX 32
+#define AMR_TUNE_F32_WTY 8
+#define AMR_TUNE_F32_NT 192
+#define AMR_TUNE_F32_MAXR 168
+#endif
 namespace amr {
-struct TileCfg_hydro_f32 { static constexpr int TX = 16, TY = 16, NT = 320, MAXR = 96; };
+struct TileCfg_hydro_f32 { static constexpr int WTX = 32, WTY = 8, STX = 16, STY = 16, NT = 192, MAXR = 168; };
+struct TileCfg_mhd_f32 {
+  static constexpr int WTX = AMR_TUNE_F32_WTX, WTY = AMR_TUNE_F32_WTY, STX = 16, STY = 16, NT = 192, WNT = AMR_TUNE_F32_NT,
+                       MAXR = 168, WMAXR = AMR_TUNE_F32_MAXR;
+};
 struct TileCfg_hydro_f64 { static constexpr int TX = 16, TY = 16, NT = 320, MAXR = 168; };
-struct TileCfg_mhd_f32 { static constexpr int TX = 16, TY = 8, NT = 192, MAXR = 128; };
 struct TileCfg_mhd_f64 { static constexpr int TX = 16, TY = 8, NT = 192, MAXR = 255; };
 }  // namespace amr
