@@ -216,7 +216,7 @@ __device__ __forceinline__ int predict_pair(const float* Wm, const float* Wc, co
   const F2 inf = F2(CUDART_INF_F);
   const B2 ok = gt(ws[0] - hr, 0.f) & gt(ws[4] - hp, 0.f) & lt(ws[0] + hr, inf) & lt(ws[4] + hp, inf);
   const B2 bad = !ok & vcell;
-  if (any(bad)) {  // rare
+  if (X2_UNLIKELY(any(bad))) {  // rare
 #pragma unroll
     for (int q = 0; q < NF; ++q) {
       ws[q] = sel(bad, w[q], ws[q]);
@@ -290,8 +290,8 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
     // Only the pending flux sum lives in registers across the phases; the face states a later phase needs
     // are staged in this thread's private shared-memory scratch (float4 j of thread tid at SCR[j*NI + tid]):
     //   0..4    W^+_z of the previous plane (left state of the next z face)
-    //   5..9    W^-_x pair (18 floats) + W^+_x of the even cell [0..1]; after the x solve: inner-face flux
-    //   10..14  W^-_y pair (18 floats) + W^+_x of the even cell [2..3]
+    //   5..9    W^-_x pair (18 floats) + W^+_x of the even cell [0..1]; after the x solve: the x flux pair
+    //   10..14  W^-_y pair (18 floats) + W^+_x of the even cell [2..3]; after the y solve: the y flux pair
     //   15..16  W^+_x of the even cell [4..8]
     float4* const sc = SCR + tid;
     auto st_block = [&](int j0, const F2* a, float e0, float e1) {  // 9 pairs + 2 floats -> 5 float4
@@ -372,7 +372,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
             riemann2<NF, RS>(WL, WR, RC, Fr, B2(true), s_cnt);
             rot_out<NF, 2>(Fr, fz);
           }
-          if (blk >= 0) {  // flux registers of a coarse-fine link (a7): z faces kk = 0..n
+          if (X2_UNLIKELY(blk >= 0)) {  // flux registers of a coarse-fine link (a7): z faces kk = 0..n
             float* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)kk * n2 + (size_t)((y0 + pj) * n + (x0 + 2 * pc)));
 #pragma unroll
             for (int q = 0; q < NF; ++q) { dstF[(size_t)q * fsz] += fz[q].v.x; dstF[(size_t)q * fsz + 1] += fz[q].v.y; }
@@ -399,7 +399,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
             float* out = P.Uout + (cell0 + (kk - 1) * n2);
 #pragma unroll
             for (int q = 0; q < NF; ++q) *reinterpret_cast<float2*>(out + q * fs_int) = un[q].v;
-            if (!(un[0].v.x > 0.f) || !(un[0].v.y > 0.f))
+            if (X2_UNLIKELY(!(un[0].v.x > 0.f) || !(un[0].v.y > 0.f)))
               atomicAdd(&s_cnt[X2_CNT_NEG_STATE], (int)!(un[0].v.x > 0.f) + (int)!(un[0].v.y > 0.f));
             const F2 sp = signal_speed<F2, NF>(un, F2(P.gamma), F2(P.gm1));
             smax_loc = fmaxf(smax_loc, fmaxf(sp.v.x, sp.v.y));
@@ -449,12 +449,12 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
             sts_n<NF, XVW>(xsol, o);
 #pragma unroll
             for (int q = NF; q < 9; ++q) fx[q] = F2(0.f);
-            // inner-face flux -> scratch 5..7 (W^-_x is consumed)
-            sc[5 * NI] = make_float4(fx[0].v.y, fx[1].v.y, fx[2].v.y, fx[3].v.y);
-            sc[6 * NI] = make_float4(fx[4].v.y, fx[5].v.y, fx[6].v.y, fx[7].v.y);
-            sc[7 * NI] = make_float4(fx[8].v.y, 0.f, 0.f, 0.f);
+            // private copy of both x fluxes -> scratch 5..9 (W^-_x is consumed).  Phase 3 must not read
+            // them back from xsol: the left neighbour overwrites that slot in ITS next phase 1, with no
+            // barrier in between
+            st_block(5, fx, 0.f, 0.f);
           }
-          if (blk >= 0) {  // record the fluxes for the reflux
+          if (X2_UNLIKELY(blk >= 0)) {  // record the fluxes for the reflux
             float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + (x0 + 2 * pc));
 #pragma unroll
             for (int q = 0; q < NF; ++q) { dstF[(size_t)q * fsz] += fx[q].v.x; dstF[(size_t)q * fsz + 1] += fx[q].v.y; }
@@ -468,7 +468,13 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
           riemann2<NF, RS>(WL, WR, RC, Fr, B2(true), s_cnt);
           rot_out<NF, 1>(Fr, fy);
           sts_pairs<NF>(ysol, fy);
-          if (blk >= 0) {
+          {
+            F2 o[9];
+#pragma unroll
+            for (int q = 0; q < 9; ++q) o[q] = q < NF ? fy[q] : F2(0.f);
+            st_block(10, o, 0.f, 0.f);  // private copy for phase 3 (same reason)
+          }
+          if (X2_UNLIKELY(blk >= 0)) {
             float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + (y0 + pj)) * n + (x0 + 2 * pc));
 #pragma unroll
             for (int q = 0; q < NF; ++q) { dstF[(size_t)q * fsz] += fy[q].v.x; dstF[(size_t)q * fsz + 1] += fy[q].v.y; }
@@ -479,24 +485,19 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
       __syncthreads();
 
       // ---- phase 3: x/y flux differences of plane kk -> registers ----------------------------------
-      // own fluxes are read back from where phase 2 left them (lo face: xsol, inner face: scratch, y: ysol);
-      // the right neighbour's lo-face flux and the upper pair's y fluxes come from the slots this very
-      // thread overwrites with its W^+ in the next phase 1, so no barrier is needed before that
+      // own fluxes are read back from the private scratch; the right neighbour's lo-face flux and the upper
+      // pair's y fluxes come from the slots this very thread overwrites with its W^+ in the next phase 1,
+      // so no barrier is needed before that
       if (mid) {
-        float xr[NF], fl[NF], fi[9];
-        F2 fu[NF], fy[NF];
+        float xr[NF], e0, e1;
+        F2 fu[NF], fx[9], fy[9];
         lds_n<NF, XVW>(xpub, xr);
-        lds_n<NF, XVW>(xsol, fl);
-        {
-          const float4 a = sc[5 * NI], b = sc[6 * NI];
-          fi[0] = a.x; fi[1] = a.y; fi[2] = a.z; fi[3] = a.w; fi[4] = b.x; fi[5] = b.y; fi[6] = b.z; fi[7] = b.w;
-          fi[8] = NF == 9 ? sc[7 * NI].x : 0.f;
-        }
         lds_pairs<NF>(ypub, fu);
-        lds_pairs<NF>(ysol, fy);
+        ld_block(5, fx, e0, e1);
+        ld_block(10, fy, e0, e1);
 #pragma unroll
         for (int q = 0; q < NF; ++q) {
-          const F2 dfx = F2(fi[q] - fl[q], xr[q] - fi[q]);
+          const F2 dfx = F2(fx[q].v.y - fx[q].v.x, xr[q] - fx[q].v.y);
           dU[q] = (dfx + (fu[q] - fy[q])) + dU[q];
         }
       }
@@ -688,7 +689,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
           for (int q = 0; q < NF; ++q) o[q] = wm[q].v.x;
           sts_n<NF, XVW>(xslot, o);
         }
-        if (blk >= 0 && x0 + TX == n) {  // the patch's last x face (a7)
+        if (X2_UNLIKELY(blk >= 0) && x0 + TX == n) {  // the patch's last x face (a7)
           float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + n);
 #pragma unroll
           for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += wm[q].v.x;
@@ -701,7 +702,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
         riemann2<NF, RS>(WL, WR, RC, Fr, B2(true), s_cnt);
         rot_out<NF, 1>(Fr, wm);
         sts_pairs<NF>(yslot, wm);
-        if (blk >= 0 && y0 + TY == n) {
+        if (X2_UNLIKELY(blk >= 0) && y0 + TY == n) {
           float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + n) * n + (x0 + 2 * (px - 1)));
 #pragma unroll
           for (int q = 0; q < NF; ++q) { dstF[(size_t)q * fsz] += wm[q].v.x; dstF[(size_t)q * fsz + 1] += wm[q].v.y; }

@@ -66,7 +66,7 @@ __device__ __forceinline__ void riemann_hydro2(const F2* WL, const F2* WR, const
     f3 = fma(cdr, wK, f3);
     f4 = fma(cK, Es - EK, f4);
   }
-  if (any(need_hll)) {  // HLL: the requested solver, or the fallback for p* <= 0 (A7)
+  if (RS == X2_RS_HLL ? any(need_hll) : X2_UNLIKELY(any(need_hll))) {  // HLL: the requested solver, or the fallback for p* <= 0 (A7)
     const F2 idS = rcp2(SR - SL), SLSR = SL * SR;
     const F2 mnL = rL * uL, mnR = rR * uR;
     const F2 h0 = hll_mix(mnL, mnR, rL, rR, SL, SR, SLSR, idS);
@@ -158,7 +158,7 @@ __device__ __forceinline__ void riemann_mhd2(const F2* WL, const F2* WR, const R
       b1s[K] = b1 * g;
       b2s[K] = b2 * g;
     }
-    if (any(degc)) {
+    if (X2_UNLIKELY(any(degc))) {
       const int c = (int)(degc.x && valid.x) + (int)(degc.y && valid.y);
       if (c) atomicAdd(&s_cnt[X2_CNT_DEGENERATE_D], c);
     }
@@ -201,7 +201,7 @@ __device__ __forceinline__ void riemann_mhd2(const F2* WL, const F2* WR, const R
     f6 = fma(cS, b1ss - b1sK, f6);
     f7 = fma(cS, b2ss - b2sK, f7);
   }
-  if (any(need_hll)) {  // HLL: the requested solver, or the fallback for pT* <= 0 (A7)
+  if (RS == X2_RS_HLL ? any(need_hll) : X2_UNLIKELY(any(need_hll))) {  // HLL: the requested solver, or the fallback for pT* <= 0 (A7)
     const F2 idS = rcp2(SR - SL), SLSR = SL * SR;
     const F2 mnL = rL * uL, mnR = rR * uR;
     const F2 h0 = hll_mix(mnL, mnR, rL, rR, SL, SR, SLSR, idS);
