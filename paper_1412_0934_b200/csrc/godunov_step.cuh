@@ -39,9 +39,11 @@ enum { RS_HLL = 0, RS_HLLC = 1, RS_HLLD = 2 };
 enum { CNT_POSITIVITY = 0, CNT_HLL_FALLBACK = 1, CNT_DEGENERATE_D = 2, CNT_NEG_STATE = 3 };
 
 __device__ __forceinline__ float rmin(float a, float b) { return fminf(a, b); }
-__device__ __forceinline__ double rmin(double a, double b) { return fmin(a, b); }
+// fp64: fmin / fmax expand to DSETP + six moves/selects each (NaN-propagation rules); a compare-select is three
+// instructions and equal for the finite operands the limiter and the solvers see (profiles/r1c)
+__device__ __forceinline__ double rmin(double a, double b) { return a < b ? a : b; }
 __device__ __forceinline__ float rmax(float a, float b) { return fmaxf(a, b); }
-__device__ __forceinline__ double rmax(double a, double b) { return fmax(a, b); }
+__device__ __forceinline__ double rmax(double a, double b) { return a > b ? a : b; }
 // three-input min / max: one FMNMX3 on sm_100a for fp32
 __device__ __forceinline__ float rmin3(float a, float b, float c) {
   float r;
@@ -53,8 +55,8 @@ __device__ __forceinline__ float rmax3(float a, float b, float c) {
   asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
   return r;
 }
-__device__ __forceinline__ double rmin3(double a, double b, double c) { return fmin(fmin(a, b), c); }
-__device__ __forceinline__ double rmax3(double a, double b, double c) { return fmax(fmax(a, b), c); }
+__device__ __forceinline__ double rmin3(double a, double b, double c) { return rmin(rmin(a, b), c); }
+__device__ __forceinline__ double rmax3(double a, double b, double c) { return rmax(rmax(a, b), c); }
 __device__ __forceinline__ float rsqrt_(float a) {
   float r;
   asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
@@ -683,7 +685,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_kernel(const __grid_constant__ St
 #pragma unroll
             for (int q = 0; q < NF; ++q) out[q * fs_int] = un[q];
             if (!(un[0] > T(0))) atomicAdd(&s_cnt[CNT_NEG_STATE], 1);
-            smax_loc = rmax(smax_loc, signal_speed<T, NF>(un, P.gamma, P.gm1));
+            smax_loc = rmax(signal_speed<T, NF>(un, P.gamma, P.gm1), smax_loc);  // a NaN speed is dropped
           }
 #pragma unroll
           for (int q = 0; q < NF; ++q) dU[q] = -fz[q];
@@ -755,7 +757,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_kernel(const __grid_constant__ St
   }
 
   // ---- epilogue: max signal speed of the new state (O7), event counters -----------------------
-  // NaN-safe: fmax drops NaNs; a NaN state shows up in the NEG_STATE counter instead.
+  // NaN-safe: rmax(x, m) keeps m when x is NaN; a NaN state shows up in the NEG_STATE counter instead.
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) smax_loc = rmax(smax_loc, __shfl_xor_sync(0xffffffffu, smax_loc, o));
   if ((tid & 31) == 0) s_red[tid >> 5] = smax_loc;

@@ -14,6 +14,12 @@
 #define AMR_TUNE_F32_NT 192
 #define AMR_TUNE_F32_MAXR 168
 #endif
+#ifndef AMR_TUNE_F64_TX
+#define AMR_TUNE_F64_TX 16
+#define AMR_TUNE_F64_TY 8
+#define AMR_TUNE_F64_NT 192
+#define AMR_TUNE_F64_MAXR 168
+#endif
 namespace amr {
 struct TileCfg_hydro_f32 { static constexpr int WTX = 32, WTY = 8, STX = 16, STY = 16, NT = 192, MAXR = 168; };
 struct TileCfg_mhd_f32 {
@@ -21,5 +27,5 @@ struct TileCfg_mhd_f32 {
                        MAXR = 168, WMAXR = AMR_TUNE_F32_MAXR;
 };
 struct TileCfg_hydro_f64 { static constexpr int TX = 16, TY = 16, NT = 320, MAXR = 168; };
-struct TileCfg_mhd_f64 { static constexpr int TX = 16, TY = 8, NT = 192, MAXR = 255; };
+struct TileCfg_mhd_f64 { static constexpr int TX = AMR_TUNE_F64_TX, TY = AMR_TUNE_F64_TY, NT = AMR_TUNE_F64_NT, MAXR = AMR_TUNE_F64_MAXR; };
 }  // namespace amr
