@@ -62,7 +62,8 @@ __device__ __forceinline__ float rsqrt_(float a) {
   asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
   return r;
 }
-__device__ __forceinline__ double rsqrt_(double a) { return sqrt(a); }
+__device__ __forceinline__ double rsqrt_(double a) { return fast_sqrt(a); }
+__device__ __forceinline__ double rrcp(double a) { return fast_rcp(a); }
 __device__ __forceinline__ float rabs(float a) { return fabsf(a); }
 __device__ __forceinline__ double rabs(double a) { return fabs(a); }
 __device__ __forceinline__ float rrcp(float a) {
@@ -70,14 +71,13 @@ __device__ __forceinline__ float rrcp(float a) {
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a));
   return r;
 }
-__device__ __forceinline__ double rrcp(double a) { return 1.0 / a; }
 // 1/sqrt(x) given x and sq = sqrt(x)
 __device__ __forceinline__ float rinvsqrt(float x, float) {
   float r;
   asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
   return r;
 }
-__device__ __forceinline__ double rinvsqrt(double, double sq) { return 1.0 / sq; }
+__device__ __forceinline__ double rinvsqrt(double, double sq) { return rrcp(sq); }
 template <class T> __device__ __forceinline__ T rinf();
 template <> __device__ __forceinline__ float rinf<float>() { return CUDART_INF_F; }
 template <> __device__ __forceinline__ double rinf<double>() { return CUDART_INF; }

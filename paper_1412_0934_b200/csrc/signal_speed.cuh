@@ -1,9 +1,9 @@
 // O7 (reading A9): max over directions of |v_d| + c_d for one cell, from its conserved state.
 // Used by the fused epilogue of the step kernels and by the standalone reduction (amr_cfl_dt); written
 // with explicitly rounded intrinsics (no FMA contraction) so that all kernels give bitwise the same
-// number for the same stored state (pin P15).  T = double: IEEE divide and square root.  T = float and
-// T = x2::F2 (two cells at once): the SFU reciprocal and square root (<= 2 ulp each, deterministic), like
-// the rest of the fp32 path; the packed *_rn operations round exactly like the scalar ones, so the F2
+// number for the same stored state (pin P15).  T = double: SFU seed + two Newton steps (fast_rcp,
+// fast_sqrt below, <= 2 ulp).  T = float and T = x2::F2 (two cells at once): the SFU reciprocal and
+// square root (<= 2 ulp each, deterministic), like the rest of the fp32 path; the packed *_rn operations round exactly like the scalar ones, so the F2
 // instantiation gives the float one's bits in each half.
 #pragma once
 #include <cuda_runtime.h>
@@ -12,14 +12,44 @@
 
 namespace amr {
 
+// fp64: MUFU seed (rcp / rsqrt.approx.ftz.f64, ~20 bits) + two Newton steps, <= 2 ulp, no slow-path
+// branch (the IEEE sequences cost ~3x the instructions and a divergent special-case check each; operands
+// here are normal-range positive numbers or differences of wave speeds).  rsqrt_(0) returns 0.
+__device__ __forceinline__ double fast_rcp(double a) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
+  double e = fma(-a, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-a, r, 1.0);
+  return fma(r, e, r);
+}
+// g ~ sqrt(a), 2 h ~ 1/sqrt(a) (coupled Newton iteration)
+__device__ __forceinline__ void sqrt_pair(double a, double& g, double& h) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+  g = a * y;
+  h = 0.5 * y;
+  double r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+  r = fma(-g, h, 0.5);
+  g = fma(g, r, g);
+  h = fma(h, r, h);
+}
+__device__ __forceinline__ double fast_sqrt(double a) {
+  double g, h;
+  sqrt_pair(a > 1e-300 ? a : 1e-300, g, h);
+  return a > 1e-300 ? g : 0.0;
+}
+
 __device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
 __device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
 __device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
 __device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
 __device__ __forceinline__ float div_rn(float a, float b) { return __fmul_rn(a, x2::rcpf(b)); }
-__device__ __forceinline__ double div_rn(double a, double b) { return __ddiv_rn(a, b); }
+__device__ __forceinline__ double div_rn(double a, double b) { return __dmul_rn(a, fast_rcp(b)); }
 __device__ __forceinline__ float sqrt_rn(float a) { return x2::sqrtf_(a); }
-__device__ __forceinline__ double sqrt_rn(double a) { return __dsqrt_rn(a); }
+__device__ __forceinline__ double sqrt_rn(double a) { return fast_sqrt(a); }
 __device__ __forceinline__ float max_(float a, float b) { return fmaxf(a, b); }
 __device__ __forceinline__ double max_(double a, double b) { return fmax(a, b); }
 __device__ __forceinline__ float abs_(float a) { return fabsf(a); }
