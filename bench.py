@@ -102,6 +102,22 @@ class ClockSampler:
                     reasons=sorted(reasons))
 
 
+def dram_traffic(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the step kernel on the full-size workload,
+    from the committed ncu capture (profiles/*_dram_traffic.csv, newest round last); None if no capture exists
+    for this workload (or the size was overridden)."""
+    if workload is None:
+        return None, None
+    import csv, glob
+    best = (None, None)
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_dram_traffic.csv"))):
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload:
+                    best = (int(row["dram_bytes_read"]) + int(row["dram_bytes_write"]), row["source"])
+    return best
+
+
 def build_workload(name: str, device, size: int | None):
     """Returns dict(U=host pinned torch tensor [nf,np,n,n,n], origin, n, dx, domain, mhd, dtype, gamma, limiter,
     riemann, cfl, alpha, label)."""
@@ -325,8 +341,11 @@ def main():
     pk = peaks()
     bpc = BYTES_PER_CELL[(kind, W["dtype"])]
     ach = bpc * ncells / (kern_avg * 1e-3) / 1e9
+    kname = "x2::godunov_step_x2_kernel" if (W["dtype"] == "f32" and W["n"] % 16 == 0) else "godunov_step_kernel"
+    traffic, traffic_src = dram_traffic(args.workload if args.size is None else None)
     roof = dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"],
-                traffic=None, peak_source=pk["source"], kernel="godunov_step_kernel", kernel_ms=kern_avg,
+                traffic=traffic, traffic_unit="bytes per launch (dram read + write, ncu --set full)",
+                traffic_source=traffic_src, peak_source=pk["source"], kernel=kname, kernel_ms=kern_avg,
                 bytes_per_cell=bpc, frac_of_nominal_8TBs=ach / 8000.0)
     lanes = 128 if W["dtype"] == "f32" else 64
     alu_peak = 148 * lanes * pk["sm_max_mhz"] * 1e6 * 2 / 1e12          # TFLOP/s, fma = 2
