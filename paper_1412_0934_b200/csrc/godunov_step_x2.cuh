@@ -10,23 +10,27 @@
 // one slot.  A thread owns the x-adjacent cells (2i, 2i+1) of one row and marches along z; every quantity
 // is an F2 (pair_math.cuh).  Riemann solvers are branch-free (riemann_x2.cuh).
 //
-// Work decomposition: one CTA owns a TX x TY column of one patch (TX = 16 or 32, the patch width when
-// n <= 32) and marches along z.  Threads: TX/2 * TY interior pairs, then the ring of the tile grown by one
-// layer (no corners): right / left x-ring pairs (cells (TX, TX+1) / (-2, -1), of which only the inner cell
-// is real) and top / bottom y-ring rows.  Shared memory (all "pair records": the NF components of a pair as
-// NF float2, padded to a bank-conflict-free stride, moved with 128-bit LDS/STS):
-//   ring   four planes of primitives on the tile + radius-2 halo; raw conserved pairs arrive by 8-byte
-//          cp.async (LDGSTS.64) and are converted in place by the thread that issued the copies
+// Work decomposition: one CTA owns a TX x TY column of one patch (TX = 32 when n % 32 == 0, else 16) and
+// marches along z.  Warp-specialised: TX/2 * TY interior pair threads (whole COMPUTE warps) and the AUX warps,
+// which hold the ring of the tile grown by one layer (no corners): right / left x-ring pairs (cells
+// (TX, TX+1) / (-2, -1), of which only the inner cell is real), bottom / top y-ring rows, and which do all
+// loading.  The two roles run separate loops with the same barrier sequence.  Shared memory (all "pair
+// records": the NF components of a pair as NF float2, padded to a bank-conflict-free stride, 128-bit LDS/STS):
+//   ring   three planes of primitives on the tile + radius-2 halo; the raw conserved pairs of plane k+2 arrive
+//          by 8-byte cp.async (LDGSTS.64) in the slot plane k-1 vacated and are converted in place by the aux
+//          thread that issued the copies
 //   XP     per x-face column: W^+_x of the odd cell left of a pair (scalar record), then that pair's lower
 //          x flux        YP   per y face: W^+_y of the pair below, then the y flux
 //   UO     (m, E) of the cell awaiting its update (conversion overwrites them in the ring)
-// Per plane, two barriers (same schedule as the scalar kernel):
-//   1  slopes, predictor, positivity; publish W^+_x (odd cell), W^+_y; the z faces (left state = this
-//      thread's W^+_z of the previous plane) are solved here and the previous plane is updated, stored
-//      and its signal speed reduced                                                       | barrier
-//   2  issue the copies of plane k+3; the two x faces (left of the even cell, between the cells) and the
-//      two y faces below the pair; convert plane k+2                                      | barrier
-//   3  flux differences of this plane -> registers; falls through into 1 of the next plane
+//   SCR    private staging of each compute thread (face states between phases, own fluxes), which keeps a
+//          thread that carries two MHD cells within 168 registers (two CTAs per SM)
+// Per plane, two barriers:
+//   1  compute: slopes, predictor, positivity; publish W^+_x (odd cell), W^+_y; stage W^-; the z faces (left
+//      state = staged W^+_z of the previous plane) are solved and the previous plane is updated, stored and
+//      its signal speed reduced.  aux: predictor of the ring pairs                          | barrier
+//   2  compute: the two x faces (left of the even cell, between the cells) and the two y faces below the
+//      pair.  aux: copies of plane k+2, the tile's last x / y faces, convert plane k+2      | barrier
+//   3  compute: flux differences of this plane -> registers; falls through into 1 of the next plane
 // Every face flux is computed once per tile by one position-independent routine from bit-identical
 // inputs, so a face shared by two tiles/patches gets the same bits on both sides (conservation to
 // round-off).
