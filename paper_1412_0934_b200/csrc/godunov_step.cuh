@@ -90,12 +90,28 @@ template <> __device__ __forceinline__ double rinf<double>() { return CUDART_INF
 template <class T, int LIM>
 __device__ __forceinline__ T half_slope(T a, T b) {
   if (LIM == LIM_NONE) return T(0);
-  if (LIM == LIM_MINMOD) {
-    const T ha = T(0.5) * a, hb = T(0.5) * b;
-    return rmax(rmin(ha, hb), rmin(rmax(ha, hb), T(0)));
+  if constexpr (sizeof(T) == 8) {
+    // fp64 has no min/max instruction (a compare-select is DSETP + 2 selects), so the sign-test definition
+    // itself is cheaper than the min/max form: smallest magnitude of the candidates, sign of a, zero unless
+    // a and b have the same sign (equal sign bits; if either is zero the smallest magnitude is zero anyway)
+    const bool same = (__double2hiint(a) ^ __double2hiint(b)) >= 0;
+    const double aa = fabs(a), ab = fabs(b);
+    double m = aa < ab ? aa : ab;
+    if (LIM == LIM_MC) {
+      const double aq = fabs(T(0.25) * (a + b));
+      m = m < aq ? m : aq;
+    } else {
+      m = T(0.5) * m;
+    }
+    return same ? copysign(m, a) : T(0);
+  } else {
+    if (LIM == LIM_MINMOD) {
+      const T ha = T(0.5) * a, hb = T(0.5) * b;
+      return rmax(rmin(ha, hb), rmin(rmax(ha, hb), T(0)));
+    }
+    const T q = T(0.25) * (a + b);
+    return rmax(rmin3(a, b, q), rmin(rmax3(a, b, q), T(0)));
   }
-  const T q = T(0.25) * (a + b);
-  return rmax(rmin3(a, b, q), rmin(rmax3(a, b, q), T(0)));
 }
 
 template <class T>
