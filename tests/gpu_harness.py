@@ -101,3 +101,30 @@ def per_step_parity(oracle, level, wl, nsteps, np_dtype, psi_floor=None):
         errs.append(rel_err(Unew, ref, psi_scale=ps))
         U = Unew
     return errs, U, b
+
+
+def sampled_patch_parity(oracle, U0, U1, origin, n, domain, dx, wl, dt, ch, sample_ids, np_dtype):
+    """Full-size parity on sampled outputs: for each sampled patch the oracle takes the same step on a
+    3x3x3-patch mini-level cut out of the GPU's input state U0 (the patch and its 26 periodic neighbours:
+    everything the radius-2 stencil of the centre patch can reach), with the GPU's dt and c_h, and its centre
+    patch is compared element by element with the GPU's output U1.  Returns the per-patch rel_err arrays."""
+    where = {tuple(int(v) for v in o): i for i, o in enumerate(np.asarray(origin))}
+    dom = np.asarray(domain)
+    mini_origin = np.array([[i * n, j * n, k * n] for k in range(3) for j in range(3) for i in range(3)], np.int32)
+    import workloads as wk
+    errs = []
+    for s in sample_ids:
+        o = np.asarray(origin[s])
+        ids = [where[tuple(int(v) for v in (o + (mo - n)) % dom)] for mo in mini_origin]
+        Um = np.ascontiguousarray(U0[:, ids]).astype(np.float64)
+        lev = wk.Level(n=n, g=3, level=0, dx=dx, origin=mini_origin, domain_cells=(3 * n,) * 3, bc=(0,) * 6,
+                       self_periodic=False, U=Um)
+        Ug = oracle.ghosted(Um, 3)
+        oracle.fill_ghosts(Ug, 3, lev.origin, lev.domain_cells, lev.bc, False)
+        r = oracle.step(Ug, 3, dt, dx, wl["gamma"], wl["limiter"], wl["riemann"], ch=ch, alpha=wl["alpha"],
+                        eps=oracle.default_eps(np_dtype))
+        ref = oracle.interior(r["U"], 3)[:, 13]
+        got = np.asarray(U1[:, s], dtype=np.float64)
+        ps = ch * np.abs(ref[5:8]).max() if ref.shape[0] == 9 else None
+        errs.append(rel_err(got[:, None], ref[:, None], psi_scale=ps))
+    return errs
