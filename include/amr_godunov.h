@@ -137,6 +137,35 @@ int amr_restrict(amr_level_link* l);
  * fine patch face, from the fluxes recorded since amr_flux_clear. */
 int amr_reflux(amr_level_link* l, double dt_coarse);
 
+/* ---- patch builder ------------------------------------------------------------
+ * The procedure the paper designed for the GPU (section 3, Figure 1): "AMR cells are
+ * ordered according to a space filling curve based layout; cells are grouped in compact (i.e. with no holes)
+ * cubic patches of maximum possible size; neighbouring patches are grouped in large chunks collecting all
+ * the data necessary".  Readings: Morton curve (bit b of x -> key bit 3b, y -> 3b+1,
+ * z -> 3b+2); a patch is an octree-aligned cube of side 2^k cells, k <= kmax, all of whose cells are present;
+ * every cell belongs to the largest such cube; patches are listed in curve order.
+ * The workspace is caller-allocated DEVICE memory (borrowed, 256-byte aligned), sized by amr_builder_bytes. */
+typedef struct amr_patch_builder amr_patch_builder;
+size_t amr_builder_bytes(int64_t ncell_max);                       /* 0 if ncell_max is outside [1, 2^30] */
+int amr_builder_create(int64_t ncell_max, void* dev_ws, size_t bytes, void* cuda_stream, amr_patch_builder** out);
+int amr_builder_destroy(amr_patch_builder* b);
+/* Steps 1 + 2.  dev_xyz: DEVICE int32 [3][ncell], the (x, y, z) of the unique leaf cells of one level, each in
+ * [0, 2^bits); bits 1..10; kmax 0..min(5, bits).  Synchronises the stream; *npatch_out = number of patches.
+ * AMR_EINVAL for bad arguments or duplicate cells. */
+int amr_builder_build(amr_patch_builder* b, const int32_t* dev_xyz, int64_t ncell, int32_t bits, int32_t kmax,
+                      int64_t* npatch_out);
+/* Results of the last build, HOST arrays, each may be NULL: perm [ncell] (perm[i] = input index of the i-th cell
+ * along the curve), first [npatch] (curve position of the patch's first cell; its 8^level cells follow in
+ * Morton order), level [npatch] (k: side 2^k), origin [npatch][3] (x, y, z of the lower corner). */
+int amr_builder_results(amr_patch_builder* b, int64_t* perm, int64_t* first, int32_t* level, int32_t* origin);
+/* Step 3 for the patches of side n = 2^k (curve order): dev_out[f][p][lz][ly][lx] = dev_fields[f][cell at
+ * origin_p + (lx, ly, lz)], i.e. the [nfields][npatch][n^3] layout amr_patch_batch_upload's device arena uses.
+ * dev_fields: DEVICE [nfields][ncell] in INPUT order; dev_out: DEVICE, room for max_patches patches;
+ * host_origin: HOST [count][3] or NULL; *count_out = number of such patches.  With dev_out == NULL and
+ * host_origin == NULL only the count is returned.  AMR_ENOMEM if count > max_patches. */
+int amr_builder_gather(amr_patch_builder* b, const void* dev_fields, int32_t nfields, int32_t dtype, int32_t k,
+                       void* dev_out, int64_t max_patches, int32_t* host_origin, int64_t* count_out);
+
 const char* amr_last_error(void);
 /* Library/build description, e.g. "amr_godunov sm_100a ..." (static string). */
 const char* amr_version(void);

@@ -24,7 +24,8 @@ EXPORTS = (
     "amr_patch_batch_download", "amr_patch_batch_state", "amr_fill_ghosts", "amr_cfl_dt", "amr_hydro_step",
     "amr_mhd_step", "amr_conserved_totals", "amr_step_counters", "amr_link_bytes", "amr_link_levels",
     "amr_link_destroy", "amr_prolong_ghosts", "amr_flux_clear", "amr_restrict", "amr_reflux", "amr_last_error",
-    "amr_version",
+    "amr_version", "amr_builder_bytes", "amr_builder_create", "amr_builder_destroy", "amr_builder_build",
+    "amr_builder_results", "amr_builder_gather",
 )
 
 
@@ -79,6 +80,14 @@ def lib():
         L.amr_flux_clear.argtypes = [C.c_void_p]
         L.amr_restrict.argtypes = [C.c_void_p]
         L.amr_reflux.argtypes = [C.c_void_p, C.c_double]
+        L.amr_builder_bytes.restype = C.c_size_t
+        L.amr_builder_bytes.argtypes = [C.c_int64]
+        L.amr_builder_create.argtypes = [C.c_int64, C.c_void_p, C.c_size_t, C.c_void_p, C.POINTER(C.c_void_p)]
+        L.amr_builder_destroy.argtypes = [C.c_void_p]
+        L.amr_builder_build.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.POINTER(C.c_int64)]
+        L.amr_builder_results.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.amr_builder_gather.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_int64,
+                                         C.c_void_p, C.POINTER(C.c_int64)]
         _lib = L
     return _lib
 
@@ -249,3 +258,67 @@ class LevelLink:
             self.close()
         except Exception:
             pass
+
+
+class PatchBuilder:
+    """amr_patch_builder: Morton curve order of the leaf cells of a level,
+    maximal compact aligned cubic patches, gather into the batch arena layout.  Marshalling only."""
+
+    def __init__(self, ncell_max: int, device: str = "cuda:0", stream: Optional[int] = None):
+        import torch  # device memory + stream only
+        L = lib()
+        nbytes = int(L.amr_builder_bytes(int(ncell_max)))
+        if nbytes == 0:
+            raise AmrError(-1, "amr_builder_bytes: ncell_max out of range")
+        self.device = torch.device(device)
+        with torch.cuda.device(self.device):
+            self.ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = int(torch.cuda.current_stream().cuda_stream) if stream is None else int(stream)
+            h = C.c_void_p()
+            _check(L.amr_builder_create(int(ncell_max), self.ws.data_ptr(), nbytes, self.stream, C.byref(h)))
+        self._h = h
+        self.ncell = 0
+        self.npatch = 0
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().amr_builder_destroy(self._h)
+            self._h = None
+
+    def build(self, xyz_dev, bits: int, kmax: int) -> int:
+        """xyz_dev: torch int32 CUDA tensor [3, ncell] (contiguous).  Returns the number of patches."""
+        assert xyz_dev.is_cuda and xyz_dev.is_contiguous() and xyz_dev.shape[0] == 3
+        np_out = C.c_int64(0)
+        _check(lib().amr_builder_build(self._h, xyz_dev.data_ptr(), int(xyz_dev.shape[1]), int(bits), int(kmax), C.byref(np_out)))
+        self.ncell, self.npatch = int(xyz_dev.shape[1]), int(np_out.value)
+        return self.npatch
+
+    def results(self, want_perm: bool = True):
+        """(perm [ncell] int64 or None, first [npatch] int64, level [npatch] int32, origin [npatch, 3] int32)."""
+        perm = np.empty(self.ncell, np.int64) if want_perm else None
+        first = np.empty(self.npatch, np.int64)
+        level = np.empty(self.npatch, np.int32)
+        origin = np.empty((self.npatch, 3), np.int32)
+        _check(lib().amr_builder_results(self._h, perm.ctypes.data if want_perm else None, first.ctypes.data,
+                                         level.ctypes.data, origin.ctypes.data))
+        return perm, first, level, origin
+
+    def count(self, k: int) -> int:
+        c = C.c_int64(0)
+        _check(lib().amr_builder_gather(self._h, None, 1, AMR_F32, int(k), None, 0, None, C.byref(c)))
+        return int(c.value)
+
+    def gather(self, fields_dev, k: int):
+        """fields_dev: torch CUDA tensor [nf, ncell] float32/float64 in input order.  Returns (out, origin): out a
+        torch CUDA tensor [nf, count, n, n, n] (n = 2^k), origin int32 [count, 3]."""
+        import torch
+        assert fields_dev.is_cuda and fields_dev.is_contiguous() and fields_dev.shape[1] == self.ncell
+        dtype = AMR_F64 if fields_dev.dtype == torch.float64 else AMR_F32
+        cnt = self.count(k)
+        n = 1 << k
+        out = torch.empty((fields_dev.shape[0], cnt, n, n, n), dtype=fields_dev.dtype, device=fields_dev.device)
+        origin = np.empty((cnt, 3), np.int32)
+        c = C.c_int64(0)
+        _check(lib().amr_builder_gather(self._h, fields_dev.data_ptr(), int(fields_dev.shape[0]), dtype, int(k),
+                                        out.data_ptr(), cnt, origin.ctypes.data, C.byref(c)))
+        return out, origin

@@ -11,6 +11,9 @@ constexpr int NBR_PATCH_MASK = 0x0FFFFFFF;  // nbr entry >= 0: low 28 bits = sou
 constexpr int NBR_MODE_SHIFT = 28;          // bits 28..30 = clamp flags (x,y,z) for outflow
 constexpr int NBR_FROM_HALO = -2;           // nbr entry: region comes from the prolongation halo buffer
 
+// sets the thread-local message amr_last_error() returns ("where: what") and returns code (batch.cu)
+int set_error(int code, const char* where, const char* what);
+
 // Everything the step kernel needs, passed by value.
 template <class T>
 struct StepParams {

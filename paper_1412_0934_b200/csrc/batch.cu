@@ -355,6 +355,10 @@ int do_step(amr_patch_batch* b, bool mhd, double dt, double gamma, int limiter, 
 
 }  // namespace
 
+namespace amr {
+int set_error(int code, const char* where, const char* what) { return fail(code, "%s: %s", where, what); }
+}  // namespace amr
+
 extern "C" {
 
 const char* amr_last_error(void) { return g_err.c_str(); }

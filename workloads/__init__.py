@@ -29,4 +29,5 @@ from .configs import (  # noqa: F401
     uniform_grid_workload,
     morton_permutation,
     turbulence_patches_torch,
+    refined_level_cells,
 )

@@ -475,3 +475,29 @@ def turbulence_patches_torch(N: int, n: int, device, mach: float = 3.0, beta: fl
         out[q] = t.index_select(0, perm)
     origin = morton_patch_origins(npd, npd, npd, n)
     return out, origin
+
+
+def refined_level_cells(bits: int = 8, frac: float = 0.25, nfields: int = 9, dtype=np.float32, stream: int = 0):
+    """Input of the patch builder: the leaf cells of one refined level as a
+    fully threaded tree would hand them over -- scattered in memory, in no spatial order.  Level index space
+    (2^bits)^3.  Octs (2^3 cells, what an AMR tree refines) are flagged where a lognormal density with
+    P(k) ~ k^-4 (the recipe of A21 with a steeper index: smooth blobs, as collapsed structures are) exceeds its
+    (1 - frac) quantile, so about `frac` of the volume is refined in blobs: compact cubes of every size in
+    the interiors, single octs along the rims.
+    Returns (xyz int32 [3, ncell] in a seeded scrambled order, fields [nfields, ncell] = seeded normals).
+    DATA ONLY: no curve ordering, no grouping happens here."""
+    rng = _rng(6, stream)
+    N = 1 << bits
+    Nc = N // 2
+    G = gaussian_random_field(Nc, -4.0, rng)
+    thr = np.quantile(G, 1.0 - frac)
+    oz, oy, ox = np.nonzero(G > thr)          # arrays are indexed [z, y, x]
+    d = np.arange(2)
+    cx = (2 * ox[:, None, None, None] + d[None, None, None, :]).repeat(2, axis=1).repeat(2, axis=2)
+    cy = (2 * oy[:, None, None, None] + d[None, None, :, None]).repeat(2, axis=1).repeat(2, axis=3)
+    cz = (2 * oz[:, None, None, None] + d[None, :, None, None]).repeat(2, axis=2).repeat(2, axis=3)
+    xyz = np.stack([cx.ravel(), cy.ravel(), cz.ravel()]).astype(np.int32)
+    order = rng.permutation(xyz.shape[1])
+    xyz = np.ascontiguousarray(xyz[:, order])
+    fields = rng.standard_normal((nfields, xyz.shape[1])).astype(dtype)
+    return xyz, fields
