@@ -226,6 +226,79 @@ def run_reference(args):
     print(json.dumps(out))
 
 
+def run_builder(args):
+    """--workload patch_builder: the next row of the scope table.  A step =
+    amr_builder_build (Morton order + maximal compact cubic patches) + amr_builder_gather of every patch size,
+    on the seeded refined-level workload (256^3 index space, ~25 % refined, 9 fp32 fields).  Same JSON contract;
+    the metric counts cells built per second."""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    import paper_1412_0934_b200 as amr
+    bits, kmax = args.size or 8, 5
+    xyz, F = wk.refined_level_cells(bits)
+    ncell, nf = xyz.shape[1], F.shape[0]
+    hx = torch.from_numpy(xyz).pin_memory(); hf = torch.from_numpy(F).pin_memory()
+    x, f = hx.cuda(), hf.cuda()
+    b = amr.PatchBuilder(ncell)
+
+    def step(xd, fd):
+        b.build(xd, bits, kmax)
+        return [b.gather(fd, k)[0] for k in range(kmax + 1)]
+
+    K, Wm = args.steps, max(args.warmup, 3)
+    for _ in range(Wm):
+        outs = step(x, f)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start(); time.sleep(0.25)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K):
+        outs = step(x, f)
+    e1.record(); torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1) / K
+    gathered = sum(int(o.shape[1]) * int(o.shape[2]) ** 3 for o in outs)
+    assert gathered == ncell, "every cell belongs to exactly one patch"
+    # end to end: cell list and fields from pinned host memory, patch arrays back to the host
+    s2, t2 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s2.record()
+    for _ in range(3):
+        outs = step(hx.cuda(non_blocking=True), hf.cuda(non_blocking=True))
+        host = [o.cpu() for o in outs]
+    t2.record(); torch.cuda.synchronize()
+    ms2 = s2.elapsed_time(t2) / 3
+    pk = peaks()
+    bpc = 12 + 4 + 2 * nf * F.itemsize      # xyz in, curve order out, every field value read once and written once
+    ach = bpc * ncell / (ms * 1e-3) / 1e9
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import patch_builder as pbo
+        sx, sf = wk.refined_level_cells(bits - 1)
+        t0 = time.perf_counter()
+        perm, keys = pbo.curve_order(sx, bits - 1)
+        first, level = pbo.build_patches(keys, kmax)
+        for k in range(kmax + 1):
+            pbo.gather_level(sf, perm, keys, first, level, k, bits - 1)
+        dt = time.perf_counter() - t0
+        cpu = dict(value=sx.shape[1] / dt, unit="cells/s", cores=1, kind="oracle",
+                   sample="the same recipe at %d^3 (%d cells), build + gather of every level, %.1f s" % (1 << (bits - 1), sx.shape[1], dt))
+    out = dict(metric="cells_built_per_sec", value=ncell / (ms * 1e-3), unit="cells/s", n_gpus=1, steps=K, warmup=Wm,
+               ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="u32", data="synthetic",
+               config=dict(workload="patch_builder (f2): leaf cells of a refined level in a %d^3 index space, %d cells, %d fp32 fields, kmax=%d"
+                           % (1 << bits, ncell, nf, kmax), step="amr_builder_build + amr_builder_gather for k = 0..%d" % kmax,
+                           l2="working set %.0f MB; buffers alternate between sort passes" % (ncell * (16 + 2 * nf * 4) / 1e6)),
+               roofline=dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"], traffic=None,
+                             peak_source=pk["source"], kernel="sort passes + level + compaction + gather (whole step)",
+                             kernel_ms=ms, bytes_per_cell=bpc),
+               cpu_baseline=cpu,
+               e2e=dict(value=ncell / (ms2 * 1e-3), unit="cells/s", h2d_bytes_per_step=int(xyz.nbytes + F.nbytes),
+                        d2h_bytes_per_step=int(F.nbytes), ms_per_step=ms2, steps=3),
+               gpu_launches=K * (1 + 3 * ((3 * bits + 7) // 8) + 5 + 5 * (kmax + 1)), clocks=clocks, npatch=int(b.npatch))
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -239,6 +312,10 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
+    if args.workload == "patch_builder":
+        if args.impl == "reference":
+            raise SystemExit("the reference arm times the hot path (config 2, 3, 5); the patch builder's oracle is timed in cpu_baseline")
+        return run_builder(args)
     if args.impl == "reference":
         return run_reference(args)
 

@@ -51,9 +51,22 @@ __global__ void key_kernel(const int* __restrict__ xyz, unsigned n, unsigned* __
   vals[i] = i;
 }
 
+// lanes of the warp whose 8-bit digit equals this lane's (invalid lanes match each other): nine ballots; on
+// sm_100a this is several times faster than __match_any_sync, which goes through the MIO queue (profiles/r1d)
+__device__ __forceinline__ unsigned same_digit_mask(unsigned d, bool ok) {
+  const unsigned okm = __ballot_sync(0xffffffffu, ok);
+  unsigned m = ok ? okm : ~okm;
+#pragma unroll
+  for (int b = 0; b < 8; ++b) {
+    const unsigned bal = __ballot_sync(0xffffffffu, (d >> b) & 1u);
+    m &= ((d >> b) & 1u) ? bal : ~bal;
+  }
+  return m;
+}
+
 // step 1b, one 8-bit LSD pass.  A block owns SORT_ITEMS consecutive items; warp w owns the w-th run of
 // 32 * SORT_GROUPS of them and walks it group by group, so (warp, group, lane) order is input order and the
-// pass is stable.  Per group: lanes with equal digits find each other with match_any; the rank of a lane
+// pass is stable.  Per group: lanes with equal digits find each other (same_digit_mask); the rank of a lane
 // among them is the popcount of the lower lanes of its mask.
 __device__ __forceinline__ void warp_digit_counts(const unsigned* __restrict__ keys, unsigned n, unsigned base, int shift,
                                                    unsigned* wh /* [256] of this warp, zeroed */) {
@@ -61,8 +74,8 @@ __device__ __forceinline__ void warp_digit_counts(const unsigned* __restrict__ k
   for (int g = 0; g < SORT_GROUPS; ++g) {
     const unsigned i = base + g * 32 + lane;
     const bool ok = i < n;
-    const unsigned d = ok ? (keys[i] >> shift) & 255u : 256u;
-    const unsigned m = __match_any_sync(0xffffffffu, d);
+    const unsigned d = ok ? (keys[i] >> shift) & 255u : 0u;
+    const unsigned m = same_digit_mask(d, ok);
     if (ok && lane == __ffs(m) - 1) wh[d] += __popc(m);
     __syncwarp();
   }
@@ -101,19 +114,53 @@ __global__ void __launch_bounds__(1024) scan_kernel(unsigned* __restrict__ a, un
   for (unsigned i = lo; i < hi; ++i) { const unsigned v = a[i]; a[i] = run; run += v; }
 }
 
+// the sort's histogram scan in two levels: block d scans row d of hist [256][nb] in place (exclusive) and
+// leaves the row total; the scatter kernel adds the exclusive scan of the 256 totals itself
+__global__ void __launch_bounds__(256) scan_rows_kernel(unsigned* __restrict__ hist, unsigned nb, unsigned* __restrict__ totals) {
+  __shared__ unsigned part[256];
+  unsigned* row = hist + (size_t)blockIdx.x * nb;
+  const unsigned chunk = (nb + 255) / 256;
+  const unsigned lo = min(nb, threadIdx.x * chunk), hi = min(nb, lo + chunk);
+  unsigned s = 0;
+  for (unsigned i = lo; i < hi; ++i) s += row[i];
+  part[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = 1; o < 256; o <<= 1) {
+    const unsigned v = threadIdx.x >= o ? part[threadIdx.x - o] : 0;
+    __syncthreads();
+    part[threadIdx.x] += v;
+    __syncthreads();
+  }
+  unsigned run = part[threadIdx.x] - s;
+  for (unsigned i = lo; i < hi; ++i) { const unsigned v = row[i]; row[i] = run; run += v; }
+  if (threadIdx.x == 255) totals[blockIdx.x] = part[255];
+}
+
 __global__ void __launch_bounds__(SORT_THREADS) scatter_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict__ vals,
                                                                unsigned n, int shift, unsigned nb,
-                                                               const unsigned* __restrict__ offs /* scanned [256][nb] */,
+                                                               const unsigned* __restrict__ offs /* row-scanned [256][nb] */,
+                                                               const unsigned* __restrict__ totals /* [256] row totals */,
                                                                unsigned* __restrict__ keys_out, unsigned* __restrict__ vals_out) {
   __shared__ unsigned wh[SORT_THREADS / 32][256];
+  __shared__ unsigned dbase[256];
   const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
   for (int d = threadIdx.x; d < (SORT_THREADS / 32) * 256; d += SORT_THREADS) (&wh[0][0])[d] = 0;
   __syncthreads();
   const unsigned base = blockIdx.x * SORT_ITEMS + w * 32 * SORT_GROUPS;
   warp_digit_counts(keys, n, base, shift, wh[w]);
   __syncthreads();
-  {  // counts -> first output position of (warp, digit): global offset of the block + the earlier warps
-    unsigned run = offs[(size_t)threadIdx.x * nb + blockIdx.x];
+  {  // exclusive scan of the digit totals (thread d = digit d)
+    const unsigned tot = totals[threadIdx.x];
+    dbase[threadIdx.x] = tot;
+    __syncthreads();
+    for (int o = 1; o < 256; o <<= 1) {
+      const unsigned v = threadIdx.x >= o ? dbase[threadIdx.x - o] : 0;
+      __syncthreads();
+      dbase[threadIdx.x] += v;
+      __syncthreads();
+    }
+    // counts -> first output position of (warp, digit): digit base + blocks before this one + earlier warps
+    unsigned run = (dbase[threadIdx.x] - tot) + offs[(size_t)threadIdx.x * nb + blockIdx.x];
 #pragma unroll
     for (int v = 0; v < SORT_THREADS / 32; ++v) { const unsigned c = wh[v][threadIdx.x]; wh[v][threadIdx.x] = run; run += c; }
   }
@@ -122,8 +169,8 @@ __global__ void __launch_bounds__(SORT_THREADS) scatter_kernel(const unsigned* _
     const unsigned i = base + g * 32 + lane;
     const bool ok = i < n;
     const unsigned k = ok ? keys[i] : 0u;
-    const unsigned d = ok ? (k >> shift) & 255u : 256u;
-    const unsigned m = __match_any_sync(0xffffffffu, d);
+    const unsigned d = (k >> shift) & 255u;
+    const unsigned m = same_digit_mask(d, ok);
     unsigned pos = 0;
     if (ok) pos = wh[w][d] + __popc(m & ((1u << lane) - 1));
     __syncwarp();
@@ -243,6 +290,7 @@ struct amr_patch_builder {
   int* porigin = nullptr;          // [cap][3] origins of all patches
   int* sorigin = nullptr;          // [cap][3] origins of the patches of the level last gathered
   unsigned* dup = nullptr;
+  unsigned* totals = nullptr;      // [256] digit totals of a sort pass
   int cur = 0;                // which keys/vals buffer holds the sorted result
   int64_t ncell = 0, npatch = 0;
   int bits = 0, kmax = 0;
@@ -251,7 +299,7 @@ struct amr_patch_builder {
 
 namespace {
 
-struct BLayout { size_t keys[2], vals[2], hist, lev, counts, pfirst, plev, slot_first, porigin, sorigin, dup, total; };
+struct BLayout { size_t keys[2], vals[2], hist, lev, counts, pfirst, plev, slot_first, porigin, sorigin, dup, totals, total; };
 
 BLayout builder_layout(int64_t cap) {
   BLayout L;
@@ -267,6 +315,7 @@ BLayout builder_layout(int64_t cap) {
   L.porigin = off; off += up(n * 12);
   L.sorigin = off; off += up(n * 12);
   L.dup = off; off += up(16);
+  L.totals = off; off += up(256 * 4);
   L.total = off;
   return L;
 }
@@ -325,6 +374,7 @@ int amr_builder_create(int64_t ncell_max, void* dev_ws, size_t bytes, void* cuda
   b->porigin = (int*)(w + L.porigin);
   b->sorigin = (int*)(w + L.sorigin);
   b->dup = (unsigned*)(w + L.dup);
+  b->totals = (unsigned*)(w + L.totals);
   *out = b;
   return AMR_OK;
 }
@@ -346,8 +396,8 @@ int amr_builder_build(amr_patch_builder* b, const int32_t* dev_xyz, int64_t ncel
   int cur = 0;
   for (int shift = 0; shift < 3 * bits; shift += 8) {   // LSD radix sort, 8 bits per pass
     hist_kernel<<<nb, SORT_THREADS, 0, b->stream>>>(b->keys[cur], n, shift, nb, b->hist);
-    scan_kernel<<<1, 1024, 0, b->stream>>>(b->hist, 256u * nb);
-    scatter_kernel<<<nb, SORT_THREADS, 0, b->stream>>>(b->keys[cur], b->vals[cur], n, shift, nb, b->hist, b->keys[1 - cur], b->vals[1 - cur]);
+    scan_rows_kernel<<<256, 256, 0, b->stream>>>(b->hist, nb, b->totals);
+    scatter_kernel<<<nb, SORT_THREADS, 0, b->stream>>>(b->keys[cur], b->vals[cur], n, shift, nb, b->hist, b->totals, b->keys[1 - cur], b->vals[1 - cur]);
     cur = 1 - cur;
   }
   B_TRY(cudaGetLastError());
