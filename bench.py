@@ -244,7 +244,9 @@ def run_builder(args):
 
     def step(xd, fd):
         b.build(xd, bits, kmax)
-        return [b.gather(fd, k)[0] for k in range(kmax + 1)]
+        outs = [b.gather(fd, k, want_origin=False)[0] for k in range(kmax + 1)]
+        b.results(want_perm=False)          # patch table (first cell, level, origin) on the host
+        return outs
 
     K, Wm = args.steps, max(args.warmup, 3)
     for _ in range(Wm):
@@ -295,7 +297,7 @@ def run_builder(args):
                cpu_baseline=cpu,
                e2e=dict(value=ncell / (ms2 * 1e-3), unit="cells/s", h2d_bytes_per_step=int(xyz.nbytes + F.nbytes),
                         d2h_bytes_per_step=int(F.nbytes), ms_per_step=ms2, steps=3),
-               gpu_launches=K * (1 + 3 * ((3 * bits + 7) // 8) + 5 + 5 * (kmax + 1)), clocks=clocks, npatch=int(b.npatch))
+               gpu_launches=K * (1 + 3 * ((3 * bits + 7) // 8) + 6 + 3 * (kmax + 1) + 2 + (kmax + 1)), clocks=clocks, npatch=int(b.npatch))
     print(json.dumps(out))
 
 

@@ -162,7 +162,9 @@ int amr_builder_results(amr_patch_builder* b, int64_t* perm, int64_t* first, int
  * origin_p + (lx, ly, lz)], i.e. the [nfields][npatch][n^3] layout amr_patch_batch_upload's device arena uses.
  * dev_fields: DEVICE [nfields][ncell] in INPUT order; dev_out: DEVICE, room for max_patches patches;
  * host_origin: HOST [count][3] or NULL; *count_out = number of such patches.  With dev_out == NULL and
- * host_origin == NULL only the count is returned.  AMR_ENOMEM if count > max_patches. */
+ * host_origin == NULL only the count is returned.  With host_origin == NULL the gather is only enqueued on
+ * the builder's stream (no synchronisation); with host_origin it synchronises.  AMR_ENOMEM if count >
+ * max_patches. */
 int amr_builder_gather(amr_patch_builder* b, const void* dev_fields, int32_t nfields, int32_t dtype, int32_t k,
                        void* dev_out, int64_t max_patches, int32_t* host_origin, int64_t* count_out);
 

@@ -308,17 +308,18 @@ class PatchBuilder:
         _check(lib().amr_builder_gather(self._h, None, 1, AMR_F32, int(k), None, 0, None, C.byref(c)))
         return int(c.value)
 
-    def gather(self, fields_dev, k: int):
+    def gather(self, fields_dev, k: int, want_origin: bool = True):
         """fields_dev: torch CUDA tensor [nf, ncell] float32/float64 in input order.  Returns (out, origin): out a
-        torch CUDA tensor [nf, count, n, n, n] (n = 2^k), origin int32 [count, 3]."""
+        torch CUDA tensor [nf, count, n, n, n] (n = 2^k), origin int32 [count, 3] (None and no synchronisation
+        with want_origin=False)."""
         import torch
         assert fields_dev.is_cuda and fields_dev.is_contiguous() and fields_dev.shape[1] == self.ncell
         dtype = AMR_F64 if fields_dev.dtype == torch.float64 else AMR_F32
         cnt = self.count(k)
         n = 1 << k
         out = torch.empty((fields_dev.shape[0], cnt, n, n, n), dtype=fields_dev.dtype, device=fields_dev.device)
-        origin = np.empty((cnt, 3), np.int32)
+        origin = np.empty((cnt, 3), np.int32) if want_origin else None
         c = C.c_int64(0)
         _check(lib().amr_builder_gather(self._h, fields_dev.data_ptr(), int(fields_dev.shape[0]), dtype, int(k),
-                                        out.data_ptr(), cnt, origin.ctypes.data, C.byref(c)))
+                                        out.data_ptr(), cnt, origin.ctypes.data if want_origin else None, C.byref(c)))
         return out, origin

@@ -225,10 +225,11 @@ __global__ void __launch_bounds__(256) count_kernel(const unsigned char* __restr
 template <int MODE>
 __global__ void __launch_bounds__(256) write_kernel(const unsigned char* __restrict__ lev, const unsigned* __restrict__ src_first,
                                                     unsigned n, int k, const unsigned* __restrict__ offs,
+                                                    const unsigned* __restrict__ base /* device scalar or null */,
                                                     unsigned* __restrict__ out_first, unsigned char* __restrict__ out_lev) {
   __shared__ unsigned s_w[8];
   __shared__ unsigned s_run;
-  if (threadIdx.x == 0) s_run = offs[blockIdx.x];
+  if (threadIdx.x == 0) s_run = offs[blockIdx.x] + (base ? *base : 0u);
   __syncthreads();
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   for (unsigned i0 = blockIdx.x * CMP_ITEMS; i0 < min(n, (blockIdx.x + 1u) * CMP_ITEMS); i0 += 256) {
@@ -265,6 +266,15 @@ __global__ void gather_kernel(const T* __restrict__ in, size_t ncell, int nf, co
   for (int f = 0; f < nf; ++f) out[((size_t)f * nslot + s) * n3 + c] = in[(size_t)f * ncell + src];
 }
 
+// lbase[k] = number of patches of the levels below k (the per-level totals sit behind each level's counts)
+__global__ void bases_kernel(const unsigned* __restrict__ counts, unsigned stride, unsigned ncb, int nlev, unsigned* __restrict__ lbase) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    unsigned run = 0;
+    for (int k = 0; k < nlev; ++k) { lbase[k] = run; run += counts[(size_t)k * stride + ncb]; }
+    lbase[nlev] = run;
+  }
+}
+
 __global__ void origin_kernel(const unsigned* __restrict__ keys, const unsigned* __restrict__ first, unsigned np, int* __restrict__ origin) {
   const unsigned p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= np) return;
@@ -286,7 +296,9 @@ struct amr_patch_builder {
   unsigned* counts = nullptr;      // compaction block counts
   unsigned* pfirst = nullptr;      // [cap] first cell (curve position) of each patch
   unsigned char* plev = nullptr;   // [cap]
-  unsigned* slot_first = nullptr;  // [cap] patches of one level
+  unsigned* slot_first = nullptr;  // [cap] first cell of every patch, grouped by level (curve order inside a level)
+  unsigned* lbase = nullptr;       // [8] device copy of lbase_host
+  unsigned lbase_host[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // patches of level k: slots [lbase[k], lbase[k+1])
   int* porigin = nullptr;          // [cap][3] origins of all patches
   int* sorigin = nullptr;          // [cap][3] origins of the patches of the level last gathered
   unsigned* dup = nullptr;
@@ -299,7 +311,7 @@ struct amr_patch_builder {
 
 namespace {
 
-struct BLayout { size_t keys[2], vals[2], hist, lev, counts, pfirst, plev, slot_first, porigin, sorigin, dup, totals, total; };
+struct BLayout { size_t keys[2], vals[2], hist, lev, counts, pfirst, plev, slot_first, porigin, sorigin, dup, totals, lbase, total; };
 
 BLayout builder_layout(int64_t cap) {
   BLayout L;
@@ -308,7 +320,7 @@ BLayout builder_layout(int64_t cap) {
   for (int b = 0; b < 2; ++b) { L.keys[b] = off; off += up(n * 4); L.vals[b] = off; off += up(n * 4); }
   L.hist = off; off += up(256 * nb * 4);
   L.lev = off; off += up(n);
-  L.counts = off; off += up((ncb + 1) * 4);
+  L.counts = off; off += up(7 * (ncb + 1) * 4);   // heads + one row per level
   L.pfirst = off; off += up(n * 4);
   L.plev = off; off += up(n);
   L.slot_first = off; off += up(n * 4);
@@ -316,6 +328,7 @@ BLayout builder_layout(int64_t cap) {
   L.sorigin = off; off += up(n * 12);
   L.dup = off; off += up(16);
   L.totals = off; off += up(256 * 4);
+  L.lbase = off; off += up(8 * 4);
   L.total = off;
   return L;
 }
@@ -334,7 +347,7 @@ int compact(amr_patch_builder* b, const unsigned char* flags, const unsigned* sr
   count_kernel<MODE><<<ncb, 256, 0, b->stream>>>(flags, n, k, b->counts);
   B_TRY(cudaMemsetAsync(b->counts + ncb, 0, 4, b->stream));
   scan_kernel<<<1, 1024, 0, b->stream>>>(b->counts, ncb + 1);     // counts[ncb] becomes the total
-  write_kernel<MODE><<<ncb, 256, 0, b->stream>>>(flags, src_first, n, k, b->counts, out_first, out_lev);
+  write_kernel<MODE><<<ncb, 256, 0, b->stream>>>(flags, src_first, n, k, b->counts, nullptr, out_first, out_lev);
   B_TRY(cudaGetLastError());
   B_TRY(cudaMemcpyAsync(total, b->counts + ncb, 4, cudaMemcpyDeviceToHost, b->stream));
   B_TRY(cudaStreamSynchronize(b->stream));
@@ -375,6 +388,7 @@ int amr_builder_create(int64_t ncell_max, void* dev_ws, size_t bytes, void* cuda
   b->sorigin = (int*)(w + L.sorigin);
   b->dup = (unsigned*)(w + L.dup);
   b->totals = (unsigned*)(w + L.totals);
+  b->lbase = (unsigned*)(w + L.lbase);
   *out = b;
   return AMR_OK;
 }
@@ -409,6 +423,20 @@ int amr_builder_build(amr_patch_builder* b, const int32_t* dev_xyz, int64_t ncel
   if (rc != AMR_OK) return rc;
   B_TRY(cudaMemcpyAsync(&dup, b->dup, 4, cudaMemcpyDeviceToHost, b->stream));
   origin_kernel<<<(np + 255) / 256, 256, 0, b->stream>>>(b->keys[cur], b->pfirst, np, b->porigin);
+  {  // group the patch table by level for the gather (ordered compaction per level, no host round trip)
+    const unsigned ncbp = (np + CMP_ITEMS - 1) / CMP_ITEMS, stride = ncbp + 1;
+    unsigned* cl = b->counts + ((size_t)n + CMP_ITEMS - 1) / CMP_ITEMS + 1;   // rows 1..6 behind the heads' row
+    B_TRY(cudaMemsetAsync(cl, 0, (size_t)(kmax + 1) * stride * 4, b->stream));
+    for (int k = 0; k <= kmax; ++k) {
+      count_kernel<1><<<ncbp, 256, 0, b->stream>>>(b->plev, np, k, cl + (size_t)k * stride);
+      scan_kernel<<<1, 1024, 0, b->stream>>>(cl + (size_t)k * stride, stride);
+    }
+    bases_kernel<<<1, 32, 0, b->stream>>>(cl, stride, ncbp, kmax + 1, b->lbase);
+    for (int k = 0; k <= kmax; ++k)
+      write_kernel<1><<<ncbp, 256, 0, b->stream>>>(b->plev, b->pfirst, np, k, cl + (size_t)k * stride, b->lbase + k, b->slot_first, nullptr);
+    origin_kernel<<<(np + 255) / 256, 256, 0, b->stream>>>(b->keys[cur], b->slot_first, np, b->sorigin);
+    B_TRY(cudaMemcpyAsync(b->lbase_host, b->lbase, (size_t)(kmax + 2) * 4, cudaMemcpyDeviceToHost, b->stream));
+  }
   B_TRY(cudaGetLastError());
   B_TRY(cudaStreamSynchronize(b->stream));
   if (dup) return amr::set_error(AMR_EINVAL, "amr_builder_build", "duplicate cells in the input");
@@ -455,9 +483,8 @@ int amr_builder_gather(amr_patch_builder* b, const void* dev_fields, int32_t nfi
   if (!b->built) return amr::set_error(AMR_ESTATE, "amr_builder_gather", "no successful amr_builder_build yet");
   if (k < 0 || k > b->kmax) return amr::set_error(AMR_EINVAL, "amr_builder_gather", "k outside 0..kmax of the build");
   if (nfields < 1 || (dtype != AMR_F32 && dtype != AMR_F64)) return amr::set_error(AMR_EINVAL, "amr_builder_gather", "bad nfields or dtype");
-  unsigned ns = 0;
-  int rc = compact<1>(b, b->plev, b->pfirst, (unsigned)b->npatch, k, b->slot_first, nullptr, &ns);
-  if (rc != AMR_OK) return rc;
+  const unsigned ns = b->lbase_host[k + 1] - b->lbase_host[k];
+  const unsigned* slots = b->slot_first + b->lbase_host[k];
   *count_out = ns;
   if ((!dev_out && !host_origin) || ns == 0) return AMR_OK;  // count query, or nothing to gather
   if (!dev_fields || !dev_out) return amr::set_error(AMR_EINVAL, "amr_builder_gather", "null field pointers");
@@ -465,15 +492,12 @@ int amr_builder_gather(amr_patch_builder* b, const void* dev_fields, int32_t nfi
   const size_t total = (size_t)ns << (3 * k);
   const unsigned grid = (unsigned)((total + 255) / 256);
   if (dtype == AMR_F32)
-    gather_kernel<float><<<grid, 256, 0, b->stream>>>((const float*)dev_fields, (size_t)b->ncell, nfields, b->vals[b->cur], b->slot_first, ns, k, (float*)dev_out);
+    gather_kernel<float><<<grid, 256, 0, b->stream>>>((const float*)dev_fields, (size_t)b->ncell, nfields, b->vals[b->cur], slots, ns, k, (float*)dev_out);
   else
-    gather_kernel<double><<<grid, 256, 0, b->stream>>>((const double*)dev_fields, (size_t)b->ncell, nfields, b->vals[b->cur], b->slot_first, ns, k, (double*)dev_out);
+    gather_kernel<double><<<grid, 256, 0, b->stream>>>((const double*)dev_fields, (size_t)b->ncell, nfields, b->vals[b->cur], slots, ns, k, (double*)dev_out);
   B_TRY(cudaGetLastError());
-  if (host_origin) {
-    origin_kernel<<<(ns + 255) / 256, 256, 0, b->stream>>>(b->keys[b->cur], b->slot_first, ns, b->sorigin);
-    B_TRY(cudaGetLastError());
-    B_TRY(cudaMemcpyAsync(host_origin, b->sorigin, (size_t)ns * 12, cudaMemcpyDeviceToHost, b->stream));
-  }
+  if (!host_origin) return AMR_OK;                           // enqueued; the caller's stream orders later work
+  B_TRY(cudaMemcpyAsync(host_origin, b->sorigin + 3 * (size_t)b->lbase_host[k], (size_t)ns * 12, cudaMemcpyDeviceToHost, b->stream));
   B_TRY(cudaStreamSynchronize(b->stream));
   return AMR_OK;
 }
