@@ -132,6 +132,20 @@ def build_workload(name: str, device, size: int | None):
         return dict(U=host, origin=origin, n=32, dx=1.0 / N, domain=(N, N, N), mhd=True, dtype="f32", gamma=5.0 / 3.0,
                     limiter=wk.configs.LIM_MC, riemann=wk.configs.RS_HLLD, cfl=0.3, alpha=0.4,
                     label="config5: %d^3 cells, %d patches of 32^3 (+3 ghost in the API), MHD fp32, MC+HLLD+GLM" % (N, origin.shape[0]))
+    if name in ("hydro_f32", "hydro_f64"):
+        # not a BASELINE config: the config-5 field without B (rho = p = 1, Mach-3 turbulence), 32^3 patches, for the
+        # hydro rows of the four-variant table in DESIGN.md section 7 (MC + HLLC)
+        N = size or (512 if name.endswith("f32") else 256)
+        U, origin = wk.turbulence_patches_torch(N, 32, device)
+        U[4] -= 0.5 * (U[5] ** 2 + U[6] ** 2 + U[7] ** 2)
+        dt = torch.float32 if name.endswith("f32") else torch.float64
+        host = torch.empty((5,) + tuple(U.shape[1:]), dtype=dt, pin_memory=True)
+        host.copy_(U[:5])
+        del U
+        torch.cuda.empty_cache()
+        return dict(U=host, origin=origin, n=32, dx=1.0 / N, domain=(N, N, N), mhd=False, dtype=name[-3:], gamma=5.0 / 3.0,
+                    limiter=wk.configs.LIM_MC, riemann=wk.configs.RS_HLLC, cfl=0.3, alpha=0.0,
+                    label="hydro: %d^3 cells, %d patches of 32^3, Mach-3 turbulence (config-5 recipe without B), hydro %s, MC+HLLC" % (N, origin.shape[0], name[-3:]))
     if name in ("config3_f32", "config3_f64"):
         N = size or 256
         w = wk.config3_orszag_tang(N=N)

@@ -131,7 +131,8 @@ struct GeomX2 {
   static constexpr int XVW = NF == 9 ? 4 : 2;
   static constexpr int SLOT = RH * NPX * REC;       // floats per ring plane
   static constexpr int NSLOT = 3;                   // planes k-1, k, k+1; plane k+2 lands in the slot k-1 vacates
-  static constexpr int NSCR = 17;                   // float4 of private staging per interior pair thread
+  static constexpr int BLK = NF == 9 ? 5 : 3;       // float4 per staging block: NF pairs + 2 floats
+  static constexpr int NSCR = 3 * BLK + (NF == 9 ? 2 : 1);   // float4 of private staging per interior pair thread
   static constexpr int NI = HX * TY;                // interior pair threads
   static constexpr int NPRED = NI + 2 * TY + 2 * HX;
   static constexpr int NXP = TY * (HX + 1);
@@ -293,24 +294,26 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
 
     // Only the pending flux sum lives in registers across the phases; the face states a later phase needs
     // are staged in this thread's private shared-memory scratch (float4 j of thread tid at SCR[j*NI + tid]):
-    //   0..4    W^+_z of the previous plane (left state of the next z face)
-    //   5..9    W^-_x pair (18 floats) + W^+_x of the even cell [0..1]; after the x solve: the x flux pair
-    //   10..14  W^-_y pair (18 floats) + W^+_x of the even cell [2..3]; after the y solve: the y flux pair
-    //   15..16  W^+_x of the even cell [4..8]
+    // (blocks of BLK float4 = NF pairs + 2 floats: 5 for MHD, 3 for hydro)
+    //   BZ      W^+_z of the previous plane (left state of the next z face)
+    //   BX      W^-_x pair + W^+_x of the even cell [0..1]; after the x solve: the x flux pair
+    //   BY      W^-_y pair + W^+_x of the even cell [2..3]; after the y solve: the y flux pair
+    //   BE      W^+_x of the even cell [4..NF-1]
     float4* const sc = SCR + tid;
-    auto st_block = [&](int j0, const F2* a, float e0, float e1) {  // 9 pairs + 2 floats -> 5 float4
+    constexpr int BLK = G::BLK, BZ = 0, BX = BLK, BY = 2 * BLK, BE = 3 * BLK, NFULL = (NF - 1) / 2;
+    auto st_block = [&](int j0, const F2* a, float e0, float e1) {  // NF pairs + 2 floats -> BLK float4
 #pragma unroll
-      for (int i = 0; i < 4; ++i) sc[(j0 + i) * NI] = make_float4(a[2 * i].v.x, a[2 * i].v.y, a[2 * i + 1].v.x, a[2 * i + 1].v.y);
-      sc[(j0 + 4) * NI] = make_float4(a[8].v.x, a[8].v.y, e0, e1);
+      for (int i = 0; i < NFULL; ++i) sc[(j0 + i) * NI] = make_float4(a[2 * i].v.x, a[2 * i].v.y, a[2 * i + 1].v.x, a[2 * i + 1].v.y);
+      sc[(j0 + NFULL) * NI] = make_float4(a[NF - 1].v.x, a[NF - 1].v.y, e0, e1);
     };
     auto ld_block = [&](int j0, F2* a, float& e0, float& e1) {
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
+      for (int i = 0; i < NFULL; ++i) {
         const float4 v = sc[(j0 + i) * NI];
         a[2 * i] = F2(v.x, v.y); a[2 * i + 1] = F2(v.z, v.w);
       }
-      const float4 v = sc[(j0 + 4) * NI];
-      a[8] = F2(v.x, v.y); e0 = v.z; e1 = v.w;
+      const float4 v = sc[(j0 + NFULL) * NI];
+      a[NF - 1] = F2(v.x, v.y); e0 = v.z; e1 = v.w;
     };
     static_assert(NF == 9 || NF == 5, "staging blocks are laid out for 9 fields (hydro uses the first 5)");
     F2 dU[NF];    // flux sum of the plane whose update is pending: ((Fx+ - Fx-) + (Fy+ - Fy-)) - Fz-
@@ -347,24 +350,24 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
             for (int q = NF; q < 9; ++q) { o[q] = F2(0.f); wpxl[q] = 0.f; ws[q] = F2(0.f); }
 #pragma unroll
             for (int q = 0; q < NF; ++q) o[q] = ws[q] - hx[q];
-            st_block(5, o, wpxl[0], wpxl[1]);
+            st_block(BX, o, wpxl[0], wpxl[1]);
 #pragma unroll
             for (int q = 0; q < NF; ++q) o[q] = ws[q] - hy[q];
-            st_block(10, o, wpxl[2], wpxl[3]);
-            sc[15 * NI] = make_float4(wpxl[4], wpxl[5], wpxl[6], wpxl[7]);
-            sc[16 * NI] = make_float4(wpxl[8], 0.f, 0.f, 0.f);
+            st_block(BY, o, wpxl[2], wpxl[3]);
+            sc[BE * NI] = make_float4(wpxl[4], wpxl[5], wpxl[6], wpxl[7]);
+            if (NF == 9) sc[(BE + 1) * NI] = make_float4(wpxl[8], 0.f, 0.f, 0.f);
           }
           // z direction: left state of the face below = W^+_z of the previous plane (scratch), then this
           // plane's W^+_z takes its place
           float e0, e1;
           F2 zl[9];
-          ld_block(0, zl, e0, e1);
+          ld_block(BZ, zl, e0, e1);
           rot_in<NF, 2>(zl, WL);
 #pragma unroll
           for (int q = 0; q < NF; ++q) zl[q] = ws[q] + hz[q];
 #pragma unroll
           for (int q = NF; q < 9; ++q) zl[q] = F2(0.f);
-          st_block(0, zl, 0.f, 0.f);
+          st_block(BZ, zl, 0.f, 0.f);
 #pragma unroll
           for (int q = 0; q < NF; ++q) zl[q] = ws[q] - hz[q];
           rot_in<NF, 2>(zl, WR);
@@ -429,13 +432,14 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
         float wpxl[9];
         F2 wmy[9];
         {
-          const float4 v15 = sc[15 * NI], v16 = sc[16 * NI];
-          wpxl[4] = v15.x; wpxl[5] = v15.y; wpxl[6] = v15.z; wpxl[7] = v15.w; wpxl[8] = v16.x;
+          const float4 v15 = sc[BE * NI];
+          wpxl[4] = v15.x; wpxl[5] = v15.y; wpxl[6] = v15.z; wpxl[7] = v15.w;
+          wpxl[8] = NF == 9 ? sc[(BE + 1) * NI].x : 0.f;
         }
         {
           F2 wl[9], wmx[9], WL[9], WR[9], Fr[NF], fx[9];
-          ld_block(5, wmx, wpxl[0], wpxl[1]);
-          ld_block(10, wmy, wpxl[2], wpxl[3]);
+          ld_block(BX, wmx, wpxl[0], wpxl[1]);
+          ld_block(BY, wmy, wpxl[2], wpxl[3]);
           {
             float xl[NF];
             lds_n<NF, XVW>(xsol, xl);
@@ -456,7 +460,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
             // private copy of both x fluxes -> scratch 5..9 (W^-_x is consumed).  Phase 3 must not read
             // them back from xsol: the left neighbour overwrites that slot in ITS next phase 1, with no
             // barrier in between
-            st_block(5, fx, 0.f, 0.f);
+            st_block(BX, fx, 0.f, 0.f);
           }
           if (X2_UNLIKELY(blk >= 0)) {  // record the fluxes for the reflux
             float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + (x0 + 2 * pc));
@@ -476,7 +480,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
             F2 o[9];
 #pragma unroll
             for (int q = 0; q < 9; ++q) o[q] = q < NF ? fy[q] : F2(0.f);
-            st_block(10, o, 0.f, 0.f);  // private copy for phase 3 (same reason)
+            st_block(BY, o, 0.f, 0.f);  // private copy for phase 3 (same reason)
           }
           if (X2_UNLIKELY(blk >= 0)) {
             float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + (y0 + pj)) * n + (x0 + 2 * pc));
@@ -497,8 +501,8 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
         F2 fu[NF], fx[9], fy[9];
         lds_n<NF, XVW>(xpub, xr);
         lds_pairs<NF>(ypub, fu);
-        ld_block(5, fx, e0, e1);
-        ld_block(10, fy, e0, e1);
+        ld_block(BX, fx, e0, e1);
+        ld_block(BY, fy, e0, e1);
 #pragma unroll
         for (int q = 0; q < NF; ++q) {
           const F2 dfx = F2(fx[q].v.y - fx[q].v.x, xr[q] - fx[q].v.y);

@@ -21,7 +21,10 @@
 #define AMR_TUNE_F64_MAXR 168
 #endif
 namespace amr {
-struct TileCfg_hydro_f32 { static constexpr int WTX = 32, WTY = 8, STX = 16, STY = 16, NT = 192, MAXR = 168; };
+#ifndef AMR_TUNE_HYDRO_F32_MAXR
+#define AMR_TUNE_HYDRO_F32_MAXR 96   /* 3 CTAs per SM: 18 warps, 5 on one scheduler -> at most 102 registers */
+#endif
+struct TileCfg_hydro_f32 { static constexpr int WTX = 32, WTY = 8, STX = 16, STY = 16, NT = 192, MAXR = AMR_TUNE_HYDRO_F32_MAXR; };
 struct TileCfg_mhd_f32 {
   static constexpr int WTX = AMR_TUNE_F32_WTX, WTY = AMR_TUNE_F32_WTY, STX = 16, STY = 16, NT = 192, WNT = AMR_TUNE_F32_NT,
                        MAXR = 168, WMAXR = AMR_TUNE_F32_MAXR;
