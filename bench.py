@@ -118,6 +118,22 @@ def dram_traffic(workload):
     return best
 
 
+def reduce_max_over_ranks(values, dist, device):
+    """Replicas only: the one exchange of a multi-rank run.  Every timing of the job is the
+    slowest rank's: element-wise MAX over ranks of a short list of floats (identity when dist is None)."""
+    if dist is None:
+        return [float(v) for v in values]
+    import torch
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def job_value(world: int, cells_per_rank: int, ms_per_step: float) -> float:
+    """Whole-job throughput: the units all ranks processed divided by the slowest rank's time."""
+    return world * cells_per_rank / (ms_per_step * 1e-3)
+
+
 def build_workload(name: str, device, size: int | None):
     """Returns dict(U=host pinned torch tensor [nf,np,n,n,n], origin, n, dx, domain, mhd, dtype, gamma, limiter,
     riemann, cfl, alpha, label)."""
@@ -386,14 +402,9 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     total_ms = start.elapsed_time(end)
     kern_ms = [a.elapsed_time(c) for a, c in zip(ev0, ev1)]
-    if dist is not None:
-        t = torch.tensor([total_ms, sum(kern_ms) / K], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, kern_avg = float(t[0]), float(t[1])
-    else:
-        kern_avg = sum(kern_ms) / K
+    total_ms, kern_avg = reduce_max_over_ranks([total_ms, sum(kern_ms) / K], dist, device)
     ms_per_step = total_ms / K
-    value = world * ncells / (ms_per_step * 1e-3)
+    value = job_value(world, ncells, ms_per_step)
 
     # sanity of the evolved state (validity of the run, not parity: parity is tests/ -m gpu)
     counters = b.step_counters()
@@ -417,13 +428,9 @@ def main():
             b.download(out=out_host)
         e2.record()
         torch.cuda.synchronize()
-        ms2 = s2.elapsed_time(e2) / ke
-        if dist is not None:
-            t = torch.tensor([ms2], device=device, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms2 = float(t[0])
+        ms2 = reduce_max_over_ranks([s2.elapsed_time(e2) / ke], dist, device)[0]
         nbytes = W["U"].numel() * W["U"].element_size()
-        e2e = dict(value=world * ncells / (ms2 * 1e-3), unit=UNIT, h2d_bytes_per_step=int(nbytes),
+        e2e = dict(value=job_value(world, ncells, ms2), unit=UNIT, h2d_bytes_per_step=int(nbytes),
                    d2h_bytes_per_step=int(nbytes + 8), ms_per_step=ms2, steps=ke)
 
     if rank != 0:
