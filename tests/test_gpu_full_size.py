@@ -84,3 +84,27 @@ def test_config3_full_size_sampled(oracle, H, np_dtype):
     absn = np.abs(U0.astype(np.float64)).sum(axis=(1, 2, 3, 4))
     grp = np.array([absn[0], absn[1:4].max(), absn[1:4].max(), absn[1:4].max(), absn[4], absn[5:8].max(), absn[5:8].max(), absn[5:8].max()])
     assert (np.abs(tot - tot0)[:8] / grp).max() <= (1e-13 if np_dtype == np.float64 else 1e-6)
+
+
+@pytest.mark.parametrize("mhd", [False, True])
+def test_config4_full_size_fp32(oracle, H, mhd):
+    """Config 4 as stated: 128^3 root = 512 patches of 16^3 + level-1 patches on the flagged blocks (A15), fp32,
+    one coarse step with two fine substeps (O9), element by element against the fp64 oracle started from the
+    fp32-rounded data (fp32 degeneracy thresholds), composite conservation to fp32 round-off."""
+    wl = wk.config4_two_level(mhd)
+    lc, lf = wl.levels
+    assert lc.npatch == 512 and 80 <= lf.npatch <= 125          # "about 20 % extra cells"
+    lc.U = lc.U.astype(np.float32).astype(np.float64)
+    lf.U = lf.U.astype(np.float32).astype(np.float64)
+    ref = oracle.two_level_step(wl, eps=oracle.default_eps(np.float32))
+    got = H.gpu_two_level_step(wl, np_dtype=np.float32)
+    assert abs(got["dt0"] - ref["dt0"]) <= 4e-6 * ref["dt0"]
+    ps = ref["smax"] * max(np.abs(ref["Uc"][5:8]).max(), 1e-300) if mhd else None
+    ec = H.rel_err(got["Uc"], ref["Uc"], psi_scale=ps)
+    ef = H.rel_err(got["Uf"], ref["Uf"], psi_scale=ps)
+    assert ec.max() <= 2e-5 and ef.max() <= 2e-5, (ec, ef)      # two fine substeps + restriction + reflux: 2 x 1e-5
+    tot = oracle.composite_totals(oracle.ghosted(got["Uc"].astype(np.float64), lc.g), lc,
+                                  oracle.ghosted(got["Uf"].astype(np.float64), lf.g), lf)
+    nfc = 8 if mhd else 5
+    absn = np.array([np.abs(lc.U[f]).sum() * lc.dx ** 3 for f in range(lc.nfields)])
+    assert (np.abs(tot - ref["totals_before"])[:nfc] / absn[:nfc]).max() <= 2e-6
