@@ -5,7 +5,9 @@
 //   fp32: two cells per thread (godunov_step_x2.cuh): TX/2*TY interior pair threads (whole warps) plus the
 //         aux warps (ring pairs + loader), NT >= TX/2*TY + 2*TY + TX; W = tile for n % 32 == 0, S = tile for
 //         the other multiples of 16; test-size patches (n = 8) run the scalar 8x8 tile
-//   fp64: one cell per thread (godunov_step.cuh), NT >= TX*TY + 2*TX + 2*TY
+//   fp64: one cell per thread with the x2 kernel's structure (godunov_step_d1.cuh): HX*TY compute threads (whole
+//         warps) plus the aux warps, NT >= HX*TY + 2*TY + 2*HX; n = 8 (and other non-multiples of 16) run the first
+//         fp64 kernel (godunov_step.cuh) on 8x8 tiles
 // The AMR_TUNE_* macros exist for tuning sweeps only (one -D per value); the defaults are the product.
 #pragma once
 #ifndef AMR_TUNE_F32_WTX
@@ -13,12 +15,6 @@
 #define AMR_TUNE_F32_WTY 8
 #define AMR_TUNE_F32_NT 192
 #define AMR_TUNE_F32_MAXR 168
-#endif
-#ifndef AMR_TUNE_F64_TX
-#define AMR_TUNE_F64_TX 16
-#define AMR_TUNE_F64_TY 8
-#define AMR_TUNE_F64_NT 192
-#define AMR_TUNE_F64_MAXR 168
 #endif
 namespace amr {
 #ifndef AMR_TUNE_HYDRO_F32_MAXR
@@ -29,6 +25,6 @@ struct TileCfg_mhd_f32 {
   static constexpr int WTX = AMR_TUNE_F32_WTX, WTY = AMR_TUNE_F32_WTY, STX = 16, STY = 16, NT = 192, WNT = AMR_TUNE_F32_NT,
                        MAXR = 168, WMAXR = AMR_TUNE_F32_MAXR;
 };
-struct TileCfg_hydro_f64 { static constexpr int TX = 16, TY = 16, NT = 320, MAXR = 168; };
-struct TileCfg_mhd_f64 { static constexpr int TX = AMR_TUNE_F64_TX, TY = AMR_TUNE_F64_TY, NT = AMR_TUNE_F64_NT, MAXR = AMR_TUNE_F64_MAXR; };
+struct TileCfg_hydro_f64 { static constexpr int HX = 16, TY = 8, NT = 192, MAXR = 168; };
+struct TileCfg_mhd_f64 { static constexpr int HX = 16, TY = 8, NT = 192, MAXR = 168; };
 }  // namespace amr

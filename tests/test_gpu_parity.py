@@ -152,8 +152,6 @@ def test_every_limiter_and_solver_fp64(oracle, H, nf, limiter, rs_exact, n):
         assert gc["positivity_fallback_cells"] == rc["positivity_fallback_cells"]
         assert gc["nonpositive_rho_after"] == rc["nonpositive_rho_after"]
         assert rc["hll_fallback_faces"] <= gc["hll_fallback_faces"] <= 1.05 * rc["hll_fallback_faces"] + 4
-        if nf == 5:  # hydro fp64 runs one 16x16 tile per 16^3 patch
-            assert gc == rc
 
 
 @pytest.mark.parametrize("nf", [5, 9])
