@@ -274,15 +274,21 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
 #pragma unroll
             for (int q = 0; q < NF; ++q) o[q] = ws[q] + hx[q];
             sts_rec<NF>(xpub, o);
+            // everything the y solve reads or writes travels in its rotated component order (y, z, x), so that
+            // phase 2 runs ONE solver instance over both directions (the kernel is bound by instruction fetch:
+            // profiles/r1f)
+            double r[NF];
 #pragma unroll
             for (int q = 0; q < NF; ++q) o[q] = ws[q] + hy[q];
-            sts_rec<NF>(ypub, o);
+            rot_in<NF, 1>(o, r);
+            sts_rec<NF>(ypub, r);
 #pragma unroll
             for (int q = 0; q < NF; ++q) o[q] = ws[q] - hx[q];
             st_block(BX, o);
 #pragma unroll
             for (int q = 0; q < NF; ++q) o[q] = ws[q] - hy[q];
-            st_block(BY, o);
+            rot_in<NF, 1>(o, r);
+            st_block(BY, r);
           }
           // z direction: left state of the face below = W^+_z of the previous plane (scratch), then this
           // plane's W^+_z takes its place
@@ -350,34 +356,27 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
       }
       cp_commit();
       if (mid) {
-        {
+        // d = 0: the x face left of this cell; d = 1: the y face below it.  One solver instance; inputs and
+        // outputs in the solver's component order (identity for x, rotated for y).
+#pragma unroll 1
+        for (int d = P.ntz - 1; d < 2; ++d) {   // ntz == 1: an opaque lower bound keeps the loop from being unrolled
+          double* const rec = d ? ysol : xsol;
+          const int bj = d ? BY : BX;
           double WL[NF], WR[NF], Fr[NF];
-          lds_rec<NF>(xsol, WL);      // rotation for x is the identity
-          ld_block(BX, WR);
+          lds_rec<NF>(rec, WL);
+          ld_block(bj, WR);
           x2::riemann2<NF, RS>(WL, WR, RC, Fr, true, s_cnt);
-          sts_rec<NF>(xsol, Fr);      // for the left neighbour's phase 3
-          st_block(BX, Fr);           // private copy for this thread's phase 3 (the left neighbour overwrites xsol
-                                      // in ITS next phase 1, with no barrier in between)
+          sts_rec<NF>(rec, Fr);       // for the left / lower neighbour's phase 3
+          st_block(bj, Fr);           // private copy for this thread's phase 3 (the neighbour overwrites rec in ITS
+                                      // next phase 1, with no barrier in between)
           if (X2_UNLIKELY(blk >= 0)) {  // record the flux for the reflux
-            double* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + (x0 + pc));
+            double f[NF];
+            if (d) rot_out<NF, 1>(Fr, f); else rot_out<NF, 0>(Fr, f);
+            double* dstF = P.fblk + ((size_t)blk * 3 + d) * NF * fsz +
+                           (d ? ((size_t)(kk * (n + 1) + (y0 + pj)) * n + (x0 + pc))
+                              : ((size_t)(kk * n + (y0 + pj)) * (n + 1) + (x0 + pc)));
 #pragma unroll
-            for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += Fr[q];
-          }
-        }
-        {
-          double wl[NF], wr[NF], WL[NF], WR[NF], Fr[NF], fy[NF];
-          lds_rec<NF>(ysol, wl);
-          ld_block(BY, wr);
-          rot_in<NF, 1>(wl, WL);
-          rot_in<NF, 1>(wr, WR);
-          x2::riemann2<NF, RS>(WL, WR, RC, Fr, true, s_cnt);
-          rot_out<NF, 1>(Fr, fy);
-          sts_rec<NF>(ysol, fy);
-          st_block(BY, fy);
-          if (X2_UNLIKELY(blk >= 0)) {
-            double* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + (y0 + pj)) * n + (x0 + pc));
-#pragma unroll
-            for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += fy[q];
+            for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += f[q];
           }
         }
       }
@@ -393,7 +392,10 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
         ld_block(BX, fx);
         ld_block(BY, fy);
 #pragma unroll
-        for (int q = 0; q < NF; ++q) dU[q] = ((xr[q] - fx[q]) + (fu[q] - fy[q])) + dU[q];
+        for (int q = 0; q < NF; ++q) fu[q] = fu[q] - fy[q];   // (rotated order)
+        rot_out<NF, 1>(fu, fy);
+#pragma unroll
+        for (int q = 0; q < NF; ++q) dU[q] = ((xr[q] - fx[q]) + fy[q]) + dU[q];
       }
       double* tmp = Wm; Wm = Wc; Wc = Wp; Wp = tmp;
     }
@@ -536,15 +538,18 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
           for (int q = 0; q < NF; ++q) o[q] = ws[q] + hx[q];
           sts_rec<NF>(xslot, o);
         } else if (bottom) {
+          double r[NF];
 #pragma unroll
           for (int q = 0; q < NF; ++q) o[q] = ws[q] + hy[q];
-          sts_rec<NF>(yslot, o);
+          rot_in<NF, 1>(o, r);
+          sts_rec<NF>(yslot, r);
         } else if (right) {
 #pragma unroll
           for (int q = 0; q < NF; ++q) wm[q] = ws[q] - hx[q];
         } else {
 #pragma unroll
-          for (int q = 0; q < NF; ++q) wm[q] = ws[q] - hy[q];
+          for (int q = 0; q < NF; ++q) o[q] = ws[q] - hy[q];
+          rot_in<NF, 1>(o, wm);
         }
       }
       __syncthreads();
@@ -553,28 +558,24 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
       //      convert plane kk+2 when it has landed (these warps have the slack to wait for it) ----------
       issue_plane(kk + 2, Wm);
       cp_commit();
-      if (mid && right) {
+      if (mid && (right || top)) {   // one solver instance: the tile's last x faces (right column) / y faces (top row)
+        double* const rec = right ? xslot : yslot;
         double WL[NF], Fr[NF];
-        lds_rec<NF>(xslot, WL);
+        lds_rec<NF>(rec, WL);
         x2::riemann2<NF, RS>(WL, wm, RC, Fr, true, s_cnt);
-        sts_rec<NF>(xslot, Fr);
-        if (X2_UNLIKELY(blk >= 0) && x0 + HX == n) {  // the patch's last x face (a7)
-          double* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + n);
+        sts_rec<NF>(rec, Fr);
+        if (X2_UNLIKELY(blk >= 0)) {   // the patch's last x / y face (a7)
+          if (right && x0 + HX == n) {
+            double* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + n);
 #pragma unroll
-          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += Fr[q];
-        }
-      } else if (mid && top) {
-        double wl[NF], WL[NF], WR[NF], Fr[NF], fy[NF];
-        lds_rec<NF>(yslot, wl);
-        rot_in<NF, 1>(wl, WL);
-        rot_in<NF, 1>(wm, WR);
-        x2::riemann2<NF, RS>(WL, WR, RC, Fr, true, s_cnt);
-        rot_out<NF, 1>(Fr, fy);
-        sts_rec<NF>(yslot, fy);
-        if (X2_UNLIKELY(blk >= 0) && y0 + TY == n) {
-          double* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + n) * n + (x0 + cx - 2));
+            for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += Fr[q];
+          } else if (top && y0 + TY == n) {
+            double fy[NF];
+            rot_out<NF, 1>(Fr, fy);
+            double* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + n) * n + (x0 + cx - 2));
 #pragma unroll
-          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += fy[q];
+            for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += fy[q];
+          }
         }
       }
       cp_wait<0>();
