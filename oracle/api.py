@@ -231,3 +231,69 @@ def two_level_step(wl, dtype=np.float64, eps: Optional[float] = None, do_reflux:
     tot1 = composite_totals(Ucnew, lc, Uf, lf)
     return dict(Uc=interior(Ucnew, g), Uf=interior(Uf, g), dt0=dt0, smax=sm, totals_before=tot0,
                 totals_after=tot1, counters=counters)
+
+
+def level_totals(U, level) -> np.ndarray:
+    """sum over the interiors of one level of U dx^3, per field (fp64)."""
+    return totals(U, level.g) * level.dx ** 3
+
+
+def hierarchy_totals(Us, levels) -> np.ndarray:
+    """Composite totals of an L-level hierarchy: every level's cells that no finer level covers.
+    composite_totals(c, f) = uncovered(c) + all(f), so the sum telescopes."""
+    tot = composite_totals(Us[0], levels[0], Us[1], levels[1])
+    for l in range(1, len(levels) - 1):
+        tot = tot - level_totals(Us[l], levels[l]) + composite_totals(Us[l], levels[l], Us[l + 1], levels[l + 1])
+    return tot
+
+
+def hierarchy_step(wl, dtype=np.float64, eps: Optional[float] = None, do_reflux: bool = True):
+    """one root step of an L-level hierarchy with recursive subcycling (PAPER.md:31
+    "the different resolution levels are advanced in time with different time-steps", :59 "once a refinement
+    level is completed the solution is corrected ... and the next (coarser) level of refinement is processed").
+    O9 applied recursively: advance(l, dt) = step level l by dt; then, if a finer level exists, twice
+    { sibling ghosts of l+1, prolong its coarse-fine ghosts from level l's old/new states at theta = 0, 1/2
+    (O8), advance(l+1, dt/2) }; restrict l+1 -> l; reflux l with its own fluxes against the time-summed fine
+    fluxes.  One dt0 = cfl dx0 / max_l smax_l and one c_h = that maximum for the whole root step; dt_l =
+    dt0 / 2^l.  For L = 2 this is two_level_step call for call.  Returns final interiors per level, dt0, smax,
+    composite totals before/after, counters in execution order."""
+    levels = wl.levels
+    L = len(levels)
+    g = levels[0].g
+    U = [ghosted(lv.U, g, dtype) for lv in levels]
+    tot0 = hierarchy_totals(U, levels)
+    sm = max(smax(U[l], g, wl.gamma) for l in range(L))
+    dt0 = wl.cfl * levels[0].dx / sm
+    Uold = [None] * L
+    counters = []
+    nsteps = [0] * L
+
+    def sibling_ghosts(l):
+        lv = levels[l]
+        return fill_ghosts(U[l], g, lv.origin, lv.domain_cells, lv.bc, False)
+
+    def advance(l, dt):
+        lv = levels[l]
+        r = step(U[l], g, dt, lv.dx, wl.gamma, wl.limiter, wl.riemann, ch=sm, alpha=wl.alpha, eps=eps,
+                 want_flux=True)
+        Uold[l], U[l] = U[l], r["U"]
+        counters.append(r["counters"])
+        nsteps[l] += 1
+        if l + 1 < L:
+            sibling_ghosts(l)                       # ghosts of the new level-l state for the theta = 1/2 stencil
+            Fsum = None
+            for theta in (0.0, 0.5):
+                mask = sibling_ghosts(l + 1)
+                prolong_ghosts(U[l + 1], mask, levels[l + 1], Uold[l], U[l], lv, theta)
+                Ff = advance(l + 1, 0.5 * dt)
+                Fsum = Ff if Fsum is None else Fsum + Ff
+            restrict(U[l + 1], levels[l + 1], U[l], lv)
+            if do_reflux:
+                reflux(U[l], lv, r["F"], levels[l + 1], Fsum, dt)
+        return r["F"]
+
+    sibling_ghosts(0)
+    advance(0, dt0)
+    tot1 = hierarchy_totals(U, levels)
+    return dict(U=[interior(U[l], g) for l in range(L)], dt0=dt0, smax=sm, totals_before=tot0, totals_after=tot1,
+                counters=counters, nsteps=nsteps)

@@ -24,6 +24,8 @@ from .configs import (  # noqa: F401
     config2_random_patches,
     config3_orszag_tang,
     config4_two_level,
+    config_hierarchy,
+    nested_hierarchy_from_fine,
     config5_turbulence,
     smooth_wave_patchset,
     uniform_grid_workload,

@@ -363,6 +363,85 @@ def config4_two_level(mhd: bool, nfine: int = 256, n: int = 16, sigma: float = C
     return w
 
 
+def _dilate_periodic(m: np.ndarray) -> np.ndarray:
+    out = np.zeros_like(m)
+    for dz in (-1, 0, 1):
+        for dy in (-1, 0, 1):
+            for dx in (-1, 0, 1):
+                out |= np.roll(m, (dz, dy, dx), axis=(0, 1, 2))
+    return out
+
+
+def _erode_periodic(m: np.ndarray) -> np.ndarray:
+    return ~_dilate_periodic(~m)
+
+
+def nested_hierarchy_from_fine(name: str, Gfine: np.ndarray, nlevels: int, n: int, thresholds: Sequence[float],
+                               gamma: float, mhd: bool, limiter: int, riemann: int) -> Workload:
+    """an L-level properly nested hierarchy cut from one fine periodic state Gfine
+    [nf, N, N, N] (N = the finest level's index space).  Level l's data are the 2x2x2 means of level l+1's
+    (so every level is the restriction of the next).  Level 0 covers the domain.  For l >= 1 a patch sits on
+    an aligned (n/2)^3 block of level l-1 cells; blocks are flagged where the level l-1 density exceeds
+    thresholds[l-1] x mean, grown by one block (for every level that has a finer one above it) and kept
+    only where all 27 blocks around them lie inside level l-1's patches (proper nesting: a level-l halo and
+    its prolongation stencil never leave level l-1).  Patches in Morton order."""
+    nf, N = Gfine.shape[0], Gfine.shape[1]
+    fields = [None] * nlevels
+    fields[nlevels - 1] = Gfine
+    for l in range(nlevels - 2, -1, -1):
+        M = fields[l + 1].shape[1] // 2
+        fields[l] = fields[l + 1].reshape(nf, M, 2, M, 2, M, 2).mean(axis=(2, 4, 6))
+    nb = n // 2
+    N0 = fields[0].shape[1]
+    origin0 = morton_patch_origins(N0 // n, N0 // n, N0 // n, n)
+    levels = [Level(n=n, g=3, level=0, dx=1.0 / N0, origin=origin0, domain_cells=(N0,) * 3, bc=(BC_PERIODIC,) * 6,
+                    self_periodic=False, U=split_into_patches(fields[0], n, origin0))]
+    cover_prev = None                                   # bool on level l-1's block grid (None: everything)
+    for l in range(1, nlevels):
+        Np = fields[l - 1].shape[1]                     # cells per side of level l-1
+        nblk = Np // nb
+        rho = fields[l - 1][0]
+        flag = rho.reshape(nblk, nb, nblk, nb, nblk, nb).max(axis=(1, 3, 5)) > thresholds[l - 1] * rho.mean()
+        if cover_prev is None:
+            allowed = np.ones_like(flag)
+        else:                                           # a level l-1 patch = 2x2x2 blocks of this grid
+            up = np.repeat(np.repeat(np.repeat(cover_prev, 2, axis=0), 2, axis=1), 2, axis=2)
+            allowed = _erode_periodic(up)
+        flag &= allowed
+        if l < nlevels - 1:
+            flag = _dilate_periodic(flag) & allowed
+        bz, by, bx = np.nonzero(flag)
+        order = np.argsort(morton_key(bx, by, bz), kind="stable")
+        bx, by, bz = bx[order], by[order], bz[order]
+        origin = (np.stack([bx, by, bz], axis=1) * n).astype(np.int32)
+        Nl = fields[l].shape[1]
+        levels.append(Level(n=n, g=3, level=l, dx=1.0 / Nl, origin=origin, domain_cells=(Nl,) * 3,
+                            bc=(BC_PERIODIC,) * 6, self_periodic=False, U=split_into_patches(fields[l], n, origin)))
+        cover_prev = flag
+    w = Workload(name, levels, gamma, mhd, limiter, riemann, 0.3, 1)
+    w.note = "patches per level: " + ", ".join(str(lv.npatch) for lv in levels)
+    return w
+
+
+def config_hierarchy(mhd: bool, nlevels: int = 3, nfine: int = 128, n: int = 16, sigma: float = CONFIG4_SIGMA,
+                     thresholds: Sequence[float] = (2.8, 4.0, 5.0, 6.0)) -> Workload:
+    """Config 4's lognormal state (A15) refined over `nlevels` levels (f3); nfine = finest index space."""
+    gamma = 5.0 / 3.0
+    N = nfine
+    rho = np.exp(sigma * gaussian_random_field(N, -2.0, _rng(4, 0)))
+    rho /= rho.mean()
+    v = np.stack([gaussian_random_field(N, -2.0, _rng(4, 1 + s)) for s in range(3)])
+    v *= 2.0 * np.sqrt(gamma) / np.sqrt(np.mean(v[0] ** 2 + v[1] ** 2 + v[2] ** 2))
+    p = np.ones_like(rho)
+    if mhd:
+        dB = solenoidal_random_field(N, -2.0, _rng(4, 4)) * 1.0e-4
+        Gf = primitive_to_conserved(rho, v, p, gamma, B=(dB[0], dB[1], dB[2] + 1.0e-3))
+    else:
+        Gf = primitive_to_conserved(rho, v, p, gamma)
+    return nested_hierarchy_from_fine("hierarchy%d_%s" % (nlevels, "mhd" if mhd else "hydro"), Gf, nlevels, n,
+                                      thresholds, gamma, mhd, LIM_MC, RS_HLLD if mhd else RS_HLLC)
+
+
 # --------------------------------------------------------------------------------------
 # smooth test states (pins P10, P12): single self-periodic patch of n^3 on [0,1]^3
 # --------------------------------------------------------------------------------------
