@@ -121,7 +121,10 @@ int amr_step_counters(amr_patch_batch* b, long long* counters, int reset);
 /* Device workspace (flux registers + tables) a link needs; 0 on error. */
 size_t amr_link_bytes(const amr_patch_batch* coarse, const amr_patch_batch* fine, int ratio);
 /* Ties a fine batch to its parent level (ratio must be 2).  dev_ws: device, borrowed like an arena.
- * From then on steps of both batches also record the face fluxes the reflux needs. */
+ * From then on steps of both batches also record the face fluxes the reflux needs.
+ * A batch can be the fine side of one link and the coarse side of another (a middle level); create the
+ * links from the root upwards and destroy them in the reverse order (AMR_ESTATE otherwise).  For a middle
+ * level amr_flux_clear of its child link zeroes only that link's own coarse faces. */
 int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, void* dev_ws, size_t bytes,
                     amr_level_link** out);
 int amr_link_destroy(amr_level_link* l);
@@ -136,6 +139,28 @@ int amr_restrict(amr_level_link* l);
 /* O9(7): U_c += s_f (dt_coarse/dx_coarse) (F_coarse - <F_fine>) on uncovered coarse cells next to a
  * fine patch face, from the fluxes recorded since amr_flux_clear. */
 int amr_reflux(amr_level_link* l, double dt_coarse);
+
+/* ---- L-level hierarchy with recursive subcycling -----------------------------------
+ * PAPER.md:31 "the different resolution levels are advanced in time with different time-steps"; :59 "once a
+ * refinement level is completed the solution is corrected ... and the next (coarser) level of refinement is
+ * processed"; :63 all levels stay resident on the device.  levels[0..nlevels) are the batches of levels
+ * 0..L-1 (all on one stream), links[l] = amr_link_levels(levels[l], levels[l+1]) created from the root
+ * upwards (a middle level is the fine side of one link and the coarse side of the next; the hierarchy must
+ * be properly nested: a level-(l+1) halo and its prolongation stencil lie inside level l's patches, else
+ * amr_link_levels fails with AMR_EINVAL).  Nothing is owned by these calls.
+ *
+ * amr_hierarchy_cfl_dt: smax = max over the levels of amr_cfl_dt's smax, dt0 = cfl * dx_0 / smax (one
+ * 8-byte read per level).
+ * amr_hierarchy_step: one root step dt0.  advance(l, dt): clear link l's flux registers; step level l by dt
+ * (hydro or MHD, with c_h = ch on every level); if level l+1 exists, twice { amr_prolong_ghosts(links[l],
+ * theta = 0, 1/2); advance(l+1, dt/2) }; amr_restrict(links[l]); amr_reflux(links[l], dt) unless do_reflux
+ * is 0.  Level l takes 2^l steps of dt0 / 2^l.  Only kernel launches are enqueued (no synchronisation).
+ * Errors: AMR_EINVAL for a null pointer, nlevels outside 1..30, links that do not tie consecutive entries of
+ * levels, dt0 not finite and > 0; otherwise the first error of the calls listed above. */
+int amr_hierarchy_cfl_dt(amr_patch_batch* const* levels, int nlevels, double gamma, double cfl, int mhd,
+                         double* dt0_out, double* smax_out);
+int amr_hierarchy_step(amr_patch_batch* const* levels, amr_level_link* const* links, int nlevels, int mhd,
+                       double dt0, double gamma, int limiter, int riemann, double ch, double alpha, int do_reflux);
 
 /* ---- patch builder ------------------------------------------------------------
  * The procedure the paper designed for the GPU (section 3, Figure 1): "AMR cells are

@@ -25,7 +25,7 @@ EXPORTS = (
     "amr_mhd_step", "amr_conserved_totals", "amr_step_counters", "amr_link_bytes", "amr_link_levels",
     "amr_link_destroy", "amr_prolong_ghosts", "amr_flux_clear", "amr_restrict", "amr_reflux", "amr_last_error",
     "amr_version", "amr_builder_bytes", "amr_builder_create", "amr_builder_destroy", "amr_builder_build",
-    "amr_builder_results", "amr_builder_gather",
+    "amr_builder_results", "amr_builder_gather", "amr_hierarchy_cfl_dt", "amr_hierarchy_step",
 )
 
 
@@ -86,6 +86,10 @@ def lib():
         L.amr_builder_destroy.argtypes = [C.c_void_p]
         L.amr_builder_build.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.POINTER(C.c_int64)]
         L.amr_builder_results.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.amr_hierarchy_cfl_dt.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.c_double, C.c_int,
+                                           C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.amr_hierarchy_step.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_double,
+                                         C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int]
         L.amr_builder_gather.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_int64,
                                          C.c_void_p, C.POINTER(C.c_int64)]
         _lib = L
@@ -252,6 +256,44 @@ class LevelLink:
         if self._h is not None and self._h.value:
             _check(lib().amr_link_destroy(self._h))
             self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Hierarchy:
+    """L levels resident on the device + the links between consecutive levels (SURVEY.md 8(f3));
+    amr_hierarchy_cfl_dt / amr_hierarchy_step do the recursive subcycling."""
+
+    def __init__(self, batches, mhd: bool):
+        self.levels = list(batches)
+        self.mhd = bool(mhd)
+        self.links = [LevelLink(self.levels[l], self.levels[l + 1]) for l in range(len(self.levels) - 1)]
+        n = len(self.levels)
+        self._lv = (C.c_void_p * n)(*[b.handle for b in self.levels])
+        self._lk = (C.c_void_p * max(n - 1, 1))(*[l._h for l in self.links])
+
+    @classmethod
+    def from_workload(cls, wl, dtype: int, **kw):
+        return cls([PatchBatch.from_level(lv, dtype, **kw) for lv in wl.levels], wl.mhd)
+
+    def cfl_dt(self, gamma: float, cfl: float):
+        dt, sm = C.c_double(), C.c_double()
+        _check(lib().amr_hierarchy_cfl_dt(self._lv, len(self.levels), gamma, cfl, int(self.mhd), C.byref(dt), C.byref(sm)))
+        return dt.value, sm.value
+
+    def step(self, dt0: float, gamma: float, limiter: int, riemann: int, ch: float = 0.0, alpha: float = 0.0,
+             do_reflux: bool = True):
+        _check(lib().amr_hierarchy_step(self._lv, self._lk, len(self.levels), int(self.mhd), dt0, gamma, limiter,
+                                        riemann, ch, alpha, int(do_reflux)))
+
+    def close(self):
+        for l in reversed(self.links):
+            l.close()
+        self.links = []
 
     def __del__(self):
         try:

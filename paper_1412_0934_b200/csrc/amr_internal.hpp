@@ -69,4 +69,7 @@ cudaError_t launch_restrict(int dtype, const void* Uf, size_t fs_f, int nf, int 
 cudaError_t launch_reflux(int dtype, void* Uc, size_t fs_c, int nf, int n, const long long* faces, int nfaces,
                           const void* Fc, const void* Ff, double dtdx, cudaStream_t s);
 
+// zeroes, for every entry of a reflux face table, the coarse flux slot it names (all fields)
+cudaError_t launch_zero_faces(int dtype, void* Fc, int nf, int n, const long long* faces, int nfaces, cudaStream_t s);
+
 }  // namespace amr

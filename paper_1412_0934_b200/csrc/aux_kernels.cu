@@ -181,6 +181,15 @@ __global__ void __launch_bounds__(256) restrict_kernel(const T* __restrict__ Uf,
   }
 }
 
+template <class T>
+__global__ void __launch_bounds__(256) zero_faces_kernel(T* __restrict__ Fc, int nf, size_t fsz,
+                                                         const long long* __restrict__ faces, int nfaces) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= nfaces) return;
+  const size_t oc = (size_t)faces[(size_t)e * 4 + 1];
+  for (int q = 0; q < nf; ++q) Fc[oc + (size_t)q * fsz] = T(0);
+}
+
 // ---- O9(7): reflux --------------------------------------------------------------------------------
 // faces[e][4] = { flat coarse interior index of the cell to correct,
 //                 flat offset of the coarse flux inside field 0 of the coarse flux-block array,
@@ -319,6 +328,17 @@ cudaError_t launch_reflux(int dtype, void* Uc, size_t fs_c, int nf, int n, const
   else
     reflux_kernel<double><<<grid, 256, 0, s>>>((double*)Uc, fs_c, nf, n, faces, nfaces, (const double*)Fc,
                                               (const double*)Ff, dtdx);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_zero_faces(int dtype, void* Fc, int nf, int n, const long long* faces, int nfaces, cudaStream_t s) {
+  if (nfaces == 0) return cudaSuccess;
+  const unsigned grid = (unsigned)((nfaces + 255) / 256);
+  const size_t fsz = (size_t)n * n * (n + 1);
+  if (dtype == 0)
+    zero_faces_kernel<float><<<grid, 256, 0, s>>>((float*)Fc, nf, fsz, faces, nfaces);
+  else
+    zero_faces_kernel<double><<<grid, 256, 0, s>>>((double*)Fc, nf, fsz, faces, nfaces);
   return cudaGetLastError();
 }
 

@@ -115,7 +115,8 @@ struct amr_patch_batch {
   bool needs_halo, halo_valid;
   bool smax_valid;
   double smax_gamma;
-  amr_level_link* link;
+  amr_level_link* link_up;    // the link this batch is the fine side of (to its parent level)
+  amr_level_link* link_down;  // the link this batch is the coarse side of (to its child level)
 };
 
 struct amr_level_link {
@@ -131,6 +132,7 @@ struct amr_level_link {
   void *fblk_c, *fblk_f;
   size_t fblk_c_bytes, fblk_f_bytes;
   int nblk_c;
+  bool shared_c;  // the coarse batch is itself a fine one: its per-patch blocks (owned by its link_up) are used
 };
 
 namespace {
@@ -139,6 +141,7 @@ struct LinkHost {
   std::vector<long long> pro_dst, pro_c7, res_dst, faces[6];
   std::vector<int> fblk_of_c;
   int nblk_c = 0;
+  bool identity_c = false;  // coarse blocks are per patch (block index = patch index)
 };
 
 struct LinkLayout {
@@ -235,7 +238,7 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
             const int* oc = &c->origin[3 * pc];
             int lc[3] = {C[0] - oc[0], C[1] - oc[1], C[2] - oc[2]};
             const long long cell = (long long)pc * (long long)n3 + ((long long)lc[2] * n + lc[1]) * n + lc[0];
-            if (H.fblk_of_c[pc] < 0) H.fblk_of_c[pc] = H.nblk_c++;
+            if (H.fblk_of_c[pc] < 0) H.fblk_of_c[pc] = H.identity_c ? pc : H.nblk_c++;
             int lface[3] = {lc[0], lc[1], lc[2]};
             if (!side) lface[d] += 1;  // upper face of the outside cell
             const long long oc_off = ((long long)H.fblk_of_c[pc] * 3 + d) * NF * fsz + slab_off(d, lface);
@@ -263,7 +266,7 @@ LinkLayout make_link_layout(const amr_patch_batch* c, const amr_patch_batch* f, 
   L.res_dst = off; off += up(H.res_dst.size() * 8 + 8);
   for (int s = 0; s < 6; ++s) { L.faces[s] = off; off += up(H.faces[s].size() * 8 + 8); }
   const size_t n = f->d.n, blk = 3 * (size_t)f->d.nfields * n * n * (n + 1) * f->esz;
-  L.fblk_c_bytes = (size_t)H.nblk_c * blk;
+  L.fblk_c_bytes = H.identity_c ? 0 : (size_t)H.nblk_c * blk;
   L.fblk_f_bytes = (size_t)f->d.npatch * blk;
   L.fblk_c = off; off += up(L.fblk_c_bytes + 8);
   L.fblk_f = off; off += up(L.fblk_f_bytes + 8);
@@ -459,7 +462,7 @@ int amr_patch_batch_create(const amr_batch_desc* desc, void* dev_arena, size_t b
   b->halo_valid = false;
   b->smax_valid = false;
   b->smax_gamma = 0;
-  b->link = nullptr;
+  b->link_up = b->link_down = nullptr;
   auto bail = [&](cudaError_t e, const char* what) {
     delete b;
     return fail(AMR_ECUDA, "%s: %s", what, cudaGetErrorString(e));
@@ -482,7 +485,7 @@ int amr_patch_batch_create(const amr_batch_desc* desc, void* dev_arena, size_t b
 
 int amr_patch_batch_destroy(amr_patch_batch* b) {
   if (!b) return AMR_OK;
-  if (b->link) return fail(AMR_ESTATE, "batch is still linked; call amr_link_destroy first");
+  if (b->link_up || b->link_down) return fail(AMR_ESTATE, "batch is still linked; call amr_link_destroy first");
   cudaStreamSynchronize(b->stream);
   delete b;
   return AMR_OK;
@@ -622,6 +625,7 @@ int amr_step_counters(amr_patch_batch* b, long long* counters, int reset) {
 size_t amr_link_bytes(const amr_patch_batch* coarse, const amr_patch_batch* fine, int ratio) {
   if (check_link_args(coarse, fine, ratio) != AMR_OK) return 0;
   LinkHost H;
+  H.identity_c = coarse->link_up != nullptr;
   if (build_link(coarse, fine, H) != AMR_OK) return 0;
   return make_link_layout(coarse, fine, H).total;
 }
@@ -632,9 +636,15 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   *out = nullptr;
   int rc = check_link_args(coarse, fine, ratio);
   if (rc != AMR_OK) return rc;
-  if (coarse->link || fine->link) return fail(AMR_ESTATE, "batch already linked");
+  if (coarse->link_down) return fail(AMR_ESTATE, "the coarse batch already has a child level");
+  if (fine->link_up) return fail(AMR_ESTATE, "the fine batch already has a parent level");
+  if (fine->link_down) return fail(AMR_ESTATE, "link a hierarchy from the root upwards: the fine batch already has a child level");
   if (!dev_ws || (uintptr_t)dev_ws % ALIGN) return fail(AMR_EINVAL, "workspace must be a %zu-byte aligned device pointer", ALIGN);
   LinkHost H;
+  // a middle level records every patch's fluxes already (it is the fine side of its parent link): its role as
+  // the coarse side of this link reads the same per-patch blocks (the two sets of faces are disjoint under
+  // proper nesting, and amr_flux_clear of this link zeroes only its own faces there)
+  H.identity_c = coarse->link_up != nullptr;
   rc = build_link(coarse, fine, H);
   if (rc != AMR_OK) return rc;
   const LinkLayout L = make_link_layout(coarse, fine, H);
@@ -651,6 +661,8 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   l->fblk_c = l->ws + L.fblk_c; l->fblk_f = l->ws + L.fblk_f;
   l->fblk_c_bytes = L.fblk_c_bytes; l->fblk_f_bytes = L.fblk_f_bytes;
   l->nblk_c = H.nblk_c;
+  l->shared_c = H.identity_c;
+  if (l->shared_c) l->fblk_c = coarse->fblk;
   cudaStream_t s = coarse->stream;
   auto h2d = [&](void* dst, const void* src, size_t nb) {
     return nb ? cudaMemcpyAsync(dst, src, nb, cudaMemcpyHostToDevice, s) : cudaSuccess;
@@ -659,27 +671,29 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   if (e == cudaSuccess) e = h2d(l->pro_c7, H.pro_c7.data(), H.pro_c7.size() * 8);
   if (e == cudaSuccess) e = h2d(l->res_dst, H.res_dst.data(), H.res_dst.size() * 8);
   for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = h2d(l->faces[k], H.faces[k].data(), H.faces[k].size() * 8);
-  if (e == cudaSuccess) e = h2d(coarse->fblk_of, H.fblk_of_c.data(), H.fblk_of_c.size() * sizeof(int));
+  if (e == cudaSuccess && !l->shared_c) e = h2d(coarse->fblk_of, H.fblk_of_c.data(), H.fblk_of_c.size() * sizeof(int));
   std::vector<int> idf(fine->d.npatch);
   for (int p = 0; p < fine->d.npatch; ++p) idf[p] = p;
   if (e == cudaSuccess) e = h2d(fine->fblk_of, idf.data(), idf.size() * sizeof(int));
-  if (e == cudaSuccess) e = cudaMemsetAsync(l->fblk_c, 0, L.fblk_c_bytes + 8, s);
+  if (e == cudaSuccess && !l->shared_c) e = cudaMemsetAsync(l->fblk_c, 0, L.fblk_c_bytes + 8, s);
   if (e == cudaSuccess) e = cudaMemsetAsync(l->fblk_f, 0, L.fblk_f_bytes + 8, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e != cudaSuccess) { delete l; return fail(AMR_ECUDA, "link upload: %s", cudaGetErrorString(e)); }
-  coarse->fblk = l->nblk_c ? l->fblk_c : nullptr;
+  if (!l->shared_c) coarse->fblk = l->nblk_c ? l->fblk_c : nullptr;
   fine->fblk = l->fblk_f;
-  coarse->link = fine->link = l;
+  coarse->link_down = fine->link_up = l;
   *out = l;
   return AMR_OK;
 }
 
 int amr_link_destroy(amr_level_link* l) {
   if (!l) return AMR_OK;
+  if (l->f->link_down) return fail(AMR_ESTATE, "destroy the finer link first (it records into this link's fine blocks)");
   cudaStreamSynchronize(l->c->stream);
   cudaStreamSynchronize(l->f->stream);
-  l->c->fblk = nullptr; l->f->fblk = nullptr;
-  l->c->link = nullptr; l->f->link = nullptr;
+  if (!l->shared_c) l->c->fblk = nullptr;
+  l->f->fblk = nullptr;
+  l->c->link_down = nullptr; l->f->link_up = nullptr;
   delete l;
   return AMR_OK;
 }
@@ -697,7 +711,15 @@ int amr_prolong_ghosts(amr_level_link* l, double theta) {
 
 int amr_flux_clear(amr_level_link* l) {
   if (!l) return fail(AMR_EINVAL, "null link");
-  if (l->fblk_c_bytes) CUDA_TRY(cudaMemsetAsync(l->fblk_c, 0, l->fblk_c_bytes, l->c->stream));
+  if (l->shared_c) {
+    for (int s = 0; s < 6; ++s) {
+      cudaError_t e = amr::launch_zero_faces(l->c->d.dtype, l->fblk_c, l->c->d.nfields, l->c->d.n, l->faces[s], l->nfaces[s],
+                                             l->c->stream);
+      if (e != cudaSuccess) return fail(AMR_ECUDA, "flux clear kernel launch: %s", cudaGetErrorString(e));
+    }
+  } else if (l->fblk_c_bytes) {
+    CUDA_TRY(cudaMemsetAsync(l->fblk_c, 0, l->fblk_c_bytes, l->c->stream));
+  }
   if (l->fblk_f_bytes) CUDA_TRY(cudaMemsetAsync(l->fblk_f, 0, l->fblk_f_bytes, l->f->stream));
   return AMR_OK;
 }
@@ -723,6 +745,77 @@ int amr_reflux(amr_level_link* l, double dt_coarse) {
   }
   c->smax_valid = false;
   return AMR_OK;
+}
+
+}  // extern "C"
+
+// ---- L-level hierarchy ---------------------------------------------------------------
+
+namespace {
+
+int check_hierarchy(amr_patch_batch* const* levels, amr_level_link* const* links, int nlevels) {
+  if (!levels || nlevels < 1 || nlevels > 30) return fail(AMR_EINVAL, "levels must hold 1..30 batches");
+  for (int l = 0; l < nlevels; ++l)
+    if (!levels[l]) return fail(AMR_EINVAL, "null batch at level %d", l);
+  if (nlevels > 1 && !links) return fail(AMR_EINVAL, "null links");
+  for (int l = 0; l + 1 < nlevels; ++l)
+    if (!links[l] || links[l]->c != levels[l] || links[l]->f != levels[l + 1])
+      return fail(AMR_EINVAL, "links[%d] must tie levels[%d] (coarse) to levels[%d] (fine)", l, l, l + 1);
+  return AMR_OK;
+}
+
+struct CycleArgs {
+  amr_patch_batch* const* levels;
+  amr_level_link* const* links;
+  int nlevels, mhd, limiter, riemann, do_reflux;
+  double gamma, ch, alpha;
+};
+
+// advance(l, dt) of oracle.api.hierarchy_step, call for call
+int advance_level(const CycleArgs& A, int l, double dt) {
+  const bool has_child = l + 1 < A.nlevels;
+  int rc;
+  if (has_child && (rc = amr_flux_clear(A.links[l])) != AMR_OK) return rc;
+  rc = A.mhd ? amr_mhd_step(A.levels[l], dt, A.gamma, A.limiter, A.riemann, A.ch, A.alpha)
+             : amr_hydro_step(A.levels[l], dt, A.gamma, A.limiter, A.riemann);
+  if (rc != AMR_OK || !has_child) return rc;
+  for (int sub = 0; sub < 2; ++sub) {
+    if ((rc = amr_prolong_ghosts(A.links[l], 0.5 * sub)) != AMR_OK) return rc;
+    if ((rc = advance_level(A, l + 1, 0.5 * dt)) != AMR_OK) return rc;
+  }
+  if ((rc = amr_restrict(A.links[l])) != AMR_OK) return rc;
+  if (A.do_reflux && (rc = amr_reflux(A.links[l], dt)) != AMR_OK) return rc;
+  return AMR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int amr_hierarchy_cfl_dt(amr_patch_batch* const* levels, int nlevels, double gamma, double cfl, int mhd,
+                         double* dt0_out, double* smax_out) {
+  if (!levels || nlevels < 1 || nlevels > 30) return fail(AMR_EINVAL, "levels must hold 1..30 batches");
+  int rc;
+  double sm = 0;
+  for (int l = 0; l < nlevels; ++l) {
+    if (!levels[l]) return fail(AMR_EINVAL, "null batch at level %d", l);
+    double dt_l, sm_l;
+    if ((rc = amr_cfl_dt(levels[l], gamma, cfl, mhd, &dt_l, &sm_l)) != AMR_OK) return rc;
+    sm = sm_l > sm ? sm_l : sm;
+  }
+  if (!(sm > 0) || !std::isfinite(sm)) return fail(AMR_ESTATE, "maximum signal speed over the levels is not finite and > 0");
+  if (dt0_out) *dt0_out = cfl * levels[0]->d.dx / sm;
+  if (smax_out) *smax_out = sm;
+  return AMR_OK;
+}
+
+int amr_hierarchy_step(amr_patch_batch* const* levels, amr_level_link* const* links, int nlevels, int mhd, double dt0,
+                       double gamma, int limiter, int riemann, double ch, double alpha, int do_reflux) {
+  int rc = check_hierarchy(levels, links, nlevels);
+  if (rc != AMR_OK) return rc;
+  if (!(dt0 > 0) || !std::isfinite(dt0)) return fail(AMR_EINVAL, "dt0 must be finite and > 0");
+  CycleArgs A{levels, links, nlevels, mhd, limiter, riemann, do_reflux, gamma, ch, alpha};
+  return advance_level(A, 0, dt0);
 }
 
 }  // extern "C"

@@ -57,6 +57,18 @@ def gpu_two_level_step(wl, np_dtype=np.float64, do_reflux=True):
     return out
 
 
+def gpu_hierarchy_step(wl, np_dtype=np.float64, do_reflux=True, nsteps=1):
+    """f3 through amr_hierarchy_cfl_dt / amr_hierarchy_step (the recursion runs inside the library, in the
+    order of oracle.api.hierarchy_step)."""
+    h = amr.Hierarchy.from_workload(wl, gpu_dtype(np_dtype))
+    dts = []
+    for _ in range(nsteps):
+        dt0, sm = h.cfl_dt(wl.gamma, wl.cfl)
+        h.step(dt0, wl.gamma, wl.limiter, wl.riemann, sm, wl.alpha, do_reflux)
+        dts.append(dt0)
+    return dict(U=[b.download() for b in h.levels], dt0=dts[-1], dts=dts, smax=sm, hierarchy=h)
+
+
 def field_groups(nf):
     """A18: momentum and B are normalised by the max over their three components."""
     g = [[0], [1, 2, 3], [4]]
