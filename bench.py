@@ -331,6 +331,94 @@ def run_builder(args):
     print(json.dumps(out))
 
 
+def run_hierarchy(args):
+    """--workload hierarchy3_f32 | hierarchy3_f64: the multi-level row of the scope table (SURVEY.md 8(f3);
+    PAPER.md:31, 59, 63).  A step = one root step of a three-level properly nested MHD hierarchy, all levels
+    resident: amr_hierarchy_cfl_dt + amr_hierarchy_step (1 + 2 + 4 level steps with prolongation, restriction and
+    reflux between them).  The metric counts cell-updates (cells of level l x 2^l per root step)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    import paper_1412_0934_b200 as amr
+    f32 = args.workload.endswith("f32")
+    nfine = args.size or 512
+    wl = wk.config_hierarchy(True, 3, nfine, n=16)
+    L = len(wl.levels)
+    tdt = torch.float32 if f32 else torch.float64
+    host = []
+    for lv in wl.levels:
+        h = torch.empty(lv.U.shape, dtype=tdt, pin_memory=True)
+        h.copy_(torch.from_numpy(lv.U))
+        host.append(h)
+    hier = amr.Hierarchy.from_workload(wl, amr.AMR_F32 if f32 else amr.AMR_F64)
+    updates = sum(lv.ncells << l for l, lv in enumerate(wl.levels))
+
+    def step():
+        dt0, sm = hier.cfl_dt(wl.gamma, wl.cfl)
+        hier.step(dt0, wl.gamma, wl.limiter, wl.riemann, sm, wl.alpha, True)
+
+    K, Wm = args.steps, max(args.warmup, 3)
+    for _ in range(Wm):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start(); time.sleep(0.25)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K):
+        step()
+    e1.record(); torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1) / K
+    # end to end: every level's state from pinned host memory, one root step, every level back
+    nbytes = int(sum(h.numel() * h.element_size() for h in host))
+    e2e = None
+    if not args.no_e2e:
+        for b, h in zip(hier.levels, host):
+            b.upload(h.numpy())
+        s2, t2 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s2.record()
+        for _ in range(3):
+            for b, h in zip(hier.levels, host):
+                b.upload(h.numpy())
+            step()
+            outs = [b.download() for b in hier.levels]
+        t2.record(); torch.cuda.synchronize()
+        ms2 = s2.elapsed_time(t2) / 3
+        e2e = dict(value=updates / (ms2 * 1e-3), unit=UNIT, h2d_bytes_per_step=nbytes, d2h_bytes_per_step=nbytes,
+                   ms_per_step=ms2, steps=3)
+    pk = peaks()
+    bpc = 2 * 9 * (4 if f32 else 8)
+    ach = bpc * updates / (ms * 1e-3) / 1e9
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import api as oracle
+        ws = wk.config_hierarchy(True, 3, 256, n=16)
+        t0 = time.perf_counter()
+        oracle.hierarchy_step(ws)
+        dt = time.perf_counter() - t0
+        nu = sum(lv.ncells << l for l, lv in enumerate(ws.levels))
+        cpu = dict(value=nu / dt, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                   sample="the same recipe at 256^3 finest index space (%s; %d cell-updates), one root step, fp64, %.1f s" % (ws.note, nu, dt))
+    # kernels per root step: level steps 2^l; per step of a level with a child: 2 prolongations, 1 restriction,
+    # up to 6 reflux launches, up to 6 face-clear launches if it is a middle level; 1 smax launch per level whose
+    # fused smax was invalidated by restriction / reflux
+    launches = sum((1 << l) * (1 + (2 + 1 + 6 + (6 if l > 0 else 0) if l + 1 < L else 0)) for l in range(L)) + (L - 1)
+    out = dict(metric=METRIC, value=updates / (ms * 1e-3), unit=UNIT, n_gpus=1, steps=K, warmup=Wm, ms_per_step=ms,
+               higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32" if f32 else "f64", data="synthetic",
+               config=dict(workload="hierarchy3 (f3): %d^3 finest index space, 16^3 patches, %s, MHD %s, MC+HLLD+GLM"
+                           % (nfine, wl.note, "fp32" if f32 else "fp64"),
+                           step="amr_hierarchy_cfl_dt + amr_hierarchy_step: 1 + 2 + 4 level steps, prolongation / restriction / reflux between levels",
+                           cell_updates_per_step=updates,
+                           l2="the whole hierarchy (%.0f MB) fits the 126 MB L2 only at small sizes; no flush: every level step rewrites its level" % (nbytes / 1e6)),
+               roofline=dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"], traffic=None,
+                             peak_source=pk["source"], kernel="whole root step (7 step-kernel launches + AMR operators)",
+                             kernel_ms=ms, bytes_per_cell=bpc),
+               cpu_baseline=cpu,
+               e2e=e2e, gpu_launches=K * launches, clocks=clocks)
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -348,6 +436,10 @@ def main():
         if args.impl == "reference":
             raise SystemExit("the reference arm times the hot path (config 2, 3, 5); the patch builder's oracle is timed in cpu_baseline")
         return run_builder(args)
+    if args.workload.startswith("hierarchy3"):
+        if args.impl == "reference":
+            raise SystemExit("the reference arm times the hot path (config 2, 3, 5); the hierarchy's oracle is timed in cpu_baseline")
+        return run_hierarchy(args)
     if args.impl == "reference":
         return run_reference(args)
 

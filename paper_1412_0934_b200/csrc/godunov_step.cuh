@@ -671,10 +671,11 @@ __global__ void __maxnreg__(MAXR) godunov_step_kernel(const __grid_constant__ St
             riemann<T, NF, RS>(WL, WR, RC, Fr, s_cnt);
             rotate_out<T, NF, 2>(Fr, fz);
           }
-          if (blk >= 0 && (t <= zc || z0 + zc == n)) {
+          // only the face planes a link can read (index 0, n/2, n along the normal) are recorded
+          if (blk >= 0 && (t <= zc || z0 + zc == n) && (kk == 0 || kk == (n >> 1) || kk == n)) {
             T* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)kk * n2 + (size_t)((y0 + bj) * n + (x0 + bi)));
 #pragma unroll
-            for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += fz[q];
+            for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, fz[q]);
           }
           if (t >= 2) {  // O6 for plane kk-1, GLM damping, O7 of the new state
             // U_old: rho, B, psi are the ring record of plane kk-1 (conversion leaves them untouched),
@@ -734,10 +735,10 @@ __global__ void __maxnreg__(MAXR) godunov_step_kernel(const __grid_constant__ St
         riemann<T, NF, RS>(WL, WR, RC, Fr, s_cnt);
         rotate_out<T, NF, 0>(Fr, wmx);
         sts_cell<T, NF>(xfp, wmx);
-        if (blk >= 0 && (bi < TX || x0 + TX == n)) {  // record the flux for the reflux
+        if (blk >= 0 && (bi < TX || x0 + TX == n) && (x0 + bi == 0 || x0 + bi == (n >> 1) || x0 + bi == n)) {  // record the flux for the reflux
           T* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + bj)) * (n + 1) + (x0 + bi));
 #pragma unroll
-          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += wmx[q];
+          for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, wmx[q]);
         }
       }
       if (do_y) {
@@ -748,10 +749,10 @@ __global__ void __maxnreg__(MAXR) godunov_step_kernel(const __grid_constant__ St
         riemann<T, NF, RS>(WL, WR, RC, Fr, s_cnt);
         rotate_out<T, NF, 1>(Fr, wmy);
         sts_cell<T, NF>(yfp, wmy);
-        if (blk >= 0 && (bj < TY || y0 + TY == n)) {
+        if (blk >= 0 && (bj < TY || y0 + TY == n) && (y0 + bj == 0 || y0 + bj == (n >> 1) || y0 + bj == n)) {
           T* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + (y0 + bj)) * n + (x0 + bi));
 #pragma unroll
-          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += wmy[q];
+          for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, wmy[q]);
         }
       }
     }

@@ -308,10 +308,12 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
             x2::riemann2<NF, RS>(WL, WR, RC, Fr, true, s_cnt);
             rot_out<NF, 2>(Fr, fz);
           }
-          if (X2_UNLIKELY(blk >= 0)) {  // flux registers of a coarse-fine link (a7): z faces kk = 0..n
+          // flux registers of a coarse-fine link (a7).  Only the face planes a link can read are recorded: index 0,
+          // n/2, n along the normal (fine patches sit on aligned (n/2)^3 blocks of the parent level)
+          if (X2_UNLIKELY(blk >= 0) && (kk == 0 || kk == (n >> 1) || kk == n)) {
             double* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)kk * n2 + (size_t)((y0 + pj) * n + (x0 + pc)));
 #pragma unroll
-            for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += fz[q];
+            for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, fz[q]);
           }
           if (t >= 2) {  // O6 for plane kk-1, GLM damping, O7 of the new state
             // U_old: rho, B, psi are the ring record of plane kk-1 (conversion leaves them untouched), (m, E)
@@ -369,14 +371,15 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
           sts_rec<NF>(rec, Fr);       // for the left / lower neighbour's phase 3
           st_block(bj, Fr);           // private copy for this thread's phase 3 (the neighbour overwrites rec in ITS
                                       // next phase 1, with no barrier in between)
-          if (X2_UNLIKELY(blk >= 0)) {  // record the flux for the reflux
+          const int fidx = d ? y0 + pj : x0 + pc;   // face index along the normal
+          if (X2_UNLIKELY(blk >= 0) && (fidx == 0 || fidx == (n >> 1))) {  // record the flux for the reflux
             double f[NF];
             if (d) rot_out<NF, 1>(Fr, f); else rot_out<NF, 0>(Fr, f);
             double* dstF = P.fblk + ((size_t)blk * 3 + d) * NF * fsz +
                            (d ? ((size_t)(kk * (n + 1) + (y0 + pj)) * n + (x0 + pc))
                               : ((size_t)(kk * n + (y0 + pj)) * (n + 1) + (x0 + pc)));
 #pragma unroll
-            for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += f[q];
+            for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, f[q]);
           }
         }
       }
@@ -568,13 +571,13 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
           if (right && x0 + HX == n) {
             double* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + n);
 #pragma unroll
-            for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += Fr[q];
+            for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, Fr[q]);
           } else if (top && y0 + TY == n) {
             double fy[NF];
             rot_out<NF, 1>(Fr, fy);
             double* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + n) * n + (x0 + cx - 2));
 #pragma unroll
-            for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += fy[q];
+            for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, fy[q]);
           }
         }
       }

@@ -379,10 +379,14 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
             riemann2<NF, RS>(WL, WR, RC, Fr, B2(true), s_cnt);
             rot_out<NF, 2>(Fr, fz);
           }
-          if (X2_UNLIKELY(blk >= 0)) {  // flux registers of a coarse-fine link (a7): z faces kk = 0..n
+          // flux registers of a coarse-fine link (a7).  Only the face planes a link can read are recorded: index 0,
+          // n/2, n along the normal (fine patches sit on aligned (n/2)^3 blocks of the parent level).  The sum over
+          // substeps is a result-less atomicAdd (RED): one writer per address and step, so the value is that of
+          // a plain +=, without exposing the load latency of a read-modify-write in this latency-bound loop
+          if (X2_UNLIKELY(blk >= 0) && (kk == 0 || kk == (n >> 1) || kk == n)) {
             float* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)kk * n2 + (size_t)((y0 + pj) * n + (x0 + 2 * pc)));
 #pragma unroll
-            for (int q = 0; q < NF; ++q) { dstF[(size_t)q * fsz] += fz[q].v.x; dstF[(size_t)q * fsz + 1] += fz[q].v.y; }
+            for (int q = 0; q < NF; ++q) { atomicAdd(dstF + (size_t)q * fsz, fz[q].v.x); atomicAdd(dstF + (size_t)q * fsz + 1, fz[q].v.y); }
           }
           if (t >= 2) {  // O6 for plane kk-1, GLM damping, O7 of the new state
             // U_old: rho, B, psi are the ring record of plane kk-1 (conversion leaves them untouched),
@@ -462,10 +466,11 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
             // barrier in between
             st_block(BX, fx, 0.f, 0.f);
           }
-          if (X2_UNLIKELY(blk >= 0)) {  // record the fluxes for the reflux
+          // record the fluxes for the reflux: x faces 0 and n/2 are the even face of a pair
+          if (X2_UNLIKELY(blk >= 0) && (x0 + 2 * pc == 0 || x0 + 2 * pc == (n >> 1))) {
             float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + (x0 + 2 * pc));
 #pragma unroll
-            for (int q = 0; q < NF; ++q) { dstF[(size_t)q * fsz] += fx[q].v.x; dstF[(size_t)q * fsz + 1] += fx[q].v.y; }
+            for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, fx[q].v.x);
           }
         }
         {
@@ -482,10 +487,10 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
             for (int q = 0; q < 9; ++q) o[q] = q < NF ? fy[q] : F2(0.f);
             st_block(BY, o, 0.f, 0.f);  // private copy for phase 3 (same reason)
           }
-          if (X2_UNLIKELY(blk >= 0)) {
+          if (X2_UNLIKELY(blk >= 0) && (y0 + pj == 0 || y0 + pj == (n >> 1))) {
             float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + (y0 + pj)) * n + (x0 + 2 * pc));
 #pragma unroll
-            for (int q = 0; q < NF; ++q) { dstF[(size_t)q * fsz] += fy[q].v.x; dstF[(size_t)q * fsz + 1] += fy[q].v.y; }
+            for (int q = 0; q < NF; ++q) { atomicAdd(dstF + (size_t)q * fsz, fy[q].v.x); atomicAdd(dstF + (size_t)q * fsz + 1, fy[q].v.y); }
           }
         }
       }
@@ -700,7 +705,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
         if (X2_UNLIKELY(blk >= 0) && x0 + TX == n) {  // the patch's last x face (a7)
           float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + n);
 #pragma unroll
-          for (int q = 0; q < NF; ++q) dstF[(size_t)q * fsz] += wm[q].v.x;
+          for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, wm[q].v.x);
         }
       } else if (mid && top) {
         F2 wl[NF], WL[NF], WR[NF], Fr[NF];
@@ -713,7 +718,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
         if (X2_UNLIKELY(blk >= 0) && y0 + TY == n) {
           float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + n) * n + (x0 + 2 * (px - 1)));
 #pragma unroll
-          for (int q = 0; q < NF; ++q) { dstF[(size_t)q * fsz] += wm[q].v.x; dstF[(size_t)q * fsz + 1] += wm[q].v.y; }
+          for (int q = 0; q < NF; ++q) { atomicAdd(dstF + (size_t)q * fsz, wm[q].v.x); atomicAdd(dstF + (size_t)q * fsz + 1, wm[q].v.y); }
         }
       }
       cp_wait<0>();
