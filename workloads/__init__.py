@@ -26,6 +26,10 @@ from .configs import (  # noqa: F401
     config4_two_level,
     config_hierarchy,
     nested_hierarchy_from_fine,
+    select_blocks,
+    blocks_to_origins,
+    origins_to_blocks,
+    patch_flags_to_block_grid,
     config5_turbulence,
     smooth_wave_patchset,
     uniform_grid_workload,

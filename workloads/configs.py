@@ -376,6 +376,50 @@ def _erode_periodic(m: np.ndarray) -> np.ndarray:
     return ~_dilate_periodic(~m)
 
 
+def select_blocks(flag: np.ndarray, cover_prev: Optional[np.ndarray], grow: bool) -> np.ndarray:
+    """Geometry policy of a (re)grid: which flagged (n/2)^3 blocks of level l-1 [bool, (z, y, x) block grid]
+    become level-l patches.  cover_prev = the block grid of level l-1's own patches one level down (None: level
+    l-1 covers the domain).  A block is allowed only where all 27 blocks around it lie inside level l-1
+    (proper nesting); `grow` adds one block around the flagged ones (for a level that will carry a finer one)."""
+    if cover_prev is None:
+        allowed = np.ones_like(flag)
+    else:                                               # a level l-1 patch = 2x2x2 blocks of this grid
+        up = np.repeat(np.repeat(np.repeat(cover_prev, 2, axis=0), 2, axis=1), 2, axis=2)
+        allowed = _erode_periodic(up)
+    flag = flag & allowed
+    if grow:
+        flag = _dilate_periodic(flag) & allowed
+    return flag
+
+
+def blocks_to_origins(flag: np.ndarray, n: int) -> np.ndarray:
+    """Patch origins (level-l cell units, Morton order) of the selected blocks of level l-1."""
+    bz, by, bx = np.nonzero(flag)
+    order = np.argsort(morton_key(bx, by, bz), kind="stable")
+    return (np.stack([bx[order], by[order], bz[order]], axis=1) * n).astype(np.int32)
+
+
+def origins_to_blocks(origin: np.ndarray, n: int, nblk: int) -> np.ndarray:
+    """Inverse of blocks_to_origins: bool block grid [nblk]^3 (z, y, x) of a level's patches."""
+    g = np.zeros((nblk, nblk, nblk), bool)
+    o = np.asarray(origin) // n
+    g[o[:, 2], o[:, 1], o[:, 0]] = True
+    return g
+
+
+def patch_flags_to_block_grid(level: Level, flags: np.ndarray) -> np.ndarray:
+    """Per-patch block flags [np, 2, 2, 2] (z, y, x halves) of `level` -> its block grid [2 N / n]^3."""
+    nb = level.n // 2
+    nblk = level.domain_cells[0] // nb
+    g = np.zeros((nblk, nblk, nblk), bool)
+    o = np.asarray(level.origin) // nb
+    for dz in range(2):
+        for dy in range(2):
+            for dx in range(2):
+                g[o[:, 2] + dz, o[:, 1] + dy, o[:, 0] + dx] = flags[:, dz, dy, dx]
+    return g
+
+
 def nested_hierarchy_from_fine(name: str, Gfine: np.ndarray, nlevels: int, n: int, thresholds: Sequence[float],
                                gamma: float, mhd: bool, limiter: int, riemann: int) -> Workload:
     """an L-level properly nested hierarchy cut from one fine periodic state Gfine
@@ -402,18 +446,8 @@ def nested_hierarchy_from_fine(name: str, Gfine: np.ndarray, nlevels: int, n: in
         nblk = Np // nb
         rho = fields[l - 1][0]
         flag = rho.reshape(nblk, nb, nblk, nb, nblk, nb).max(axis=(1, 3, 5)) > thresholds[l - 1] * rho.mean()
-        if cover_prev is None:
-            allowed = np.ones_like(flag)
-        else:                                           # a level l-1 patch = 2x2x2 blocks of this grid
-            up = np.repeat(np.repeat(np.repeat(cover_prev, 2, axis=0), 2, axis=1), 2, axis=2)
-            allowed = _erode_periodic(up)
-        flag &= allowed
-        if l < nlevels - 1:
-            flag = _dilate_periodic(flag) & allowed
-        bz, by, bx = np.nonzero(flag)
-        order = np.argsort(morton_key(bx, by, bz), kind="stable")
-        bx, by, bz = bx[order], by[order], bz[order]
-        origin = (np.stack([bx, by, bz], axis=1) * n).astype(np.int32)
+        flag = select_blocks(flag, cover_prev, grow=l < nlevels - 1)
+        origin = blocks_to_origins(flag, n)
         Nl = fields[l].shape[1]
         levels.append(Level(n=n, g=3, level=l, dx=1.0 / Nl, origin=origin, domain_cells=(Nl,) * 3,
                             bc=(BC_PERIODIC,) * 6, self_periodic=False, U=split_into_patches(fields[l], n, origin)))
