@@ -26,6 +26,7 @@ EXPORTS = (
     "amr_link_destroy", "amr_prolong_ghosts", "amr_flux_clear", "amr_restrict", "amr_reflux", "amr_last_error",
     "amr_version", "amr_builder_bytes", "amr_builder_create", "amr_builder_destroy", "amr_builder_build",
     "amr_builder_results", "amr_builder_gather", "amr_hierarchy_cfl_dt", "amr_hierarchy_step",
+    "amr_flag_blocks", "amr_regrid_bytes", "amr_regrid_fill",
 )
 
 
@@ -86,6 +87,10 @@ def lib():
         L.amr_builder_destroy.argtypes = [C.c_void_p]
         L.amr_builder_build.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.POINTER(C.c_int64)]
         L.amr_builder_results.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.amr_flag_blocks.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_void_p]
+        L.amr_regrid_bytes.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.amr_regrid_bytes.restype = C.c_size_t
+        L.amr_regrid_fill.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t]
         L.amr_hierarchy_cfl_dt.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.c_double, C.c_int,
                                            C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.amr_hierarchy_step.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_double,
@@ -209,6 +214,23 @@ class PatchBatch:
         _check(lib().amr_step_counters(self._h, out.ctypes.data, int(reset)))
         return dict(zip(CNT_NAMES, out.tolist()))
 
+    def flag_blocks(self, field: int, threshold: float) -> np.ndarray:
+        """amr_flag_blocks: bool [npatch, 2, 2, 2] (z, y, x halves of each patch)."""
+        out = np.zeros(self.npatch * 8, dtype=np.uint8)
+        _check(lib().amr_flag_blocks(self.handle, int(field), float(threshold), out.ctypes.data))
+        return out.reshape(self.npatch, 2, 2, 2).astype(bool)
+
+    def regrid_fill(self, old_fine, coarse):
+        """amr_regrid_fill into this (new, not yet linked) fine batch."""
+        import torch
+        L = lib()
+        oh = old_fine.handle if old_fine is not None else None
+        nbytes = L.amr_regrid_bytes(self.handle, oh, coarse.handle)
+        if nbytes == 0:
+            raise AmrError(-1, L.amr_last_error().decode())
+        ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        _check(L.amr_regrid_fill(self.handle, oh, coarse.handle, ws.data_ptr(), nbytes))
+
     def synchronize(self):
         self._torch.cuda.synchronize(self.device)
 
@@ -272,6 +294,9 @@ class Hierarchy:
         self.levels = list(batches)
         self.mhd = bool(mhd)
         self.links = [LevelLink(self.levels[l], self.levels[l + 1]) for l in range(len(self.levels) - 1)]
+        self._tables()
+
+    def _tables(self):
         n = len(self.levels)
         self._lv = (C.c_void_p * n)(*[b.handle for b in self.levels])
         self._lk = (C.c_void_p * max(n - 1, 1))(*[l._h for l in self.links])
@@ -279,6 +304,18 @@ class Hierarchy:
     @classmethod
     def from_workload(cls, wl, dtype: int, **kw):
         return cls([PatchBatch.from_level(lv, dtype, **kw) for lv in wl.levels], wl.mhd)
+
+    def replace_level(self, l: int, new_batch):
+        """After a regrid: level l's batch is replaced by new_batch (already filled, amr_regrid_fill).  The links
+        from level l-1 upwards are destroyed finest first and rebuilt root upwards."""
+        assert 1 <= l < len(self.levels)
+        for k in range(len(self.links) - 1, l - 2, -1):
+            self.links[k].close()
+        self.links = self.links[:l - 1]
+        self.levels[l] = new_batch
+        for k in range(l - 1, len(self.levels) - 1):
+            self.links.append(LevelLink(self.levels[k], self.levels[k + 1]))
+        self._tables()
 
     def cfl_dt(self, gamma: float, cfl: float):
         dt, sm = C.c_double(), C.c_double()

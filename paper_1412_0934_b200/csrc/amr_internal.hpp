@@ -72,4 +72,12 @@ cudaError_t launch_reflux(int dtype, void* Uc, size_t fs_c, int nf, int n, const
 // zeroes, for every entry of a reflux face table, the coarse flux slot it names (all fields)
 cudaError_t launch_zero_faces(int dtype, void* Fc, int nf, int n, const long long* faces, int nfaces, cudaStream_t s);
 
+// regridding (aux_kernels.cu): block flags of one field [np*8]; whole-patch copies; whole-patch prolongation
+cudaError_t launch_flag_blocks(int dtype, const void* Ufield, int np, int n, double threshold, unsigned char* flags,
+                               cudaStream_t s);
+cudaError_t launch_copy_patches(int dtype, void* Unew, size_t fs_new, const void* Uold, size_t fs_old, const void* pairs,
+                                int npairs, int nf, int n, cudaStream_t s);
+cudaError_t launch_prolong_patches(int dtype, void* Unew, size_t fs_new, int nf, int n, const int* born, const long long* c7,
+                                   int nparents, const void* Uc, size_t fs_c, cudaStream_t s);
+
 }  // namespace amr

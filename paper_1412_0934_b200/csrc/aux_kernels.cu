@@ -152,6 +152,72 @@ __global__ void __launch_bounds__(256) prolong_kernel(T* __restrict__ halo, size
   }
 }
 
+// ---- regridding ------------------------------------------------------------------
+// One block per (patch, aligned (n/2)^3 block): flag = max of one field over the block > threshold.
+template <class T>
+__global__ void __launch_bounds__(128) flag_blocks_kernel(const T* __restrict__ U, int n, T threshold,
+                                                          unsigned char* __restrict__ flags) {
+  const int p = blockIdx.x >> 3, blk = blockIdx.x & 7;
+  const int h = n >> 1, h3 = h * h * h;
+  const int bx = blk & 1, by = (blk >> 1) & 1, bz = blk >> 2;
+  const T* u = U + (size_t)p * n * n * n;
+  bool hit = false;
+  for (int r = threadIdx.x; r < h3; r += blockDim.x) {
+    const int i = r % h, j = (r / h) % h, k = r / (h * h);
+    hit |= u[((size_t)(bz * h + k) * n + (by * h + j)) * n + (bx * h + i)] > threshold;
+  }
+  const int any = __syncthreads_or(hit ? 1 : 0);
+  if (threadIdx.x == 0) flags[blockIdx.x] = any ? 1 : 0;
+}
+
+// kept patches: pairs[e] = (new patch, old patch); grid (npairs, nf)
+template <class T>
+__global__ void __launch_bounds__(256) copy_patches_kernel(T* __restrict__ Unew, size_t fs_new,
+                                                           const T* __restrict__ Uold, size_t fs_old,
+                                                           const int2* __restrict__ pairs, int n3) {
+  const int2 pr = pairs[blockIdx.x];
+  const T* src = Uold + (size_t)blockIdx.y * fs_old + (size_t)pr.y * n3;
+  T* dst = Unew + (size_t)blockIdx.y * fs_new + (size_t)pr.x * n3;
+  for (int r = threadIdx.x; r < n3; r += blockDim.x) dst[r] = src[r];
+}
+
+// new-born patches: one thread per coarse parent cell; born[b] = new patch index, c7[(b h^3 + r) 7 + .] = flat
+// coarse interior indices (centre, x-, x+, y-, y+, z-, z+) of parent r = (ck h + cj) h + ci.  The 8 children get
+// U_C -+ 1/4 minmod slopes, accumulated in the order x, y, z (as prolong_kernel, O8).
+template <class T>
+__global__ void __launch_bounds__(128) prolong_patches_kernel(T* __restrict__ Unew, size_t fs_new, int nf, int n,
+                                                              const int* __restrict__ born,
+                                                              const long long* __restrict__ c7, int nparents,
+                                                              const T* __restrict__ Uc, size_t fs_c) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= nparents) return;
+  const int h = n >> 1, h3 = h * h * h;
+  const int b = e / h3, r = e - b * h3;
+  const int ci = r % h, cj = (r / h) % h, ck = r / (h * h);
+  long long s[7];
+#pragma unroll
+  for (int k = 0; k < 7; ++k) s[k] = c7[(size_t)e * 7 + k];
+  T* dst0 = Unew + (size_t)born[b] * n * n * n + ((size_t)(2 * ck) * n + 2 * cj) * n + 2 * ci;
+  for (int q = 0; q < nf; ++q) {
+    const T* a = Uc + (size_t)q * fs_c;
+    T st[7];
+#pragma unroll
+    for (int k = 0; k < 7; ++k) st[k] = a[s[k]];
+    T sl[3];
+#pragma unroll
+    for (int dd = 0; dd < 3; ++dd) sl[dd] = minmod2<T>(st[0] - st[1 + 2 * dd], st[2 + 2 * dd] - st[0]);
+    T* dst = dst0 + (size_t)q * fs_new;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      T val = st[0];
+      val += ((c & 1) ? T(0.25) : T(-0.25)) * sl[0];
+      val += ((c & 2) ? T(0.25) : T(-0.25)) * sl[1];
+      val += ((c & 4) ? T(0.25) : T(-0.25)) * sl[2];
+      dst[((size_t)((c >> 2) & 1) * n + ((c >> 1) & 1)) * n + (c & 1)] = val;
+    }
+  }
+}
+
 // ---- O9(6): restriction ---------------------------------------------------------------------------
 // entry e <-> (fine patch p, coarse-cell offset inside the patch); dst[e] = flat coarse interior index
 template <class T>
@@ -339,6 +405,35 @@ cudaError_t launch_zero_faces(int dtype, void* Fc, int nf, int n, const long lon
     zero_faces_kernel<float><<<grid, 256, 0, s>>>((float*)Fc, nf, fsz, faces, nfaces);
   else
     zero_faces_kernel<double><<<grid, 256, 0, s>>>((double*)Fc, nf, fsz, faces, nfaces);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_flag_blocks(int dtype, const void* Ufield, int np, int n, double threshold, unsigned char* flags,
+                               cudaStream_t s) {
+  if (np == 0) return cudaSuccess;
+  if (dtype == 0) flag_blocks_kernel<float><<<(unsigned)np * 8, 128, 0, s>>>((const float*)Ufield, n, (float)threshold, flags);
+  else flag_blocks_kernel<double><<<(unsigned)np * 8, 128, 0, s>>>((const double*)Ufield, n, threshold, flags);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_copy_patches(int dtype, void* Unew, size_t fs_new, const void* Uold, size_t fs_old, const void* pairs,
+                                int npairs, int nf, int n, cudaStream_t s) {
+  if (npairs == 0) return cudaSuccess;
+  const dim3 grid((unsigned)npairs, (unsigned)nf);
+  const int n3 = n * n * n;
+  if (dtype == 0) copy_patches_kernel<float><<<grid, 256, 0, s>>>((float*)Unew, fs_new, (const float*)Uold, fs_old, (const int2*)pairs, n3);
+  else copy_patches_kernel<double><<<grid, 256, 0, s>>>((double*)Unew, fs_new, (const double*)Uold, fs_old, (const int2*)pairs, n3);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_prolong_patches(int dtype, void* Unew, size_t fs_new, int nf, int n, const int* born, const long long* c7,
+                                   int nparents, const void* Uc, size_t fs_c, cudaStream_t s) {
+  if (nparents == 0) return cudaSuccess;
+  const unsigned grid = (unsigned)((nparents + 127) / 128);
+  if (dtype == 0)
+    prolong_patches_kernel<float><<<grid, 128, 0, s>>>((float*)Unew, fs_new, nf, n, born, c7, nparents, (const float*)Uc, fs_c);
+  else
+    prolong_patches_kernel<double><<<grid, 128, 0, s>>>((double*)Unew, fs_new, nf, n, born, c7, nparents, (const double*)Uc, fs_c);
   return cudaGetLastError();
 }
 

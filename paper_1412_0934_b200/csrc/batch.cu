@@ -819,3 +819,147 @@ int amr_hierarchy_step(amr_patch_batch* const* levels, amr_level_link* const* li
 }
 
 }  // extern "C"
+
+// ---- regridding between steps -----------------------------------------------------------
+
+namespace {
+
+// flat interior index of coarse cell C (level index space, wrapped / clamped by the level's boundary
+// conditions) in the coarse batch; false if no patch of the batch holds it
+bool coarse_cell_flat(const amr_patch_batch* c, int Cx, int Cy, int Cz, long long* out) {
+  const int n = c->d.n;
+  const int* domc = c->d.domain_cells;
+  int C[3] = {Cx, Cy, Cz};
+  for (int a = 0; a < 3; ++a) {
+    if (C[a] < 0) C[a] = (c->d.bc[2 * a] == AMR_BC_PERIODIC) ? C[a] + domc[a] : 0;
+    else if (C[a] >= domc[a]) C[a] = (c->d.bc[2 * a + 1] == AMR_BC_PERIODIC) ? C[a] - domc[a] : domc[a] - 1;
+  }
+  const int pc = c->map.at(C[0] / n, C[1] / n, C[2] / n);
+  if (pc < 0) return false;
+  const int* oc = &c->origin[3 * pc];
+  *out = (long long)pc * (long long)c->n3 + ((long long)(C[2] - oc[2]) * n + (C[1] - oc[1])) * n + (C[0] - oc[0]);
+  return true;
+}
+
+struct RegridHost {
+  std::vector<int> pairs;       // (new, old) per kept patch
+  std::vector<int> born;        // new patch index per new-born patch
+  std::vector<long long> c7;    // [born][h^3][7]
+};
+
+struct RegridLayout { size_t pairs, born, c7, total; };
+
+int check_regrid_args(const amr_patch_batch* nw, const amr_patch_batch* old, const amr_patch_batch* c) {
+  if (!nw || !c) return fail(AMR_EINVAL, "null batch");
+  int rc = check_link_args(c, nw, 2);
+  if (rc != AMR_OK) return rc;
+  if (old && (old->d.n != nw->d.n || old->d.nfields != nw->d.nfields || old->d.dtype != nw->d.dtype ||
+              old->d.level != nw->d.level))
+    return fail(AMR_EINVAL, "old and new fine batches must agree in n, nfields, dtype, level");
+  if (old)
+    for (int a = 0; a < 3; ++a)
+      if (old->d.domain_cells[a] != nw->d.domain_cells[a]) return fail(AMR_EINVAL, "old and new fine batches must share the index space");
+  return AMR_OK;
+}
+
+int build_regrid(const amr_patch_batch* nw, const amr_patch_batch* old, const amr_patch_batch* c, RegridHost& H) {
+  const int n = nw->d.n, h = n / 2;
+  for (int p = 0; p < nw->d.npatch; ++p) {
+    const int* o = &nw->origin[3 * p];
+    const int po = old ? old->map.at(o[0] / n, o[1] / n, o[2] / n) : -1;
+    if (po >= 0) { H.pairs.push_back(p); H.pairs.push_back(po); continue; }
+    H.born.push_back(p);
+    for (int ck = 0; ck < h; ++ck)
+      for (int cj = 0; cj < h; ++cj)
+        for (int ci = 0; ci < h; ++ci) {
+          const int C[3] = {o[0] / 2 + ci, o[1] / 2 + cj, o[2] / 2 + ck};
+          long long s7[7];
+          bool ok = coarse_cell_flat(c, C[0], C[1], C[2], &s7[0]);
+          for (int a = 0; a < 3 && ok; ++a) {
+            int Cm[3] = {C[0], C[1], C[2]}, Cp[3] = {C[0], C[1], C[2]};
+            Cm[a] -= 1;
+            Cp[a] += 1;
+            ok = coarse_cell_flat(c, Cm[0], Cm[1], Cm[2], &s7[1 + 2 * a]) && coarse_cell_flat(c, Cp[0], Cp[1], Cp[2], &s7[2 + 2 * a]);
+          }
+          if (!ok) return fail(AMR_EINVAL, "new patch %d is not properly nested in the coarse level (a parent cell or its stencil is missing)", p);
+          for (int q = 0; q < 7; ++q) H.c7.push_back(s7[q]);
+        }
+  }
+  return AMR_OK;
+}
+
+RegridLayout make_regrid_layout(const RegridHost& H) {
+  RegridLayout L;
+  size_t off = 0;
+  L.pairs = off; off += up(H.pairs.size() * sizeof(int) + 8);
+  L.born = off; off += up(H.born.size() * sizeof(int) + 8);
+  L.c7 = off; off += up(H.c7.size() * 8 + 8);
+  L.total = off;
+  return L;
+}
+
+}  // namespace
+
+extern "C" {
+
+int amr_flag_blocks(amr_patch_batch* b, int field, double threshold, unsigned char* host_flags) {
+  if (!b || !host_flags) return fail(AMR_EINVAL, "null pointer");
+  if (field < 0 || field >= b->d.nfields) return fail(AMR_EINVAL, "field must be in [0, nfields)");
+  if (b->d.n % 2) return fail(AMR_EINVAL, "n must be even");
+  const size_t nflag = (size_t)b->d.npatch * 8;
+  unsigned char* dflags = nullptr;
+  CUDA_TRY(cudaMallocAsync((void**)&dflags, nflag, b->stream));
+  const char* U = (const char*)b->U[b->cur] + (size_t)field * b->d.npatch * b->n3 * b->esz;
+  cudaError_t e = amr::launch_flag_blocks(b->d.dtype, U, b->d.npatch, b->d.n, threshold, dflags, b->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(host_flags, dflags, nflag, cudaMemcpyDeviceToHost, b->stream);
+  cudaError_t e2 = cudaFreeAsync(dflags, b->stream);
+  if (e == cudaSuccess) e = e2;
+  if (e == cudaSuccess) e = cudaStreamSynchronize(b->stream);
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "flag kernel: %s", cudaGetErrorString(e));
+  return AMR_OK;
+}
+
+size_t amr_regrid_bytes(const amr_patch_batch* new_fine, const amr_patch_batch* old_fine, const amr_patch_batch* coarse) {
+  if (check_regrid_args(new_fine, old_fine, coarse) != AMR_OK) return 0;
+  RegridHost H;
+  if (build_regrid(new_fine, old_fine, coarse, H) != AMR_OK) return 0;
+  return make_regrid_layout(H).total;
+}
+
+int amr_regrid_fill(amr_patch_batch* new_fine, const amr_patch_batch* old_fine, const amr_patch_batch* coarse, void* dev_ws,
+                    size_t bytes) {
+  int rc = check_regrid_args(new_fine, old_fine, coarse);
+  if (rc != AMR_OK) return rc;
+  if (old_fine && old_fine->stream != new_fine->stream) return fail(AMR_EINVAL, "old and new fine batches must share the stream");
+  if (!dev_ws || (uintptr_t)dev_ws % ALIGN) return fail(AMR_EINVAL, "workspace must be a %zu-byte aligned device pointer", ALIGN);
+  RegridHost H;
+  rc = build_regrid(new_fine, old_fine, coarse, H);
+  if (rc != AMR_OK) return rc;
+  const RegridLayout L = make_regrid_layout(H);
+  if (bytes < L.total) return fail(AMR_EINVAL, "workspace too small: %zu < %zu bytes", bytes, L.total);
+  cudaStream_t s = new_fine->stream;
+  char* ws = (char*)dev_ws;
+  auto h2d = [&](void* dst, const void* src, size_t nb) {
+    return nb ? cudaMemcpyAsync(dst, src, nb, cudaMemcpyHostToDevice, s) : cudaSuccess;
+  };
+  cudaError_t e = h2d(ws + L.pairs, H.pairs.data(), H.pairs.size() * sizeof(int));
+  if (e == cudaSuccess) e = h2d(ws + L.born, H.born.data(), H.born.size() * sizeof(int));
+  if (e == cudaSuccess) e = h2d(ws + L.c7, H.c7.data(), H.c7.size() * 8);
+  const int nf = new_fine->d.nfields, n = new_fine->d.n, h = n / 2;
+  const size_t fs_new = (size_t)new_fine->d.npatch * new_fine->n3;
+  if (e == cudaSuccess && old_fine)
+    e = amr::launch_copy_patches(new_fine->d.dtype, new_fine->U[new_fine->cur], fs_new, old_fine->U[old_fine->cur],
+                                 (size_t)old_fine->d.npatch * old_fine->n3, ws + L.pairs, (int)(H.pairs.size() / 2), nf, n, s);
+  if (e == cudaSuccess)
+    e = amr::launch_prolong_patches(new_fine->d.dtype, new_fine->U[new_fine->cur], fs_new, nf, n, (const int*)(ws + L.born),
+                                    (const long long*)(ws + L.c7), (int)H.born.size() * h * h * h, coarse->U[coarse->cur],
+                                    (size_t)coarse->d.npatch * coarse->n3, s);
+  // the tables are host vectors: the copies above must have left them before they go out of scope
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "regrid fill: %s", cudaGetErrorString(e));
+  new_fine->smax_valid = false;
+  new_fine->halo_valid = false;
+  return AMR_OK;
+}
+
+}  // extern "C"
