@@ -12,6 +12,8 @@
 #include <new>
 #include <string>
 #include <vector>
+#include <atomic>
+#include <utility>
 
 #include "../../include/amr_godunov.h"
 #include "amr_internal.hpp"
@@ -115,6 +117,7 @@ struct amr_patch_batch {
   bool needs_halo, halo_valid;
   bool smax_valid;
   double smax_gamma;
+  unsigned long long serial;  // unique per created batch (keys the link-table cache)
   amr_level_link* link_up;    // the link this batch is the fine side of (to its parent level)
   amr_level_link* link_down;  // the link this batch is the coarse side of (to its child level)
 };
@@ -258,6 +261,15 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
   return AMR_OK;
 }
 
+// amr_link_bytes has to build the tables to size the workspace; amr_link_levels, called next for the same pair,
+// takes them from here instead of building them again (host work: O(halo cells) map look-ups)
+struct LinkCache {
+  unsigned long long c = 0, f = 0;
+  bool identity_c = false;
+  LinkHost H;
+};
+thread_local LinkCache g_link_cache;
+
 LinkLayout make_link_layout(const amr_patch_batch* c, const amr_patch_batch* f, const LinkHost& H) {
   LinkLayout L;
   size_t off = 0;
@@ -385,6 +397,8 @@ int amr_patch_batch_create(const amr_batch_desc* desc, void* dev_arena, size_t b
   if (bytes < L.total) return fail(AMR_EINVAL, "arena too small: %zu < %zu bytes", bytes, L.total);
 
   amr_patch_batch* b = new (std::nothrow) amr_patch_batch();
+  static std::atomic<unsigned long long> next_serial{1};
+  if (b) b->serial = next_serial.fetch_add(1);
   if (!b) return fail(AMR_ENOMEM, "out of host memory");
   b->d = *desc;
   b->d.origin = nullptr;
@@ -627,7 +641,12 @@ size_t amr_link_bytes(const amr_patch_batch* coarse, const amr_patch_batch* fine
   LinkHost H;
   H.identity_c = coarse->link_up != nullptr;
   if (build_link(coarse, fine, H) != AMR_OK) return 0;
-  return make_link_layout(coarse, fine, H).total;
+  const size_t total = make_link_layout(coarse, fine, H).total;
+  g_link_cache.c = coarse->serial;
+  g_link_cache.f = fine->serial;
+  g_link_cache.identity_c = H.identity_c;
+  g_link_cache.H = std::move(H);
+  return total;
 }
 
 int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, void* dev_ws, size_t bytes,
@@ -645,7 +664,13 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   // the coarse side of this link reads the same per-patch blocks (the two sets of faces are disjoint under
   // proper nesting, and amr_flux_clear of this link zeroes only its own faces there)
   H.identity_c = coarse->link_up != nullptr;
-  rc = build_link(coarse, fine, H);
+  if (g_link_cache.c == coarse->serial && g_link_cache.f == fine->serial && g_link_cache.identity_c == H.identity_c) {
+    H = std::move(g_link_cache.H);
+    rc = AMR_OK;
+  } else {
+    rc = build_link(coarse, fine, H);
+  }
+  g_link_cache = LinkCache();
   if (rc != AMR_OK) return rc;
   const LinkLayout L = make_link_layout(coarse, fine, H);
   if (bytes < L.total) return fail(AMR_EINVAL, "workspace too small: %zu < %zu bytes", bytes, L.total);
