@@ -427,9 +427,9 @@ def run_hierarchy(args):
         cpu = dict(value=nu / dt, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
                    sample="the same recipe at 256^3 finest index space (%s; %d cell-updates), one root step, fp64, %.1f s" % (ws.note, nu, dt))
     # kernels per root step: level steps 2^l; per step of a level with a child: 2 prolongations, 1 restriction,
-    # up to 6 reflux launches, up to 6 face-clear launches if it is a middle level; 1 smax launch per level whose
-    # fused smax was invalidated by restriction / reflux
-    launches = sum((1 << l) * (1 + (2 + 1 + 6 + (6 if l > 0 else 0) if l + 1 < L else 0)) for l in range(L)) + (L - 1)
+    # 1 reflux, 1 face-clear launch if it is a middle level; 1 smax launch per level whose fused smax was
+    # invalidated by restriction / reflux
+    launches = sum((1 << l) * (1 + (2 + 1 + 1 + (1 if l > 0 else 0) if l + 1 < L else 0)) for l in range(L)) + (L - 1)
     out = dict(metric=METRIC, value=updates / (ms * 1e-3), unit=UNIT, n_gpus=1, steps=K, warmup=Wm, ms_per_step=ms,
                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32" if f32 else "f64", data="synthetic",
                config=dict(workload="hierarchy3 (f3): %d^3 finest index space, 16^3 patches, %s, MHD %s, MC+HLLD+GLM"

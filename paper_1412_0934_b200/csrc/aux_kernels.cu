@@ -140,8 +140,13 @@ __global__ void __launch_bounds__(256) prolong_kernel(T* __restrict__ halo, size
     const T* a = Uold + (size_t)q * fs_c;
     const T* b = Unew + (size_t)q * fs_c;
     T st[7];
+    if (theta == T(0)) {        // first substep: the old state alone (w0 = 1: the same value, half the loads)
 #pragma unroll
-    for (int k = 0; k < 7; ++k) st[k] = w0 * a[s[k]] + theta * b[s[k]];
+      for (int k = 0; k < 7; ++k) st[k] = a[s[k]];
+    } else {
+#pragma unroll
+      for (int k = 0; k < 7; ++k) st[k] = w0 * a[s[k]] + theta * b[s[k]];
+    }
     T val = st[0];
 #pragma unroll
     for (int dd = 0; dd < 3; ++dd) {
@@ -266,33 +271,39 @@ template <class T>
 __global__ void __launch_bounds__(256) reflux_kernel(T* __restrict__ Uc, size_t fs_c, int nf, int n,
                                                      const long long* __restrict__ faces, int nfaces,
                                                      const T* __restrict__ Fc, const T* __restrict__ Ff, T dtdx) {
-  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  int e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= nfaces) return;
-  const size_t cell = (size_t)faces[(size_t)e * 4 + 0];
-  const size_t oc = (size_t)faces[(size_t)e * 4 + 1];
-  const size_t of = (size_t)faces[(size_t)e * 4 + 2];
-  const int code = (int)faces[(size_t)e * 4 + 3];
-  const T sf = (code & 1) ? T(-1) : T(1);
-  const int d = (code >> 1) & 3;
+  // the table is sorted by coarse cell: the thread at the first entry of a cell applies all of that cell's entries
+  // in table order ((direction, side) ascending), every other thread of the run has nothing to do
+  const long long cell_ll = faces[(size_t)e * 4 + 0];
+  if (e > 0 && faces[(size_t)(e - 1) * 4 + 0] == cell_ll) return;
+  const size_t cell = (size_t)cell_ll;
   const size_t fsz = (size_t)n * n * (n + 1);
-  // strides of the two transverse directions t1 = (d+1)%3 (a), t2 = (d+2)%3 (b) inside a d-slab
-  // slab extents: (z, y, x) with n+1 along d
-  size_t sx = 1, sy, sz;
-  if (d == 0) { sy = n + 1; sz = (size_t)n * (n + 1); }
-  else if (d == 1) { sy = n; sz = (size_t)n * (n + 1); }
-  else { sy = n; sz = (size_t)n * n; }
-  const size_t str3[3] = {sx, sy, sz};
-  const size_t sa = str3[(d + 1) % 3], sb = str3[(d + 2) % 3];
-  for (int q = 0; q < nf; ++q) {
-    const T Fcoarse = Fc[oc + (size_t)q * fsz];
-    const T* f = Ff + of + (size_t)q * fsz;
-    T sum = T(0);
-    sum += f[0];
-    sum += f[sa];
-    sum += f[sb];
-    sum += f[sa + sb];
-    const T Ffine = T(0.25) * T(0.5) * sum;
-    Uc[(size_t)q * fs_c + cell] += sf * dtdx * (Fcoarse - Ffine);
+  for (; e < nfaces && faces[(size_t)e * 4 + 0] == cell_ll; ++e) {
+    const size_t oc = (size_t)faces[(size_t)e * 4 + 1];
+    const size_t of = (size_t)faces[(size_t)e * 4 + 2];
+    const int code = (int)faces[(size_t)e * 4 + 3];
+    const T sf = (code & 1) ? T(-1) : T(1);
+    const int d = (code >> 1) & 3;
+    // strides of the two transverse directions t1 = (d+1)%3 (a), t2 = (d+2)%3 (b) inside a d-slab
+    // slab extents: (z, y, x) with n+1 along d
+    size_t sx = 1, sy, sz;
+    if (d == 0) { sy = n + 1; sz = (size_t)n * (n + 1); }
+    else if (d == 1) { sy = n; sz = (size_t)n * (n + 1); }
+    else { sy = n; sz = (size_t)n * n; }
+    const size_t str3[3] = {sx, sy, sz};
+    const size_t sa = str3[(d + 1) % 3], sb = str3[(d + 2) % 3];
+    for (int q = 0; q < nf; ++q) {
+      const T Fcoarse = Fc[oc + (size_t)q * fsz];
+      const T* f = Ff + of + (size_t)q * fsz;
+      T sum = T(0);
+      sum += f[0];
+      sum += f[sa];
+      sum += f[sb];
+      sum += f[sa + sb];
+      const T Ffine = T(0.25) * T(0.5) * sum;
+      Uc[(size_t)q * fs_c + cell] += sf * dtdx * (Fcoarse - Ffine);
+    }
   }
 }
 

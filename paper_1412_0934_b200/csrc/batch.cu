@@ -130,8 +130,8 @@ struct amr_level_link {
   int npro;
   long long* res_dst;
   int nres;
-  long long* faces[6];
-  int nfaces[6];
+  long long* faces;  // all (direction, side) tables merged, sorted by coarse cell (stable in d*2+side)
+  int nfaces;
   void *fblk_c, *fblk_f;
   size_t fblk_c_bytes, fblk_f_bytes;
   int nblk_c;
@@ -141,14 +141,14 @@ struct amr_level_link {
 namespace {
 
 struct LinkHost {
-  std::vector<long long> pro_dst, pro_c7, res_dst, faces[6];
+  std::vector<long long> pro_dst, pro_c7, res_dst, faces[6], faces_all;
   std::vector<int> fblk_of_c;
   int nblk_c = 0;
   bool identity_c = false;  // coarse blocks are per patch (block index = patch index)
 };
 
 struct LinkLayout {
-  size_t pro_dst, pro_c7, res_dst, faces[6], fblk_c, fblk_f, total, fblk_c_bytes, fblk_f_bytes;
+  size_t pro_dst, pro_c7, res_dst, faces, fblk_c, fblk_f, total, fblk_c_bytes, fblk_f_bytes;
 };
 
 int wrapi(int v, int m) { return ((v % m) + m) % m; }
@@ -258,6 +258,17 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
           }
       }
   }
+  // one table for one launch: entries sorted by coarse cell, (direction, side) order kept inside a cell, so a
+  // cell that touches fine patches on several sides gets its corrections in a fixed order from one thread
+  struct Ent { long long v[4]; int s; };
+  std::vector<Ent> all;
+  for (int sd = 0; sd < 6; ++sd)
+    for (size_t e = 0; e + 3 < H.faces[sd].size(); e += 4)
+      all.push_back(Ent{{H.faces[sd][e], H.faces[sd][e + 1], H.faces[sd][e + 2], H.faces[sd][e + 3]}, sd});
+  std::stable_sort(all.begin(), all.end(), [](const Ent& a, const Ent& b) { return a.v[0] < b.v[0]; });
+  H.faces_all.reserve(all.size() * 4);
+  for (const Ent& en : all)
+    for (int q = 0; q < 4; ++q) H.faces_all.push_back(en.v[q]);
   return AMR_OK;
 }
 
@@ -276,7 +287,7 @@ LinkLayout make_link_layout(const amr_patch_batch* c, const amr_patch_batch* f, 
   L.pro_dst = off; off += up(H.pro_dst.size() * 8 + 8);
   L.pro_c7 = off; off += up(H.pro_c7.size() * 8 + 8);
   L.res_dst = off; off += up(H.res_dst.size() * 8 + 8);
-  for (int s = 0; s < 6; ++s) { L.faces[s] = off; off += up(H.faces[s].size() * 8 + 8); }
+  L.faces = off; off += up(H.faces_all.size() * 8 + 8);
   const size_t n = f->d.n, blk = 3 * (size_t)f->d.nfields * n * n * (n + 1) * f->esz;
   L.fblk_c_bytes = H.identity_c ? 0 : (size_t)H.nblk_c * blk;
   L.fblk_f_bytes = (size_t)f->d.npatch * blk;
@@ -682,7 +693,8 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   l->res_dst = (long long*)(l->ws + L.res_dst);
   l->npro = (int)H.pro_dst.size();
   l->nres = (int)H.res_dst.size();
-  for (int s = 0; s < 6; ++s) { l->faces[s] = (long long*)(l->ws + L.faces[s]); l->nfaces[s] = (int)(H.faces[s].size() / 4); }
+  l->faces = (long long*)(l->ws + L.faces);
+  l->nfaces = (int)(H.faces_all.size() / 4);
   l->fblk_c = l->ws + L.fblk_c; l->fblk_f = l->ws + L.fblk_f;
   l->fblk_c_bytes = L.fblk_c_bytes; l->fblk_f_bytes = L.fblk_f_bytes;
   l->nblk_c = H.nblk_c;
@@ -695,7 +707,7 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   cudaError_t e = h2d(l->pro_dst, H.pro_dst.data(), H.pro_dst.size() * 8);
   if (e == cudaSuccess) e = h2d(l->pro_c7, H.pro_c7.data(), H.pro_c7.size() * 8);
   if (e == cudaSuccess) e = h2d(l->res_dst, H.res_dst.data(), H.res_dst.size() * 8);
-  for (int k = 0; k < 6 && e == cudaSuccess; ++k) e = h2d(l->faces[k], H.faces[k].data(), H.faces[k].size() * 8);
+  if (e == cudaSuccess) e = h2d(l->faces, H.faces_all.data(), H.faces_all.size() * 8);
   if (e == cudaSuccess && !l->shared_c) e = h2d(coarse->fblk_of, H.fblk_of_c.data(), H.fblk_of_c.size() * sizeof(int));
   std::vector<int> idf(fine->d.npatch);
   for (int p = 0; p < fine->d.npatch; ++p) idf[p] = p;
@@ -737,11 +749,8 @@ int amr_prolong_ghosts(amr_level_link* l, double theta) {
 int amr_flux_clear(amr_level_link* l) {
   if (!l) return fail(AMR_EINVAL, "null link");
   if (l->shared_c) {
-    for (int s = 0; s < 6; ++s) {
-      cudaError_t e = amr::launch_zero_faces(l->c->d.dtype, l->fblk_c, l->c->d.nfields, l->c->d.n, l->faces[s], l->nfaces[s],
-                                             l->c->stream);
-      if (e != cudaSuccess) return fail(AMR_ECUDA, "flux clear kernel launch: %s", cudaGetErrorString(e));
-    }
+    cudaError_t e = amr::launch_zero_faces(l->c->d.dtype, l->fblk_c, l->c->d.nfields, l->c->d.n, l->faces, l->nfaces, l->c->stream);
+    if (e != cudaSuccess) return fail(AMR_ECUDA, "flux clear kernel launch: %s", cudaGetErrorString(e));
   } else if (l->fblk_c_bytes) {
     CUDA_TRY(cudaMemsetAsync(l->fblk_c, 0, l->fblk_c_bytes, l->c->stream));
   }
@@ -763,11 +772,9 @@ int amr_reflux(amr_level_link* l, double dt_coarse) {
   if (!l) return fail(AMR_EINVAL, "null link");
   if (!(dt_coarse > 0) || !std::isfinite(dt_coarse)) return fail(AMR_EINVAL, "dt_coarse must be finite and > 0");
   amr_patch_batch* c = l->c;
-  for (int s = 0; s < 6; ++s) {
-    cudaError_t e = amr::launch_reflux(c->d.dtype, c->U[c->cur], (size_t)c->d.npatch * c->n3, c->d.nfields, c->d.n,
-                                       l->faces[s], l->nfaces[s], l->fblk_c, l->fblk_f, dt_coarse / c->d.dx, c->stream);
-    if (e != cudaSuccess) return fail(AMR_ECUDA, "reflux kernel launch: %s", cudaGetErrorString(e));
-  }
+  cudaError_t e = amr::launch_reflux(c->d.dtype, c->U[c->cur], (size_t)c->d.npatch * c->n3, c->d.nfields, c->d.n, l->faces,
+                                     l->nfaces, l->fblk_c, l->fblk_f, dt_coarse / c->d.dx, c->stream);
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "reflux kernel launch: %s", cudaGetErrorString(e));
   c->smax_valid = false;
   return AMR_OK;
 }
