@@ -61,6 +61,7 @@ cudaError_t launch_scatter_interior(int dtype, const void* staged, int with_ghos
 cudaError_t launch_fill_nan(int dtype, void* ptr, size_t count, cudaStream_t s);
 
 // two-level kernels (aux_kernels.cu); table formats are documented at the kernels
+// dst: [nparents][8] child halo indices or -1, c7: [nparents][7] (formats at the kernel)
 cudaError_t launch_prolong(int dtype, void* halo, size_t fs_halo, int nf, const long long* dst, const long long* c7,
                            int ncells, const void* Ucold, const void* Ucnew, size_t fs_c, double theta,
                            cudaStream_t s);

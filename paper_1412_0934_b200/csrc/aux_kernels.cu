@@ -119,22 +119,22 @@ template <class T> __device__ __forceinline__ T minmod2(T a, T b) {
   return (lo > T(0) ? lo : T(0)) + (hi < T(0) ? hi : T(0));
 }
 
-// dst[e]: flat index into one field of the halo buffer (bit 62..60 = parity x,y,z of the fine cell
-// inside its coarse cell).  c7[e][7]: flat coarse interior indices: centre, x-, x+, y-, y+, z-, z+.
+// One thread per (fine patch, parent cell) entry e.  c7[e][7]: flat coarse interior indices: centre, x-, x+, y-,
+// y+, z-, z+.  dst[e][8]: flat index into one field of the halo buffer of child c = (pz, py, px) parity bits, or
+// -1 if that child is not a coarse-fine halo cell of the patch.  The slopes are computed once per parent.
 template <class T>
-__global__ void __launch_bounds__(256) prolong_kernel(T* __restrict__ halo, size_t fs_halo, int nf,
+__global__ void __launch_bounds__(128) prolong_kernel(T* __restrict__ halo, size_t fs_halo, int nf,
                                                       const long long* __restrict__ dst,
-                                                      const long long* __restrict__ c7, int ncells,
+                                                      const long long* __restrict__ c7, int nparents,
                                                       const T* __restrict__ Uold, const T* __restrict__ Unew,
                                                       size_t fs_c, T theta) {
   const int e = blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= ncells) return;
-  const long long dcode = dst[e];
-  const size_t d = (size_t)(dcode & ((1LL << 60) - 1));
-  const int par = (int)(dcode >> 60) & 7;
-  long long s[7];
+  if (e >= nparents) return;
+  long long s[7], d[8];
 #pragma unroll
   for (int k = 0; k < 7; ++k) s[k] = c7[(size_t)e * 7 + k];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) d[k] = dst[(size_t)e * 8 + k];
   const T w0 = T(1) - theta;
   for (int q = 0; q < nf; ++q) {
     const T* a = Uold + (size_t)q * fs_c;
@@ -147,13 +147,18 @@ __global__ void __launch_bounds__(256) prolong_kernel(T* __restrict__ halo, size
 #pragma unroll
       for (int k = 0; k < 7; ++k) st[k] = w0 * a[s[k]] + theta * b[s[k]];
     }
-    T val = st[0];
+    T sl[3];
 #pragma unroll
-    for (int dd = 0; dd < 3; ++dd) {
-      const T sl = minmod2<T>(st[0] - st[1 + 2 * dd], st[2 + 2 * dd] - st[0]);
-      val += (((par >> dd) & 1) ? T(0.25) : T(-0.25)) * sl;
+    for (int dd = 0; dd < 3; ++dd) sl[dd] = minmod2<T>(st[0] - st[1 + 2 * dd], st[2 + 2 * dd] - st[0]);
+    T* out = halo + (size_t)q * fs_halo;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      if (d[c] < 0) continue;
+      T val = st[0];
+#pragma unroll
+      for (int dd = 0; dd < 3; ++dd) val += (((c >> dd) & 1) ? T(0.25) : T(-0.25)) * sl[dd];
+      out[d[c]] = val;
     }
-    halo[(size_t)q * fs_halo + d] = val;
   }
 }
 
@@ -374,12 +379,12 @@ cudaError_t launch_prolong(int dtype, void* halo, size_t fs_halo, int nf, const 
                            int ncells, const void* Ucold, const void* Ucnew, size_t fs_c, double theta,
                            cudaStream_t s) {
   if (ncells == 0) return cudaSuccess;
-  const unsigned grid = (unsigned)((ncells + 255) / 256);
+  const unsigned grid = (unsigned)((ncells + 127) / 128);
   if (dtype == 0)
-    prolong_kernel<float><<<grid, 256, 0, s>>>((float*)halo, fs_halo, nf, dst, c7, ncells, (const float*)Ucold,
+    prolong_kernel<float><<<grid, 128, 0, s>>>((float*)halo, fs_halo, nf, dst, c7, ncells, (const float*)Ucold,
                                               (const float*)Ucnew, fs_c, (float)theta);
   else
-    prolong_kernel<double><<<grid, 256, 0, s>>>((double*)halo, fs_halo, nf, dst, c7, ncells, (const double*)Ucold,
+    prolong_kernel<double><<<grid, 128, 0, s>>>((double*)halo, fs_halo, nf, dst, c7, ncells, (const double*)Ucold,
                                                (const double*)Ucnew, fs_c, theta);
   return cudaGetLastError();
 }

@@ -171,9 +171,14 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
     *out = (long long)pc * (long long)n3 + ((long long)(C[2] - oc[2]) * n + (C[1] - oc[1])) * n + (C[0] - oc[0]);
     return true;
   };
-  // O8 list: fine halo cells in regions no sibling covers
+  // O8 list: fine halo cells in regions no sibling covers, grouped by parent cell: one entry per (patch, parent)
+  // = 7 stencil indices (pro_c7) + the halo index of each of its 8 children that is needed, else -1 (pro_dst)
+  const int hp = n / 2 + 4;   // parent cells along one side of a patch's halo box (fine -g..n+g-1, g <= 4)
+  if (g > 4) return fail(AMR_EINVAL, "nghost > 4 is not supported by the prolongation tables");
+  std::vector<int> slot((size_t)hp * hp * hp);
   for (int p = 0; p < f->d.npatch; ++p) {
     const int* o = &f->origin[3 * p];
+    std::fill(slot.begin(), slot.end(), -1);
     for (int k = -g; k < n + g; ++k)
       for (int j = -g; j < n + g; ++j)
         for (int i = -g; i < n + g; ++i) {
@@ -197,8 +202,15 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
           }
           if (!ok) return fail(AMR_EINVAL, "fine patch %d has a halo cell with no coarse parent", p);
           const long long cell = (long long)p * (long long)M3 + ((long long)(k + g) * M + (j + g)) * M + (i + g);
-          H.pro_dst.push_back(cell | (par << 60));
-          for (int q = 0; q < 7; ++q) H.pro_c7.push_back(s7[q]);
+          // patch origins are even: the parent's position in the patch's halo box is floor(offset / 2) + 2
+          const int li = ((i + 4) >> 1), lj = ((j + 4) >> 1), lk = ((k + 4) >> 1);
+          int& sl = slot[((size_t)lk * hp + lj) * hp + li];
+          if (sl < 0) {
+            sl = (int)(H.pro_dst.size() / 8);
+            for (int q = 0; q < 8; ++q) H.pro_dst.push_back(-1);
+            for (int q = 0; q < 7; ++q) H.pro_c7.push_back(s7[q]);
+          }
+          H.pro_dst[(size_t)sl * 8 + (size_t)par] = cell;
         }
   }
   // O9(6) list: entry e = (p, ck, cj, ci)
@@ -691,7 +703,7 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   l->pro_dst = (long long*)(l->ws + L.pro_dst);
   l->pro_c7 = (long long*)(l->ws + L.pro_c7);
   l->res_dst = (long long*)(l->ws + L.res_dst);
-  l->npro = (int)H.pro_dst.size();
+  l->npro = (int)(H.pro_dst.size() / 8);
   l->nres = (int)H.res_dst.size();
   l->faces = (long long*)(l->ws + L.faces);
   l->nfaces = (int)(H.faces_all.size() / 4);
