@@ -191,21 +191,21 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
             par |= (long long)wrapi(gi[a], 2) << a;
             gi[a] = wrapi(gi[a], domf[a]);
           }
-          const int C[3] = {gi[0] / 2, gi[1] / 2, gi[2] / 2};
-          long long s7[7];
-          bool ok = coarse_flat(C[0], C[1], C[2], &s7[0]);
-          for (int a = 0; a < 3 && ok; ++a) {
-            int Cm[3] = {C[0], C[1], C[2]}, Cp[3] = {C[0], C[1], C[2]};
-            Cm[a] -= 1;
-            Cp[a] += 1;
-            ok = coarse_flat(Cm[0], Cm[1], Cm[2], &s7[1 + 2 * a]) && coarse_flat(Cp[0], Cp[1], Cp[2], &s7[2 + 2 * a]);
-          }
-          if (!ok) return fail(AMR_EINVAL, "fine patch %d has a halo cell with no coarse parent", p);
           const long long cell = (long long)p * (long long)M3 + ((long long)(k + g) * M + (j + g)) * M + (i + g);
           // patch origins are even: the parent's position in the patch's halo box is floor(offset / 2) + 2
           const int li = ((i + 4) >> 1), lj = ((j + 4) >> 1), lk = ((k + 4) >> 1);
           int& sl = slot[((size_t)lk * hp + lj) * hp + li];
-          if (sl < 0) {
+          if (sl < 0) {   // first child of this parent: resolve the 7-point stencil in the coarse batch
+            const int C[3] = {gi[0] / 2, gi[1] / 2, gi[2] / 2};
+            long long s7[7];
+            bool ok = coarse_flat(C[0], C[1], C[2], &s7[0]);
+            for (int a = 0; a < 3 && ok; ++a) {
+              int Cm[3] = {C[0], C[1], C[2]}, Cp[3] = {C[0], C[1], C[2]};
+              Cm[a] -= 1;
+              Cp[a] += 1;
+              ok = coarse_flat(Cm[0], Cm[1], Cm[2], &s7[1 + 2 * a]) && coarse_flat(Cp[0], Cp[1], Cp[2], &s7[2 + 2 * a]);
+            }
+            if (!ok) return fail(AMR_EINVAL, "fine patch %d has a halo cell with no coarse parent", p);
             sl = (int)(H.pro_dst.size() / 8);
             for (int q = 0; q < 8; ++q) H.pro_dst.push_back(-1);
             for (int q = 0; q < 7; ++q) H.pro_c7.push_back(s7[q]);

@@ -115,3 +115,20 @@ def test_link_order_is_enforced(H, hierarchies):
         l01.close()                        # the finer link records into l01's blocks
     l12.close()
     l01.close()
+
+
+def test_four_level_step_fp64(oracle, H):
+    """L = 4: two middle levels (each the fine side of one link and the coarse side of the next), 15 level steps
+    per root step."""
+    wl = wk.config_hierarchy(True, 4, 256, n=16, thresholds=(1.8, 2.8, 4.0))
+    assert all(lv.npatch >= 4 for lv in wl.levels), wl.note
+    ref = oracle.hierarchy_step(wl)
+    got = H.gpu_hierarchy_step(wl)
+    assert abs(got["dt0"] - ref["dt0"]) <= 1e-13 * ref["dt0"]
+    ps = ref["smax"] * max(np.abs(ref["U"][0][5:8]).max(), 1e-300)
+    for l in range(4):
+        e = H.rel_err(got["U"][l], ref["U"][l], psi_scale=ps)
+        assert e.max() <= 8 * TOL64_STEP, (l, e)
+    g = wl.levels[0].g
+    tot = oracle.hierarchy_totals([oracle.ghosted(u, g) for u in got["U"]], wl.levels)
+    assert (np.abs(tot - ref["totals_before"])[:8] / _absn(wl.levels[0])[:8]).max() <= 1e-13

@@ -201,3 +201,15 @@ def test_schedule_of_a_three_level_root_step(oracle, small_hierarchy, monkeypatc
             + [("prolong", 1, 0.5), ("step", 1, dt0 / 2)] + fine_pair
             + [("restrict", 0, None), ("reflux", 0, dt0)])
     assert log == want
+
+
+def test_four_levels_two_middle_levels(oracle):
+    """L = 4 (two levels that are fine side and coarse side at once): 1 + 2 + 4 + 8 level steps, composite
+    totals conserved to 1e-13."""
+    wl = wk.config_hierarchy(True, 4, 128, n=8, thresholds=(1.5, 2.5, 3.5))
+    assert [lv.npatch for lv in wl.levels][0] == 8 and all(lv.npatch >= 4 for lv in wl.levels), wl.note
+    r = oracle.hierarchy_step(wl)
+    assert r["nsteps"] == [1, 2, 4, 8]
+    l0 = wl.levels[0]
+    absn = np.array([np.abs(l0.U[f]).sum() * l0.dx ** 3 for f in range(9)])
+    assert (np.abs(r["totals_after"] - r["totals_before"])[:8] / absn[:8]).max() < 1e-13
