@@ -684,41 +684,45 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
       //      convert plane kk+2 when it has landed (these warps have the slack to wait for it) ---------
       issue_plane(kk + 2, Wm);
       cp_commit();
-      if (mid && right) {
-        F2 wl[NF], WL[NF], WR[NF], Fr[NF];
-        {
+      if (mid && (right || top)) {
+        // ONE solver instance for the tile's last x faces (right ring: lo half real) and last y faces (top ring):
+        // the kernel is bound by instruction fetch (profiles/r1c), these warps have the slack for the few moves
+        // that bring the two roles' operands into the same registers
+        F2 WL[NF], WR[NF], Fr[NF];
+        if (right) {
           float xl[NF];
           lds_n<NF, XVW>(xslot, xl);
+          F2 wl[NF];
 #pragma unroll
           for (int q = 0; q < NF; ++q) wl[q] = F2(xl[q], xl[q]);
+          rot_in<NF, 0>(wl, WL);
+          rot_in<NF, 0>(wm, WR);
+        } else {
+          F2 wl[NF];
+          lds_pairs<NF>(yslot, wl);
+          rot_in<NF, 1>(wl, WL);
+          rot_in<NF, 1>(wm, WR);
         }
-        rot_in<NF, 0>(wl, WL);
-        rot_in<NF, 0>(wm, WR);
-        riemann2<NF, RS>(WL, WR, RC, Fr, B2(true, false), s_cnt);
-        rot_out<NF, 0>(Fr, wm);
-        {
+        riemann2<NF, RS>(WL, WR, RC, Fr, B2(true, !right), s_cnt);
+        if (right) {
+          rot_out<NF, 0>(Fr, wm);
           float o[NF];
 #pragma unroll
           for (int q = 0; q < NF; ++q) o[q] = wm[q].v.x;
           sts_n<NF, XVW>(xslot, o);
-        }
-        if (X2_UNLIKELY(blk >= 0) && x0 + TX == n) {  // the patch's last x face (a7)
-          float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + n);
+          if (X2_UNLIKELY(blk >= 0) && x0 + TX == n) {  // the patch's last x face (a7)
+            float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + n);
 #pragma unroll
-          for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, wm[q].v.x);
-        }
-      } else if (mid && top) {
-        F2 wl[NF], WL[NF], WR[NF], Fr[NF];
-        lds_pairs<NF>(yslot, wl);
-        rot_in<NF, 1>(wl, WL);
-        rot_in<NF, 1>(wm, WR);
-        riemann2<NF, RS>(WL, WR, RC, Fr, B2(true), s_cnt);
-        rot_out<NF, 1>(Fr, wm);
-        sts_pairs<NF>(yslot, wm);
-        if (X2_UNLIKELY(blk >= 0) && y0 + TY == n) {
-          float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + n) * n + (x0 + 2 * (px - 1)));
+            for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, wm[q].v.x);
+          }
+        } else {
+          rot_out<NF, 1>(Fr, wm);
+          sts_pairs<NF>(yslot, wm);
+          if (X2_UNLIKELY(blk >= 0) && y0 + TY == n) {
+            float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + n) * n + (x0 + 2 * (px - 1)));
 #pragma unroll
-          for (int q = 0; q < NF; ++q) { atomicAdd(dstF + (size_t)q * fsz, wm[q].v.x); atomicAdd(dstF + (size_t)q * fsz + 1, wm[q].v.y); }
+            for (int q = 0; q < NF; ++q) { atomicAdd(dstF + (size_t)q * fsz, wm[q].v.x); atomicAdd(dstF + (size_t)q * fsz + 1, wm[q].v.y); }
+          }
         }
       }
       cp_wait<0>();
