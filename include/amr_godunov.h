@@ -166,15 +166,16 @@ int amr_hierarchy_step(amr_patch_batch* const* levels, amr_level_link* const* li
  * readings in DESIGN.md 12) ---------------------------------------------------------------------------
  * amr_flag_blocks: host_flags[p*8 + bz*4 + by*2 + bx] (host, caller-owned, npatch*8 bytes) = 1 if the maximum of
  * field `field` of the current state over the aligned (n/2)^3 block (bx, by, bz) of patch p exceeds
- * `threshold` (strictly), else 0.  One kernel + one npatch*8-byte read; synchronises the batch's stream.
+ * `threshold` (strictly), else 0.  One kernel + one npatch*8-byte read through a stream-ordered temporary of
+ * that size (cudaMallocAsync); synchronises the batch's stream.
  * Which flagged blocks become patches of the next level is the caller's policy; the caller then creates the
  * new fine batch (amr_patch_batch_create with the new origins) and calls
  * amr_regrid_fill(new_fine, old_fine, coarse, ws, bytes): the current state of new_fine becomes, patch by
  * patch, a copy of old_fine's patch with the same origin if there is one (old_fine may be NULL), else the
  * conservative limited linear interpolation of O8 from coarse's current state (the 8 children of a coarse cell
  * average to it: composite totals are unchanged).  dev_ws: device workspace of amr_regrid_bytes(...) bytes,
- * borrowed for the call only.  new_fine must not be linked yet; link it afterwards (after destroying the old
- * link).  AMR_EINVAL if a new patch without an old twin is not properly nested in coarse. */
+ * borrowed for the call only.  new_fine must not be linked yet (AMR_ESTATE); link it afterwards (after
+ * destroying the old link).  AMR_EINVAL if a new patch without an old twin is not properly nested in coarse. */
 int amr_flag_blocks(amr_patch_batch* b, int field, double threshold, unsigned char* host_flags);
 size_t amr_regrid_bytes(const amr_patch_batch* new_fine, const amr_patch_batch* old_fine, const amr_patch_batch* coarse);
 int amr_regrid_fill(amr_patch_batch* new_fine, const amr_patch_batch* old_fine, const amr_patch_batch* coarse,

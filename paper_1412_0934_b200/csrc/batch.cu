@@ -974,6 +974,7 @@ int amr_regrid_fill(amr_patch_batch* new_fine, const amr_patch_batch* old_fine, 
                     size_t bytes) {
   int rc = check_regrid_args(new_fine, old_fine, coarse);
   if (rc != AMR_OK) return rc;
+  if (new_fine->link_up || new_fine->link_down) return fail(AMR_ESTATE, "fill the new batch before linking it");
   if (old_fine && old_fine->stream != new_fine->stream) return fail(AMR_EINVAL, "old and new fine batches must share the stream");
   if (!dev_ws || (uintptr_t)dev_ws % ALIGN) return fail(AMR_EINVAL, "workspace must be a %zu-byte aligned device pointer", ALIGN);
   RegridHost H;
