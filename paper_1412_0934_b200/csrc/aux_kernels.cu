@@ -271,7 +271,7 @@ __global__ void __launch_bounds__(256) zero_faces_kernel(T* __restrict__ Fc, int
 //                 flat offset of the coarse flux inside field 0 of the coarse flux-block array,
 //                 flat offset of the first of the 4 fine fluxes inside field 0 of the fine flux-block array,
 //                 code: bit0 = sign (1: s_f = -1), bits 1..2 = d }.
-// blk_stride_*: elements between fields inside one (block, d) slab = n^2 (n+1).
+// elements between fields inside one (block, d) slab = 3 n^2 (the face planes 0, n/2, n).
 template <class T>
 __global__ void __launch_bounds__(256) reflux_kernel(T* __restrict__ Uc, size_t fs_c, int nf, int n,
                                                      const long long* __restrict__ faces, int nfaces,
@@ -283,21 +283,16 @@ __global__ void __launch_bounds__(256) reflux_kernel(T* __restrict__ Uc, size_t 
   const long long cell_ll = faces[(size_t)e * 4 + 0];
   if (e > 0 && faces[(size_t)(e - 1) * 4 + 0] == cell_ll) return;
   const size_t cell = (size_t)cell_ll;
-  const size_t fsz = (size_t)n * n * (n + 1);
+  const size_t fsz = (size_t)3 * n * n;
   for (; e < nfaces && faces[(size_t)e * 4 + 0] == cell_ll; ++e) {
     const size_t oc = (size_t)faces[(size_t)e * 4 + 1];
     const size_t of = (size_t)faces[(size_t)e * 4 + 2];
     const int code = (int)faces[(size_t)e * 4 + 3];
     const T sf = (code & 1) ? T(-1) : T(1);
     const int d = (code >> 1) & 3;
-    // strides of the two transverse directions t1 = (d+1)%3 (a), t2 = (d+2)%3 (b) inside a d-slab
-    // slab extents: (z, y, x) with n+1 along d
-    size_t sx = 1, sy, sz;
-    if (d == 0) { sy = n + 1; sz = (size_t)n * (n + 1); }
-    else if (d == 1) { sy = n; sz = (size_t)n * (n + 1); }
-    else { sy = n; sz = (size_t)n * n; }
-    const size_t str3[3] = {sx, sy, sz};
-    const size_t sa = str3[(d + 1) % 3], sb = str3[(d + 2) % 3];
+    // strides of the two transverse directions t1 = (d+1)%3 (a), t2 = (d+2)%3 (b) inside a face plane, whose
+    // in-plane layout has the lower remaining axis fastest: d = 0: (z, y), d = 1: (z, x), d = 2: (y, x)
+    const size_t sa = (d == 1) ? (size_t)n : 1, sb = (d == 1) ? 1 : (size_t)n;
     for (int q = 0; q < nf; ++q) {
       const T Fcoarse = Fc[oc + (size_t)q * fsz];
       const T* f = Ff + of + (size_t)q * fsz;
@@ -416,7 +411,7 @@ cudaError_t launch_reflux(int dtype, void* Uc, size_t fs_c, int nf, int n, const
 cudaError_t launch_zero_faces(int dtype, void* Fc, int nf, int n, const long long* faces, int nfaces, cudaStream_t s) {
   if (nfaces == 0) return cudaSuccess;
   const unsigned grid = (unsigned)((nfaces + 255) / 256);
-  const size_t fsz = (size_t)n * n * (n + 1);
+  const size_t fsz = (size_t)3 * n * n;
   if (dtype == 0)
     zero_faces_kernel<float><<<grid, 256, 0, s>>>((float*)Fc, nf, fsz, faces, nfaces);
   else

@@ -227,12 +227,15 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
   }
   // O9(7) list, one per (d, side) so that no coarse cell appears twice in a launch
   H.fblk_of_c.assign(c->d.npatch, -1);
-  const long long fsz = (long long)n * n * (n + 1);
+  // flux blocks: [block][direction][field][3 face planes: index 0, n/2, n along the normal][n^2 in-plane, the
+  // lower remaining axis fastest] - all a link can read (fine patches sit on aligned (n/2)^3 parent blocks)
+  const long long fsz = 3LL * n * n;
   const int NF = f->d.nfields;
-  auto slab_off = [&](int d, const int l[3]) -> long long {  // l = (x,y,z) with face index along d
-    if (d == 0) return ((long long)l[2] * n + l[1]) * (n + 1) + l[0];
-    if (d == 1) return ((long long)l[2] * (n + 1) + l[1]) * n + l[0];
-    return ((long long)l[2] * n + l[1]) * n + l[0];
+  auto slab_off = [&](int d, const int l[3]) -> long long {  // l = (x,y,z) with the face index along d
+    const long long s = l[d] == 0 ? 0 : (l[d] == n ? 2 : (l[d] == n / 2 ? 1 : -1));
+    if (s < 0) return -1;
+    const long long idx = d == 0 ? (long long)l[2] * n + l[1] : (d == 1 ? (long long)l[2] * n + l[0] : (long long)l[1] * n + l[0]);
+    return s * n * n + idx;
   };
   for (int p = 0; p < f->d.npatch; ++p) {
     const int* o = &f->origin[3 * p];
@@ -256,6 +259,7 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
             if (H.fblk_of_c[pc] < 0) H.fblk_of_c[pc] = H.identity_c ? pc : H.nblk_c++;
             int lface[3] = {lc[0], lc[1], lc[2]};
             if (!side) lface[d] += 1;  // upper face of the outside cell
+            if (slab_off(d, lface) < 0) return fail(AMR_EINVAL, "fine patch %d is not aligned to an (n/2)^3 block of its parent level", p);
             const long long oc_off = ((long long)H.fblk_of_c[pc] * 3 + d) * NF * fsz + slab_off(d, lface);
             int lf[3];
             lf[d] = side ? n : 0;
@@ -300,7 +304,7 @@ LinkLayout make_link_layout(const amr_patch_batch* c, const amr_patch_batch* f, 
   L.pro_c7 = off; off += up(H.pro_c7.size() * 8 + 8);
   L.res_dst = off; off += up(H.res_dst.size() * 8 + 8);
   L.faces = off; off += up(H.faces_all.size() * 8 + 8);
-  const size_t n = f->d.n, blk = 3 * (size_t)f->d.nfields * n * n * (n + 1) * f->esz;
+  const size_t n = f->d.n, blk = 3 * (size_t)f->d.nfields * 3 * n * n * f->esz;
   L.fblk_c_bytes = H.identity_c ? 0 : (size_t)H.nblk_c * blk;
   L.fblk_f_bytes = (size_t)f->d.npatch * blk;
   L.fblk_c = off; off += up(L.fblk_c_bytes + 8);

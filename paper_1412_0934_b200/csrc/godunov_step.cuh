@@ -576,7 +576,9 @@ __global__ void __maxnreg__(MAXR) godunov_step_kernel(const __grid_constant__ St
   __syncthreads();
 
   const int blk = (P.fblk != nullptr) ? P.fblk_of[p] : -1;  // flux-register block of this patch
-  const size_t fsz = (size_t)n2 * (n + 1);
+  // flux blocks: [block][direction][field][3 face planes: index 0, n/2, n along the normal][n^2 in-plane, the
+  // lower remaining axis fastest]
+  const size_t fsz = (size_t)3 * n2;
 
   for (int t = 0; t <= zc + 1; ++t) {
     const int kk = z0 - 1 + t;               // plane being predicted
@@ -673,7 +675,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_kernel(const __grid_constant__ St
           }
           // only the face planes a link can read (index 0, n/2, n along the normal) are recorded
           if (blk >= 0 && (t <= zc || z0 + zc == n) && (kk == 0 || kk == (n >> 1) || kk == n)) {
-            T* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)kk * n2 + (size_t)((y0 + bj) * n + (x0 + bi)));
+            T* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)((kk) == 0 ? 0 : ((kk) == n ? 2 : 1)) * n2 + (size_t)((y0 + bj) * n + (x0 + bi)));
 #pragma unroll
             for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, fz[q]);
           }
@@ -736,7 +738,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_kernel(const __grid_constant__ St
         rotate_out<T, NF, 0>(Fr, wmx);
         sts_cell<T, NF>(xfp, wmx);
         if (blk >= 0 && (bi < TX || x0 + TX == n) && (x0 + bi == 0 || x0 + bi == (n >> 1) || x0 + bi == n)) {  // record the flux for the reflux
-          T* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + bj)) * (n + 1) + (x0 + bi));
+          T* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)((x0 + bi) == 0 ? 0 : ((x0 + bi) == n ? 2 : 1)) * n2 + (size_t)(kk * n + (y0 + bj)));
 #pragma unroll
           for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, wmx[q]);
         }
@@ -750,7 +752,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_kernel(const __grid_constant__ St
         rotate_out<T, NF, 1>(Fr, wmy);
         sts_cell<T, NF>(yfp, wmy);
         if (blk >= 0 && (bj < TY || y0 + TY == n) && (y0 + bj == 0 || y0 + bj == (n >> 1) || y0 + bj == n)) {
-          T* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + (y0 + bj)) * n + (x0 + bi));
+          T* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)((y0 + bj) == 0 ? 0 : ((y0 + bj) == n ? 2 : 1)) * n2 + (size_t)(kk * n + (x0 + bi)));
 #pragma unroll
           for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, wmy[q]);
         }

@@ -217,7 +217,9 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
   RC.gamma = P.gamma; RC.igm1 = P.igm1; RC.ch2 = P.ch2; RC.half_ch = 0.5 * P.ch; RC.half_ich = P.half_ich;
   RC.eps = P.eps;
   const int blk = (P.fblk != nullptr) ? P.fblk_of[p] : -1;  // flux-register block of this patch
-  const size_t fsz = (size_t)n2 * (n + 1);
+  // flux blocks: [block][direction][field][3 face planes: index 0, n/2, n along the normal][n^2 in-plane, the
+  // lower remaining axis fastest]
+  const size_t fsz = (size_t)3 * n2;
 
   double* Wm = ring;
   double* Wc = ring + SLOT;
@@ -311,7 +313,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
           // flux registers of a coarse-fine link (a7).  Only the face planes a link can read are recorded: index 0,
           // n/2, n along the normal (fine patches sit on aligned (n/2)^3 blocks of the parent level)
           if (X2_UNLIKELY(blk >= 0) && (kk == 0 || kk == (n >> 1) || kk == n)) {
-            double* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)kk * n2 + (size_t)((y0 + pj) * n + (x0 + pc)));
+            double* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)((kk) == 0 ? 0 : ((kk) == n ? 2 : 1)) * n2 + (size_t)((y0 + pj) * n + (x0 + pc)));
 #pragma unroll
             for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, fz[q]);
           }
@@ -376,8 +378,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
             double f[NF];
             if (d) rot_out<NF, 1>(Fr, f); else rot_out<NF, 0>(Fr, f);
             double* dstF = P.fblk + ((size_t)blk * 3 + d) * NF * fsz +
-                           (d ? ((size_t)(kk * (n + 1) + (y0 + pj)) * n + (x0 + pc))
-                              : ((size_t)(kk * n + (y0 + pj)) * (n + 1) + (x0 + pc)));
+                           (size_t)((fidx) == 0 ? 0 : ((fidx) == n ? 2 : 1)) * n2 + (size_t)(kk * n + (d ? x0 + pc : y0 + pj));
 #pragma unroll
             for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, f[q]);
           }
@@ -569,13 +570,13 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
         sts_rec<NF>(rec, Fr);
         if (X2_UNLIKELY(blk >= 0)) {   // the patch's last x / y face (a7)
           if (right && x0 + HX == n) {
-            double* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + n);
+            double* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)2 * n2 + (size_t)(kk * n + (y0 + pj)));
 #pragma unroll
             for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, Fr[q]);
           } else if (top && y0 + TY == n) {
             double fy[NF];
             rot_out<NF, 1>(Fr, fy);
-            double* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + n) * n + (x0 + cx - 2));
+            double* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)2 * n2 + (size_t)(kk * n + (x0 + cx - 2)));
 #pragma unroll
             for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, fy[q]);
           }

@@ -274,7 +274,9 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
   RC.gamma = P.gamma; RC.igm1 = P.igm1; RC.ch2 = P.ch2; RC.half_ch = 0.5f * P.ch; RC.half_ich = P.half_ich;
   RC.eps = P.eps;
   const int blk = (P.fblk != nullptr) ? P.fblk_of[p] : -1;  // flux-register block of this patch
-  const size_t fsz = (size_t)n2 * (n + 1);
+  // flux blocks: [block][direction][field][3 face planes: index 0, n/2, n along the normal][n^2 in-plane, the
+  // lower remaining axis fastest]
+  const size_t fsz = (size_t)3 * n2;
   const F2 ms = F2(-P.dtdx);
 
   float* Wm = ring;
@@ -384,7 +386,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
           // substeps is a result-less atomicAdd (RED): one writer per address and step, so the value is that of
           // a plain +=, without exposing the load latency of a read-modify-write in this latency-bound loop
           if (X2_UNLIKELY(blk >= 0) && (kk == 0 || kk == (n >> 1) || kk == n)) {
-            float* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)kk * n2 + (size_t)((y0 + pj) * n + (x0 + 2 * pc)));
+            float* dstF = P.fblk + ((size_t)blk * 3 + 2) * NF * fsz + ((size_t)((kk) == 0 ? 0 : ((kk) == n ? 2 : 1)) * n2 + (size_t)((y0 + pj) * n + (x0 + 2 * pc)));
 #pragma unroll
             for (int q = 0; q < NF; ++q) { atomicAdd(dstF + (size_t)q * fsz, fz[q].v.x); atomicAdd(dstF + (size_t)q * fsz + 1, fz[q].v.y); }
           }
@@ -468,7 +470,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
           }
           // record the fluxes for the reflux: x faces 0 and n/2 are the even face of a pair
           if (X2_UNLIKELY(blk >= 0) && (x0 + 2 * pc == 0 || x0 + 2 * pc == (n >> 1))) {
-            float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + (x0 + 2 * pc));
+            float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)((x0 + 2 * pc) == 0 ? 0 : ((x0 + 2 * pc) == n ? 2 : 1)) * n2 + (size_t)(kk * n + (y0 + pj)));
 #pragma unroll
             for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, fx[q].v.x);
           }
@@ -488,7 +490,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
             st_block(BY, o, 0.f, 0.f);  // private copy for phase 3 (same reason)
           }
           if (X2_UNLIKELY(blk >= 0) && (y0 + pj == 0 || y0 + pj == (n >> 1))) {
-            float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + (y0 + pj)) * n + (x0 + 2 * pc));
+            float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)((y0 + pj) == 0 ? 0 : ((y0 + pj) == n ? 2 : 1)) * n2 + (size_t)(kk * n + (x0 + 2 * pc)));
 #pragma unroll
             for (int q = 0; q < NF; ++q) { atomicAdd(dstF + (size_t)q * fsz, fy[q].v.x); atomicAdd(dstF + (size_t)q * fsz + 1, fy[q].v.y); }
           }
@@ -711,7 +713,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
           for (int q = 0; q < NF; ++q) o[q] = wm[q].v.x;
           sts_n<NF, XVW>(xslot, o);
           if (X2_UNLIKELY(blk >= 0) && x0 + TX == n) {  // the patch's last x face (a7)
-            float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)(kk * n + (y0 + pj)) * (n + 1) + n);
+            float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)2 * n2 + (size_t)(kk * n + (y0 + pj)));
 #pragma unroll
             for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, wm[q].v.x);
           }
@@ -719,7 +721,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
           rot_out<NF, 1>(Fr, wm);
           sts_pairs<NF>(yslot, wm);
           if (X2_UNLIKELY(blk >= 0) && y0 + TY == n) {
-            float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)(kk * (n + 1) + n) * n + (x0 + 2 * (px - 1)));
+            float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)2 * n2 + (size_t)(kk * n + (x0 + 2 * (px - 1))));
 #pragma unroll
             for (int q = 0; q < NF; ++q) { atomicAdd(dstF + (size_t)q * fsz, wm[q].v.x); atomicAdd(dstF + (size_t)q * fsz + 1, wm[q].v.y); }
           }

@@ -132,3 +132,30 @@ def test_four_level_step_fp64(oracle, H):
     g = wl.levels[0].g
     tot = oracle.hierarchy_totals([oracle.ghosted(u, g) for u in got["U"]], wl.levels)
     assert (np.abs(tot - ref["totals_before"])[:8] / _absn(wl.levels[0])[:8]).max() <= 1e-13
+
+
+@pytest.mark.parametrize("np_dtype", [np.float64, np.float32])
+def test_three_level_step_patch_size_8(oracle, H, np_dtype):
+    """8^3 patches run the first kernel (godunov_step.cuh, 8x8 tiles): its flux capture in all three link roles."""
+    import copy
+    f32 = np_dtype == np.float32
+    wl = copy.deepcopy(wk.config_hierarchy(True, 3, 128, n=8, thresholds=(2.5, 3.5)))
+    if f32:
+        for lv in wl.levels:
+            lv.U = lv.U.astype(np.float32).astype(np.float64)
+    ref = oracle.hierarchy_step(wl, eps=oracle.default_eps(np_dtype))
+    got = H.gpu_hierarchy_step(wl, np_dtype=np_dtype)
+    ps = ref["smax"] * max(np.abs(ref["U"][0][5:8]).max(), 1e-300)
+    for l in range(3):
+        for grp in H.field_groups(9):
+            den = np.abs(ref["U"][l][grp]).max()
+            if grp == [8]:
+                den = max(den, ps)
+            e = np.abs(got["U"][l][grp].astype(np.float64) - ref["U"][l][grp]).max(axis=0) / den
+            if f32:
+                assert np.quantile(e, 0.9999) <= 4 * TOL32 and int((e > 8 * TOL32).sum()) <= 8, (l, grp, e.max())
+            else:
+                assert e.max() <= 4 * TOL64_STEP, (l, grp, e.max())
+    g = wl.levels[0].g
+    tot = oracle.hierarchy_totals([oracle.ghosted(u.astype(np.float64), g) for u in got["U"]], wl.levels)
+    assert (np.abs(tot - ref["totals_before"])[:8] / _absn(wl.levels[0])[:8]).max() <= (4e-6 if f32 else 1e-13)
