@@ -21,7 +21,7 @@ struct StepParams {
   T* Uout;             // device, [NF][np][n^3]
   const T* halo;       // device, [NF][np][(n+2g)^3] or nullptr (level 0)
   const int* nbr;      // device, [np][27]
-  T* fblk;             // device flux blocks [nblk][3][NF][n^2 (n+1)] or nullptr
+  T* fblk;             // device flux blocks [nblk][3][NF][3 face planes 0, n/2, n][n^2] or nullptr
   const int* fblk_of;  // device, [np] block index or -1 (nullptr if fblk is)
   unsigned long long* counters;  // device [4]
   void* smax;          // device, one T-sized slot (bit pattern ordered as unsigned), pre-zeroed
