@@ -155,6 +155,11 @@ int amr_reflux(amr_level_link* l, double dt_coarse);
  * (hydro or MHD, with c_h = ch on every level); if level l+1 exists, twice { amr_prolong_ghosts(links[l],
  * theta = 0, 1/2); advance(l+1, dt/2) }; amr_restrict(links[l]); amr_reflux(links[l], dt) unless do_reflux
  * is 0.  Level l takes 2^l steps of dt0 / 2^l.  Only kernel launches are enqueued (no synchronisation).
+ * Scheduling: the theta = 0 prolongation needs only the coarse level's state BEFORE its step, so it and the fine
+ * level's first substep are enqueued on a per-level internal stream before the coarse step goes to the caller's
+ * stream (levels overlap on the device; every cross-level dependency is an event; the caller's stream continues
+ * after all levels when the call returns).  All levels must have been created on one stream (AMR_EINVAL).
+ * AMR_HIERARCHY_OVERLAP=0 in the environment keeps every level on the caller's stream (same results).
  * Errors: AMR_EINVAL for a null pointer, nlevels outside 1..30, links that do not tie consecutive entries of
  * levels, dt0 not finite and > 0; otherwise the first error of the calls listed above. */
 int amr_hierarchy_cfl_dt(amr_patch_batch* const* levels, int nlevels, double gamma, double cfl, int mhd,

@@ -12,6 +12,7 @@
 #include <new>
 #include <string>
 #include <vector>
+#include <cstdlib>
 #include <atomic>
 #include <utility>
 
@@ -817,24 +818,78 @@ struct CycleArgs {
   amr_level_link* const* links;
   int nlevels, mhd, limiter, riemann, do_reflux;
   double gamma, ch, alpha;
+  cudaEvent_t* ev;   // one event per level (nullptr: every level on the caller's stream, no overlap)
 };
 
-// advance(l, dt) of oracle.api.hierarchy_step, call for call
-int advance_level(const CycleArgs& A, int l, double dt) {
-  const bool has_child = l + 1 < A.nlevels;
-  int rc;
-  if (has_child && (rc = amr_flux_clear(A.links[l])) != AMR_OK) return rc;
-  rc = A.mhd ? amr_mhd_step(A.levels[l], dt, A.gamma, A.limiter, A.riemann, A.ch, A.alpha)
-             : amr_hydro_step(A.levels[l], dt, A.gamma, A.limiter, A.riemann);
-  if (rc != AMR_OK || !has_child) return rc;
-  for (int sub = 0; sub < 2; ++sub) {
-    if ((rc = amr_prolong_ghosts(A.links[l], 0.5 * sub)) != AMR_OK) return rc;
-    if ((rc = advance_level(A, l + 1, 0.5 * dt)) != AMR_OK) return rc;
-  }
-  if ((rc = amr_restrict(A.links[l])) != AMR_OK) return rc;
-  if (A.do_reflux && (rc = amr_reflux(A.links[l], dt)) != AMR_OK) return rc;
+// `waiter` continues after everything enqueued on `producer` so far (no-op for one stream)
+int stream_after(cudaStream_t waiter, cudaStream_t producer, cudaEvent_t ev) {
+  if (waiter == producer) return AMR_OK;
+  CUDA_TRY(cudaEventRecord(ev, producer));
+  CUDA_TRY(cudaStreamWaitEvent(waiter, ev, 0));
   return AMR_OK;
 }
+
+// O8 at theta = 0 from the coarse level's CURRENT state, i.e. before its step is enqueued (the same values
+// amr_prolong_ghosts(l, 0) reads after it): lets the fine level's first substep run beside the coarse step
+int prolong_from_current(amr_level_link* l) {
+  amr_patch_batch *c = l->c, *f = l->f;
+  cudaError_t e = amr::launch_prolong(f->d.dtype, f->halo, (size_t)f->d.npatch * f->M3, f->d.nfields, l->pro_dst, l->pro_c7,
+                                      l->npro, c->U[c->cur], c->U[c->cur], (size_t)c->d.npatch * c->n3, 0.0, f->stream);
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "prolong kernel launch: %s", cudaGetErrorString(e));
+  f->halo_valid = true;
+  return AMR_OK;
+}
+
+// advance(l, dt) of oracle.api.hierarchy_step.  Same operators on the same data; the only freedom taken is
+// WHEN they are enqueued: the theta = 0 prolongation needs the coarse level's old state only, so it and the
+// fine level's first substep (and, recursively, its children's) go to the fine level's stream before the coarse
+// step goes to the coarse level's - a level launch of 0.5-3 waves leaves SMs idle that the other levels' CTAs
+// fill (profiles/r1g).  Everything that crosses levels is ordered by events.
+int advance_level(const CycleArgs& A, int l, double dt) {
+  const bool has_child = l + 1 < A.nlevels;
+  amr_patch_batch* b = A.levels[l];
+  int rc;
+  if (has_child) {
+    amr_level_link* lk = A.links[l];
+    // the fine stream first catches up with this level's: its current state is complete, and the previous
+    // reflux of this link (which read the fine flux blocks on this level's stream) is over before they are cleared
+    if (A.ev && (rc = stream_after(lk->f->stream, b->stream, A.ev[l])) != AMR_OK) return rc;
+    if ((rc = amr_flux_clear(lk)) != AMR_OK) return rc;
+    if ((rc = prolong_from_current(lk)) != AMR_OK) return rc;
+  }
+  rc = A.mhd ? amr_mhd_step(b, dt, A.gamma, A.limiter, A.riemann, A.ch, A.alpha)
+             : amr_hydro_step(b, dt, A.gamma, A.limiter, A.riemann);
+  if (rc != AMR_OK || !has_child) return rc;
+  amr_level_link* lk = A.links[l];
+  if ((rc = advance_level(A, l + 1, 0.5 * dt)) != AMR_OK) return rc;
+  if (A.ev && (rc = stream_after(lk->f->stream, b->stream, A.ev[l])) != AMR_OK) return rc;   // the coarse step is done
+  if ((rc = amr_prolong_ghosts(lk, 0.5)) != AMR_OK) return rc;
+  if ((rc = advance_level(A, l + 1, 0.5 * dt)) != AMR_OK) return rc;
+  if (A.ev && (rc = stream_after(b->stream, lk->f->stream, A.ev[l])) != AMR_OK) return rc;   // the fine level caught up
+  if ((rc = amr_restrict(lk)) != AMR_OK) return rc;
+  if (A.do_reflux && (rc = amr_reflux(lk, dt)) != AMR_OK) return rc;
+  return AMR_OK;
+}
+
+// per-level streams and events of amr_hierarchy_step, created on first use and kept for the life of the thread
+struct LevelStreams {
+  std::vector<cudaStream_t> s;
+  std::vector<cudaEvent_t> ev;
+  cudaEvent_t fork = nullptr;
+  int ensure(int n) {
+    if (!fork) CUDA_TRY(cudaEventCreateWithFlags(&fork, cudaEventDisableTiming));
+    while ((int)s.size() < n) {
+      cudaStream_t st;
+      cudaEvent_t e;
+      CUDA_TRY(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+      CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+      s.push_back(st);
+      ev.push_back(e);
+    }
+    return AMR_OK;
+  }
+};
+thread_local LevelStreams g_level_streams;
 
 }  // namespace
 
@@ -862,8 +917,31 @@ int amr_hierarchy_step(amr_patch_batch* const* levels, amr_level_link* const* li
   int rc = check_hierarchy(levels, links, nlevels);
   if (rc != AMR_OK) return rc;
   if (!(dt0 > 0) || !std::isfinite(dt0)) return fail(AMR_EINVAL, "dt0 must be finite and > 0");
-  CycleArgs A{levels, links, nlevels, mhd, limiter, riemann, do_reflux, gamma, ch, alpha};
-  return advance_level(A, 0, dt0);
+  CycleArgs A{levels, links, nlevels, mhd, limiter, riemann, do_reflux, gamma, ch, alpha, nullptr};
+  const char* env = std::getenv("AMR_HIERARCHY_OVERLAP");
+  const bool overlap = nlevels > 1 && !(env && env[0] == '0');
+  if (!overlap) return advance_level(A, 0, dt0);
+  // level l > 0 runs on its own stream for the duration of this call (level 0 stays on the caller's)
+  LevelStreams& LS = g_level_streams;
+  if ((rc = LS.ensure(nlevels)) != AMR_OK) return rc;
+  cudaStream_t caller = levels[0]->stream;
+  for (int l = 1; l < nlevels; ++l)
+    if (levels[l]->stream != caller) return fail(AMR_EINVAL, "all levels must have been created on one stream");
+  CUDA_TRY(cudaEventRecord(LS.fork, caller));
+  for (int l = 1; l < nlevels; ++l) {
+    CUDA_TRY(cudaStreamWaitEvent(LS.s[l], LS.fork, 0));
+    levels[l]->stream = LS.s[l];
+  }
+  A.ev = LS.ev.data();
+  rc = advance_level(A, 0, dt0);
+  cudaError_t e = cudaSuccess;
+  for (int l = 1; l < nlevels; ++l) {   // join: the caller's stream continues after every level
+    levels[l]->stream = caller;
+    if (e == cudaSuccess) e = cudaEventRecord(LS.ev[l], LS.s[l]);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(caller, LS.ev[l], 0);
+  }
+  if (rc == AMR_OK && e != cudaSuccess) return fail(AMR_ECUDA, "stream join: %s", cudaGetErrorString(e));
+  return rc;
 }
 
 }  // extern "C"
