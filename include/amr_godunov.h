@@ -149,8 +149,9 @@ int amr_reflux(amr_level_link* l, double dt_coarse);
  * be properly nested: a level-(l+1) halo and its prolongation stencil lie inside level l's patches, else
  * amr_link_levels fails with AMR_EINVAL).  Nothing is owned by these calls.
  *
- * amr_hierarchy_cfl_dt: smax = max over the levels of amr_cfl_dt's smax, dt0 = cfl * dx_0 / smax (one
- * 8-byte read per level).
+ * amr_hierarchy_cfl_dt: smax = max over the levels of amr_cfl_dt's smax, dt0 = cfl * dx_0 / smax (the smax
+ * kernels of the levels whose fused value is stale and one 8-byte read per level are enqueued first, then one
+ * synchronisation).
  * amr_hierarchy_step: one root step dt0.  advance(l, dt): clear link l's flux registers; step level l by dt
  * (hydro or MHD, with c_h = ch on every level); if level l+1 exists, twice { amr_prolong_ghosts(links[l],
  * theta = 0, 1/2); advance(l+1, dt/2) }; amr_restrict(links[l]); amr_reflux(links[l], dt) unless do_reflux

@@ -898,12 +898,33 @@ extern "C" {
 int amr_hierarchy_cfl_dt(amr_patch_batch* const* levels, int nlevels, double gamma, double cfl, int mhd,
                          double* dt0_out, double* smax_out) {
   if (!levels || nlevels < 1 || nlevels > 30) return fail(AMR_EINVAL, "levels must hold 1..30 batches");
-  int rc;
+  if (!std::isfinite(gamma) || !(gamma > 1)) return fail(AMR_EINVAL, "gamma must be finite and > 1");
+  if (!(cfl > 0) || !std::isfinite(cfl)) return fail(AMR_EINVAL, "cfl must be finite and > 0");
+  // every level's smax kernel (where the fused value is stale) and 8-byte read are enqueued first, into pinned
+  // host memory, then ONE synchronisation per distinct stream - not one round trip per level
+  thread_local double* pinned = nullptr;
+  if (!pinned) CUDA_TRY(cudaHostAlloc((void**)&pinned, 32 * sizeof(double), cudaHostAllocDefault));
+  for (int l = 0; l < nlevels; ++l) {
+    amr_patch_batch* b = levels[l];
+    if (!b) return fail(AMR_EINVAL, "null batch at level %d", l);
+    if ((mhd != 0) != (b->d.nfields == 9)) return fail(AMR_EINVAL, "mhd flag does not match nfields = %d", b->d.nfields);
+    if (!(b->smax_valid && b->smax_gamma == gamma)) {
+      CUDA_TRY(cudaMemsetAsync(b->smax_slot, 0, 16, b->stream));
+      cudaError_t e = amr::launch_smax(b->d.dtype, b->U[b->cur], b->d.nfields, b->d.npatch, b->d.n, gamma, b->smax_slot, b->stream);
+      if (e != cudaSuccess) return fail(AMR_ECUDA, "smax kernel launch: %s", cudaGetErrorString(e));
+      b->smax_valid = true;
+      b->smax_gamma = gamma;
+    }
+    pinned[l] = 0;
+    CUDA_TRY(cudaMemcpyAsync(&pinned[l], b->smax_slot, b->d.dtype == AMR_F32 ? 4 : 8, cudaMemcpyDeviceToHost, b->stream));
+  }
+  for (int l = 0; l < nlevels; ++l)
+    if (l == 0 || levels[l]->stream != levels[l - 1]->stream) CUDA_TRY(cudaStreamSynchronize(levels[l]->stream));
   double sm = 0;
   for (int l = 0; l < nlevels; ++l) {
-    if (!levels[l]) return fail(AMR_EINVAL, "null batch at level %d", l);
-    double dt_l, sm_l;
-    if ((rc = amr_cfl_dt(levels[l], gamma, cfl, mhd, &dt_l, &sm_l)) != AMR_OK) return rc;
+    double sm_l;
+    if (levels[l]->d.dtype == AMR_F32) { float v; std::memcpy(&v, &pinned[l], 4); sm_l = v; }
+    else sm_l = pinned[l];
     sm = sm_l > sm ? sm_l : sm;
   }
   if (!(sm > 0) || !std::isfinite(sm)) return fail(AMR_ESTATE, "maximum signal speed over the levels is not finite and > 0");
