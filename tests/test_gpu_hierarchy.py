@@ -159,3 +159,19 @@ def test_three_level_step_patch_size_8(oracle, H, np_dtype):
     g = wl.levels[0].g
     tot = oracle.hierarchy_totals([oracle.ghosted(u.astype(np.float64), g) for u in got["U"]], wl.levels)
     assert (np.abs(tot - ref["totals_before"])[:8] / _absn(wl.levels[0])[:8]).max() <= (4e-6 if f32 else 1e-13)
+
+
+@pytest.mark.parametrize("np_dtype", [np.float64, np.float32])
+def test_overlapped_levels_give_the_bits_of_the_serial_schedule(H, hierarchies, np_dtype, monkeypatch):
+    """amr_hierarchy_step runs the levels on their own streams (a level's first substep beside its parent's step).
+    With AMR_HIERARCHY_OVERLAP=0 everything goes to the caller's stream in program order; three root steps must
+    give bitwise the same state either way (any missing cross-level dependency shows up as a difference)."""
+    wl = hierarchies[True]
+    monkeypatch.setenv("AMR_HIERARCHY_OVERLAP", "0")
+    serial = H.gpu_hierarchy_step(wl, np_dtype=np_dtype, nsteps=3)
+    for rep in range(3):
+        monkeypatch.setenv("AMR_HIERARCHY_OVERLAP", "1")
+        over = H.gpu_hierarchy_step(wl, np_dtype=np_dtype, nsteps=3)
+        assert serial["dts"] == over["dts"]
+        for l in range(3):
+            assert np.array_equal(serial["U"][l], over["U"][l]), (rep, l)
