@@ -180,23 +180,22 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
   for (int p = 0; p < f->d.npatch; ++p) {
     const int* o = &f->origin[3 * p];
     std::fill(slot.begin(), slot.end(), -1);
-    for (int k = -g; k < n + g; ++k)
-      for (int j = -g; j < n + g; ++j)
-        for (int i = -g; i < n + g; ++i) {
-          const int rx = i < 0 ? 0 : (i >= n ? 2 : 1), ry = j < 0 ? 0 : (j >= n ? 2 : 1), rz = k < 0 ? 0 : (k >= n ? 2 : 1);
-          if (rx == 1 && ry == 1 && rz == 1) continue;
-          if (f->nbr_host[(size_t)p * 27 + rz * 9 + ry * 3 + rx] != amr::NBR_FROM_HALO) continue;
-          int gi[3] = {o[0] + i, o[1] + j, o[2] + k};
-          long long par = 0;
-          for (int a = 0; a < 3; ++a) {
-            par |= (long long)wrapi(gi[a], 2) << a;
-            gi[a] = wrapi(gi[a], domf[a]);
-          }
+    // region by region (27 neighbour regions of the patch; only those no sibling covers have entries)
+    const int lo[3] = {-g, 0, n}, hi[3] = {0, n, n + g};
+    for (int reg = 0; reg < 27; ++reg) {
+      const int rx = reg % 3, ry = (reg / 3) % 3, rz = reg / 9;
+      if (reg == 13 || f->nbr_host[(size_t)p * 27 + reg] != amr::NBR_FROM_HALO) continue;
+    for (int k = lo[rz]; k < hi[rz]; ++k)
+      for (int j = lo[ry]; j < hi[ry]; ++j)
+        for (int i = lo[rx]; i < hi[rx]; ++i) {
+          // patch origins are even: the parity of a fine cell inside its parent is that of its offset
+          const long long par = (long long)(i & 1) | ((long long)(j & 1) << 1) | ((long long)(k & 1) << 2);
           const long long cell = (long long)p * (long long)M3 + ((long long)(k + g) * M + (j + g)) * M + (i + g);
           // patch origins are even: the parent's position in the patch's halo box is floor(offset / 2) + 2
           const int li = ((i + 4) >> 1), lj = ((j + 4) >> 1), lk = ((k + 4) >> 1);
           int& sl = slot[((size_t)lk * hp + lj) * hp + li];
           if (sl < 0) {   // first child of this parent: resolve the 7-point stencil in the coarse batch
+            const int gi[3] = {wrapi(o[0] + i, domf[0]), wrapi(o[1] + j, domf[1]), wrapi(o[2] + k, domf[2])};
             const int C[3] = {gi[0] / 2, gi[1] / 2, gi[2] / 2};
             long long s7[7];
             bool ok = coarse_flat(C[0], C[1], C[2], &s7[0]);
@@ -213,6 +212,7 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
           }
           H.pro_dst[(size_t)sl * 8 + (size_t)par] = cell;
         }
+    }
   }
   // O9(6) list: entry e = (p, ck, cj, ci)
   for (int p = 0; p < f->d.npatch; ++p) {
@@ -318,6 +318,7 @@ LinkLayout make_link_layout(const amr_patch_batch* c, const amr_patch_batch* f, 
 int check_link_args(const amr_patch_batch* c, const amr_patch_batch* f, int ratio) {
   if (!c || !f) return fail(AMR_EINVAL, "null batch");
   if (ratio != 2) return fail(AMR_EINVAL, "only refinement ratio 2 is supported");
+  if (f->d.n % 2) return fail(AMR_EINVAL, "linked batches need an even patch size");
   if (c->d.n != f->d.n || c->d.nfields != f->d.nfields || c->d.dtype != f->d.dtype || c->d.nghost != f->d.nghost)
     return fail(AMR_EINVAL, "coarse and fine batches must agree in n, nfields, dtype, nghost");
   if (c->d.self_periodic || f->d.self_periodic) return fail(AMR_EINVAL, "self-periodic batches cannot be linked");
