@@ -177,6 +177,11 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
   const int hp = n / 2 + 4;   // parent cells along one side of a patch's halo box (fine -g..n+g-1, g <= 4)
   if (g > 4) return fail(AMR_EINVAL, "nghost > 4 is not supported by the prolongation tables");
   std::vector<int> slot((size_t)hp * hp * hp);
+  {  // at most the parents of the halo shell per patch; untouched reserve costs nothing, regrowth copies do
+    const size_t h = (size_t)n / 2, shell = (size_t)hp * hp * hp - (h > 2 ? (h - 2) * (h - 2) * (h - 2) : 0);
+    H.pro_dst.reserve((size_t)f->d.npatch * shell * 8);
+    H.pro_c7.reserve((size_t)f->d.npatch * shell * 7);
+  }
   for (int p = 0; p < f->d.npatch; ++p) {
     const int* o = &f->origin[3 * p];
     std::fill(slot.begin(), slot.end(), -1);
