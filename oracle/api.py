@@ -174,7 +174,8 @@ def prolong_ghosts(Uf, mask, lf, Ucold, Ucnew, lc, theta: float):
     oc, dc = _geom_args(lc)
     nf, npf, M = Uf.shape[0], Uf.shape[1], Uf.shape[2]
     lib().oracle_prolong_ghosts(_dt(Uf), _p(Uf), _p(mask), npf, lf.n, lf.g, nf, _p(of), _p(df),
-                                _p(Ucold), _p(Ucnew), Ucold.shape[1], _p(oc), _p(dc), C.c_double(theta))
+                                _p(Ucold), _p(Ucnew), Ucold.shape[1], _p(oc), _p(dc), C.c_double(theta),
+                                _p(_ip(lf.bc)))
 
 
 def restrict(Uf, lf, Uc, lc):
@@ -188,7 +189,8 @@ def reflux(Uc, lc, Fc, lf, Ffsum, dt0: float):
     of, df = _geom_args(lf)
     oc, dc = _geom_args(lc)
     lib().oracle_reflux(_dt(Uc), _p(Uc), Uc.shape[1], lc.n, lc.g, Uc.shape[0], _p(oc), _p(dc), _p(Fc),
-                        Ffsum.shape[2], _p(of), _p(df), _p(Ffsum), C.c_double(dt0), C.c_double(lc.dx))
+                        Ffsum.shape[2], _p(of), _p(df), _p(Ffsum), C.c_double(dt0), C.c_double(lc.dx),
+                        _p(_ip(lc.bc)))
 
 
 def composite_totals(Uc, lc, Uf, lf) -> np.ndarray:

@@ -588,10 +588,14 @@ void prolong_ghosts(T* Uf, unsigned char* mask, const Geom& Gf, const T* Ucold, 
           const size_t c = Gf.cell(i, j, k);
           if (mask[(size_t)p * Gf.M3() + c]) continue;
           int gi[3] = {o[0] + i, o[1] + j, o[2] + k};
-          int par[3];  // parity of the fine index inside its coarse cell (before wrapping)
+          int par[3];  // parity of the fine index inside its coarse cell
           for (int d = 0; d < 3; ++d) {
-            par[d] = ((gi[d] % 2) + 2) % 2;
-            gi[d] = ((gi[d] % Gf.dom[d]) + Gf.dom[d]) % Gf.dom[d];
+            // a ghost cell beyond a domain face: periodic -> wrapped cell (even domain: parity unchanged);
+            // outflow -> O0 rule (ii): it takes the value of the clamped in-domain cell, which no fine
+            // patch covers (else O0 had filled it), i.e. the prolongation AT that cell (A12/A14)
+            if (gi[d] < 0) { if (Gf.bc[2 * d] == BC_PERIODIC) gi[d] += Gf.dom[d]; else gi[d] = 0; }
+            else if (gi[d] >= Gf.dom[d]) { if (Gf.bc[2 * d + 1] == BC_PERIODIC) gi[d] -= Gf.dom[d]; else gi[d] = Gf.dom[d] - 1; }
+            par[d] = gi[d] % 2;
           }
           const int C[3] = {gi[0] / 2, gi[1] / 2, gi[2] / 2};
           const int pc = pmc.at(C[0], C[1], C[2], Gc.n);
@@ -660,6 +664,9 @@ void reflux(T* Uc, const Geom& Gc, const T* Fc, const Geom& Gf, const T* Ffsum, 
             Cin[d] = o[d] / 2 + (side ? nc : -1);
             Cin[t1] = o[t1] / 2 + a;
             Cin[t2] = o[t2] / 2 + b;
+            // a fine face on a non-periodic domain face has no coarse cell outside it: nothing to correct
+            // (its flux is a boundary flux of the composite grid, A12/A14)
+            if ((Cin[d] < 0 && Gc.bc[2 * d] != BC_PERIODIC) || (Cin[d] >= Gc.dom[d] && Gc.bc[2 * d + 1] != BC_PERIODIC)) continue;
             int C[3];
             for (int e = 0; e < 3; ++e) C[e] = ((Cin[e] % Gc.dom[e]) + Gc.dom[e]) % Gc.dom[e];
             // covered by a sibling fine patch?  then the face is fine-fine: no correction
@@ -761,9 +768,9 @@ int oracle_fill_ghosts(int dtype, void* U, unsigned char* mask, int np, int n, i
 
 int oracle_prolong_ghosts(int dtype, void* Uf, unsigned char* mask, int npf, int n, int g, int nf,
                           const int* originf, const int* domf, const void* Ucold, const void* Ucnew,
-                          int npc, const int* originc, const int* domc, double theta) {
-  Geom Gf = make_geom(npf, n, g, nf, originf, domf, nullptr, 0);
-  Geom Gc = make_geom(npc, n, g, nf, originc, domc, nullptr, 0);
+                          int npc, const int* originc, const int* domc, double theta, const int* bc) {
+  Geom Gf = make_geom(npf, n, g, nf, originf, domf, bc, 0);
+  Geom Gc = make_geom(npc, n, g, nf, originc, domc, bc, 0);
   if (dtype == 1) prolong_ghosts<double>((double*)Uf, mask, Gf, (const double*)Ucold, (const double*)Ucnew, Gc, theta);
   else prolong_ghosts<float>((float*)Uf, mask, Gf, (const float*)Ucold, (const float*)Ucnew, Gc, (float)theta);
   return 0;
@@ -780,9 +787,9 @@ int oracle_restrict(int dtype, const void* Uf, int npf, int n, int g, int nf, co
 
 int oracle_reflux(int dtype, void* Uc, int npc, int n, int g, int nf, const int* originc, const int* domc,
                   const void* Fc, int npf, const int* originf, const int* domf, const void* Ffsum,
-                  double dt0, double dx0) {
-  Geom Gf = make_geom(npf, n, g, nf, originf, domf, nullptr, 0);
-  Geom Gc = make_geom(npc, n, g, nf, originc, domc, nullptr, 0);
+                  double dt0, double dx0, const int* bc) {
+  Geom Gf = make_geom(npf, n, g, nf, originf, domf, bc, 0);
+  Geom Gc = make_geom(npc, n, g, nf, originc, domc, bc, 0);
   if (dtype == 1) reflux<double>((double*)Uc, Gc, (const double*)Fc, Gf, (const double*)Ffsum, dt0, dx0);
   else reflux<float>((float*)Uc, Gc, (const float*)Fc, Gf, (const float*)Ffsum, (float)dt0, (float)dx0);
   return 0;

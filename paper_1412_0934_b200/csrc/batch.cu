@@ -193,14 +193,26 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
     for (int k = lo[rz]; k < hi[rz]; ++k)
       for (int j = lo[ry]; j < hi[ry]; ++j)
         for (int i = lo[rx]; i < hi[rx]; ++i) {
-          // patch origins are even: the parity of a fine cell inside its parent is that of its offset
-          const long long par = (long long)(i & 1) | ((long long)(j & 1) << 1) | ((long long)(k & 1) << 2);
+          // global fine index: periodic faces wrap, outflow faces clamp (O0 rule (ii): the halo cell takes the
+          // value of the clamped in-domain cell, which no fine patch covers, i.e. the prolongation AT that cell)
+          int gi[3] = {o[0] + i, o[1] + j, o[2] + k};
+          bool clamped = false;
+          for (int a = 0; a < 3; ++a) {
+            if (gi[a] < 0) {
+              if (f->d.bc[2 * a] == AMR_BC_PERIODIC) gi[a] += domf[a]; else { gi[a] = 0; clamped = true; }
+            } else if (gi[a] >= domf[a]) {
+              if (f->d.bc[2 * a + 1] == AMR_BC_PERIODIC) gi[a] -= domf[a]; else { gi[a] = domf[a] - 1; clamped = true; }
+            }
+          }
+          // patch origins and domain sizes are even: the parity of a fine cell inside its parent
+          const long long par = (long long)(gi[0] & 1) | ((long long)(gi[1] & 1) << 1) | ((long long)(gi[2] & 1) << 2);
           const long long cell = (long long)p * (long long)M3 + ((long long)(k + g) * M + (j + g)) * M + (i + g);
-          // patch origins are even: the parent's position in the patch's halo box is floor(offset / 2) + 2
+          // patch origins are even: the parent's position in the patch's halo box is floor(offset / 2) + 2.  Several
+          // clamped cells share one (parent, child), so each of them gets an entry of its own
           const int li = ((i + 4) >> 1), lj = ((j + 4) >> 1), lk = ((k + 4) >> 1);
-          int& sl = slot[((size_t)lk * hp + lj) * hp + li];
+          int own = -1;
+          int& sl = clamped ? own : slot[((size_t)lk * hp + lj) * hp + li];
           if (sl < 0) {   // first child of this parent: resolve the 7-point stencil in the coarse batch
-            const int gi[3] = {wrapi(o[0] + i, domf[0]), wrapi(o[1] + j, domf[1]), wrapi(o[2] + k, domf[2])};
             const int C[3] = {gi[0] / 2, gi[1] / 2, gi[2] / 2};
             long long s7[7];
             bool ok = coarse_flat(C[0], C[1], C[2], &s7[0]);
@@ -254,6 +266,9 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
             Cin[d] = o[d] / 2 + (side ? nc : -1);
             Cin[t1] = o[t1] / 2 + a;
             Cin[t2] = o[t2] / 2 + b;
+            // a fine face on a non-periodic domain face has no coarse cell outside it: its flux is a boundary
+            // flux of the composite grid, nothing to correct
+            if ((Cin[d] < 0 && c->d.bc[2 * d] != AMR_BC_PERIODIC) || (Cin[d] >= domc[d] && c->d.bc[2 * d + 1] != AMR_BC_PERIODIC)) continue;
             int C[3];
             for (int e = 0; e < 3; ++e) C[e] = wrapi(Cin[e], domc[e]);
             if (f->map.at(2 * C[0] / n, 2 * C[1] / n, 2 * C[2] / n) >= 0) continue;  // fine-fine face
@@ -327,6 +342,8 @@ int check_link_args(const amr_patch_batch* c, const amr_patch_batch* f, int rati
   if (c->d.n != f->d.n || c->d.nfields != f->d.nfields || c->d.dtype != f->d.dtype || c->d.nghost != f->d.nghost)
     return fail(AMR_EINVAL, "coarse and fine batches must agree in n, nfields, dtype, nghost");
   if (c->d.self_periodic || f->d.self_periodic) return fail(AMR_EINVAL, "self-periodic batches cannot be linked");
+  for (int a = 0; a < 6; ++a)
+    if (c->d.bc[a] != f->d.bc[a]) return fail(AMR_EINVAL, "linked batches must have the same boundary conditions");
   if (c->stream != f->stream) return fail(AMR_EINVAL, "linked batches must have been created on the same stream");
   if (f->d.level != c->d.level + 1) return fail(AMR_EINVAL, "fine.level must be coarse.level + 1");
   for (int a = 0; a < 3; ++a)

@@ -338,6 +338,35 @@ def test_two_level_step_fp32(oracle, H, mhd):
     assert (np.abs(tot - ref["totals_before"])[:nfc] / absn[:nfc]).max() <= 2e-6
 
 
+@pytest.mark.parametrize("mhd", [False, True])
+@pytest.mark.parametrize("np_dtype", [np.float64, np.float32])
+def test_two_level_step_with_fine_patches_on_outflow_faces(oracle, H, mhd, np_dtype):
+    """The boundary readings of O8 / O9: fine patches ON the outflow x faces.  Halo cells beyond
+    the face are clamped copies or prolongations at the clamped cell, fine faces on the domain face are not
+    refluxed.  Against the oracle, plus its own pin on the GPU result: the totals change only by the boundary
+    pressure force (tests/test_oracle_amr.py)."""
+    wl = wk.two_level_outflow(mhd)
+    lc, lf = wl.levels
+    f32 = np.dtype(np_dtype) == np.float32
+    if f32:
+        lc.U = lc.U.astype(np.float32).astype(np.float64)
+        lf.U = lf.U.astype(np.float32).astype(np.float64)
+    ref = oracle.two_level_step(wl, eps=oracle.default_eps(np_dtype))
+    got = H.gpu_two_level_step(wl, np_dtype=np_dtype)
+    tol = TOL32 if f32 else TOL64_STEP
+    ps = ref["smax"] * np.abs(ref["Uc"][5:8]).max() if mhd else None
+    ec = H.rel_err(got["Uc"], ref["Uc"], psi_scale=ps)
+    ef = H.rel_err(got["Uf"], ref["Uf"], psi_scale=ps)
+    assert ec.max() <= 2 * tol and ef.max() <= 2 * tol, (ec, ef)
+    tot = oracle.composite_totals(oracle.ghosted(got["Uc"].astype(np.float64), lc.g), lc,
+                                  oracle.ghosted(got["Uf"].astype(np.float64), lf.g), lf)
+    d = tot - ref["totals_before"]
+    keep = [0, 2, 3, 4] + ([5, 6, 7] if mhd else [])
+    assert np.abs(d[keep]).max() <= (2e-6 if f32 else 1e-13)
+    expect = got["dt0"] * (1.0 - 0.4)
+    assert abs(d[1] - expect) <= (1e-4 if f32 else 1e-11) * expect
+
+
 def test_prolonged_halo_seen_through_the_api(oracle, H):
     """O8 through the API: after amr_prolong_ghosts the fine ghosts equal the oracle's (theta = 0.5)."""
     import paper_1412_0934_b200 as amr

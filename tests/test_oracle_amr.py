@@ -109,3 +109,73 @@ def test_prolongation_is_limited_at_extrema(oracle):
     oracle.prolong_ghosts(Uf, mask, lf, Uc, Uc, lc, 0.0)
     assert np.all(Uf[:, 0, 1:3, 1:3, 7:9] == 5.0)
     assert np.all(Uf[:, 0, 1:3, 1:3, 9:11] == 1.0)
+
+
+# ---- boundary readings of O8 / O9: fine patches ON non-periodic domain faces (A12/A14) ----
+
+@pytest.mark.parametrize("mhd", [False, True])
+def test_two_level_outflow_totals_change_only_by_the_boundary_fluxes(oracle, mhd):
+    """Fine patches touch both OUTFLOW x faces; the gas at the faces is uniform and at rest for the whole
+    step, so the only boundary flux is the pressure force: d(sum m_x dV) = dt0 (p_left - p_right) A with
+    A = 1, and rho, m_y, m_z, E (and B) are conserved to round-off.  A reflux that wrapped through the
+    outflow face would add dt0/dx0 (F_coarse(far face) - F_fine(near face)) = O(p_right - p_left) to the
+    cells on the far side and fail both checks."""
+    wl = wk.two_level_outflow(mhd)
+    lc, lf = wl.levels
+    r = oracle.two_level_step(wl)
+    nf = lc.nfields
+    absn = np.array([max(np.abs(lc.U[f]).sum() * lc.dx ** 3, 1.0) for f in range(nf)])
+    d = (r["totals_after"] - r["totals_before"]) / absn
+    keep = [0, 2, 3, 4] + ([5, 6, 7] if mhd else [])
+    assert np.abs(d[keep]).max() < 1e-13, d
+    expect = r["dt0"] * (1.0 - 0.4)
+    got = r["totals_after"][1] - r["totals_before"][1]
+    assert abs(got - expect) < 1e-12 * expect, (got, expect)
+    # the step did something on both levels (the jump sits inside the second fine patch)
+    assert np.abs(r["Uf"][:, 1] - lf.U[:, 1]).max() > 1e-3 and np.abs(r["Uc"] - lc.U).max() > 1e-3
+    # ... and nothing at all next to the faces, bitwise (uniform state at rest, zero-gradient ghosts)
+    assert np.array_equal(r["Uf"][:, 0, :, :, :4], lf.U[:, 0, :, :, :4])
+    assert np.array_equal(r["Uf"][:, 2, :, :, -4:], lf.U[:, 2, :, :, -4:])
+
+
+def test_two_level_outflow_uniform_state_is_a_fixed_point(oracle):
+    wl = wk.two_level_outflow(True)
+    for lv in wl.levels:
+        lv.U[...] = lv.U[:, :1, :1, :1, :1]          # the lower-left cell's state everywhere
+        lv.U[1:4] = 0.3 * lv.U[0]                    # ... moving (outflow faces see a uniform flow)
+        lv.U[4] += 0.5 * 3 * 0.09 * lv.U[0]
+    r = oracle.two_level_step(wl)
+    assert np.array_equal(r["Uf"][:8], wl.levels[1].U[:8])
+    # the covered root cells went through the 8-cell mean (a sum of eight equal numbers rounds): 1 ulp
+    assert np.abs(r["Uc"][:8] - wl.levels[0].U[:8]).max() <= 4e-16
+
+
+def test_prolongation_beyond_an_outflow_face_takes_the_clamped_cell(oracle):
+    """O0 rule (ii) + O8: a fine ghost cell beyond an OUTFLOW face takes the value of the clamped in-domain
+    fine cell; where no fine patch covers that cell it is the prolongation AT that cell (parent and child
+    parity of the clamped index), never data from the far side of the domain."""
+    wl = wk.two_level_outflow(False)
+    lc, lf = wl.levels
+    g, n = lf.g, lf.n
+    rng = np.random.default_rng([wk.SEED, 141])
+    lc.U[...] = rng.standard_normal(lc.U.shape)
+    Uc = oracle.ghosted(lc.U, g)
+    oracle.fill_ghosts(Uc, g, lc.origin, lc.domain_cells, lc.bc, False)
+    Uf = oracle.ghosted(np.zeros_like(lf.U), g)
+    mask = oracle.fill_ghosts(Uf, g, lf.origin, lf.domain_cells, lf.bc, False)
+    # patch 0 = (0,16,16): beyond the face, inside the patch's y-z footprint, O0 clamps onto the patch itself;
+    # the edge / corner regions beyond the face are left for O8
+    assert mask[0, g + 4, g + 4, 0] == 1 and mask[0, g + 4, 0, 0] == 0 and mask[0, 0, 0, 0] == 0
+    oracle.prolong_ghosts(Uf, mask, lf, Uc, Uc, lc, 0.0)
+    assert (mask == 0).sum() == 0
+    for ii in range(g):                                # array x index ii <-> i = ii - g < 0; clamped: array index g
+        assert np.array_equal(Uf[:, 0, :, :g, ii], Uf[:, 0, :, :g, g])
+        assert np.array_equal(Uf[:, 0, :g, :, ii], Uf[:, 0, :g, :, g])
+        assert np.array_equal(Uf[:, 0, n + g:, n + g:, ii], Uf[:, 0, n + g:, n + g:, g])
+    # same at the upper face for patch 2 = (48,32,32)
+    for ii in range(n + g, n + 2 * g):
+        assert np.array_equal(Uf[:, 2, :, :g, ii], Uf[:, 2, :, :g, n + g - 1])
+    # the clamped cells themselves are ordinary prolongations: children average to the parent
+    kids = Uf[:, 0, g + 2:g + 4, 1:3, g:g + 2]         # fine (k 2..3, j -2..-1, i 0..1) <-> coarse (9, 7, 0)
+    G0 = wk.configs.join_patches(lc.U, lc.origin, (32, 32, 32))
+    assert np.allclose(kids.mean(axis=(1, 2, 3)), G0[:, 9, 7, 0], rtol=1e-13, atol=1e-14)

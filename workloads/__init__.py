@@ -24,6 +24,7 @@ from .configs import (  # noqa: F401
     config2_random_patches,
     config3_orszag_tang,
     config4_two_level,
+    two_level_outflow,
     config_hierarchy,
     nested_hierarchy_from_fine,
     select_blocks,

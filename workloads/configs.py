@@ -363,6 +363,42 @@ def config4_two_level(mhd: bool, nfine: int = 256, n: int = 16, sigma: float = C
     return w
 
 
+def two_level_outflow(mhd: bool = False, n: int = 16) -> Workload:
+    """Two-level test set-up with OUTFLOW faces in x (periodic in y, z) and fine patches ON the x faces:
+    a 32^3 root ([0,1]^3, 2x2x2 patches) at rest; left state (rho, p) = (1, 1) for x < 3/8, right state
+    (0.5, 0.4) beyond, the jump modulated in y, z only for 1/4 < x < 3/4, so both x faces see a uniform state
+    at rest for a whole step.  Fine patches: (0,16,16) on the lower x face, its x-sibling (16,16,16) (holds
+    the jump), (48,32,32) on the upper x face.  Used by the pins of the boundary readings of O8 / O9."""
+    gamma = 1.4
+    N = 64
+    c = (np.arange(N) + 0.5) / N
+    Z, Y, X = np.meshgrid(c, c, c, indexing="ij")
+    left = X < 0.375
+    mod = np.where((X > 0.25) & (X < 0.75), 1.0 + 0.2 * np.sin(2 * np.pi * Y) * np.cos(2 * np.pi * Z), 1.0)
+    rho = np.where(left, 1.0, 0.5) * mod
+    p = np.where(left, 1.0, 0.4) * np.where((X > 0.25) & (X < 0.75), 1.0 + 0.1 * np.cos(2 * np.pi * Y), 1.0)
+    v = np.zeros((3, N, N, N))
+    if mhd:
+        B = (np.full_like(rho, 0.05), np.full_like(rho, 0.1), np.full_like(rho, -0.07))
+        Gf = primitive_to_conserved(rho, v, p, gamma, B=B)
+    else:
+        Gf = primitive_to_conserved(rho, v, p, gamma)
+    nf = Gf.shape[0]
+    Nc = N // 2
+    Gc = Gf.reshape(nf, Nc, 2, Nc, 2, Nc, 2).mean(axis=(2, 4, 6))
+    bc = (BC_OUTFLOW, BC_OUTFLOW, BC_PERIODIC, BC_PERIODIC, BC_PERIODIC, BC_PERIODIC)
+    origin0 = morton_patch_origins(Nc // n, Nc // n, Nc // n, n)
+    origin1 = np.array([[0, 16, 16], [16, 16, 16], [48, 32, 32]], np.int32)
+    lev0 = Level(n=n, g=3, level=0, dx=1.0 / Nc, origin=origin0, domain_cells=(Nc, Nc, Nc), bc=bc,
+                 self_periodic=False, U=split_into_patches(Gc, n, origin0))
+    lev1 = Level(n=n, g=3, level=1, dx=1.0 / N, origin=origin1, domain_cells=(N, N, N), bc=bc,
+                 self_periodic=False, U=split_into_patches(Gf, n, origin1))
+    w = Workload("two_level_outflow_" + ("mhd" if mhd else "hydro"), [lev0, lev1], gamma, mhd,
+                 LIM_MC, RS_HLLD if mhd else RS_HLLC, 0.3, 1)
+    w.note = "p_left=1 p_right=0.4"
+    return w
+
+
 def _dilate_periodic(m: np.ndarray) -> np.ndarray:
     out = np.zeros_like(m)
     for dz in (-1, 0, 1):
