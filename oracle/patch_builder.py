@@ -60,32 +60,47 @@ def curve_order(xyz: np.ndarray, bits: int):
 
 
 def build_patches(keys_sorted: np.ndarray, kmax: int):
-    """Step 2 on the sorted keys.  An aligned cube of side 2^k is the set of 8^k consecutive keys that share
-    the bits above 3k, so it is compact iff those 8^k keys are all present, i.e. (keys unique and sorted) iff
-    the run starting at its first key has length 8^k with last - first == 8^k - 1.  Every cell gets the
-    largest k <= kmax whose cube around it is compact; the cubes found are the patches.
+    """Step 2, written as the definition itself: the cells are a SET of coordinates; an
+    octree-aligned cube of side 2^k is compact iff every one of its 8^k coordinates is in the set; every cell
+    belongs to the largest compact cube (k <= kmax) that contains it.  The cells are visited in curve order;
+    a cell no earlier patch covers starts a patch: the largest k whose aligned cube around it is compact, by
+    direct membership tests (each aligned cube is tested once and the answer remembered).  Aligned cubes are
+    nested or disjoint, so the cubes found are disjoint, cover the cells, and the visited cell is the cube's
+    first cell along the curve.  No property of sorted keys is used.
     Returns (first, level): first[p] = position in curve order of the first cell of patch p, level[p] = k."""
     keys = np.asarray(keys_sorted, dtype=np.uint64)
     n = keys.shape[0]
-    pos_of = {int(k): i for i, k in enumerate(keys)}
+    bits = max(1, (int(keys.max()).bit_length() + 2) // 3) if n else 1
+    x, y, z = morton_decode(keys, bits)
+    coords = list(zip(x.tolist(), y.tolist(), z.tolist()))
+    cells = set(coords)
+    assert len(cells) == n, "cells are unique"
+    compact = {}                                   # (k, ox, oy, oz) -> every coordinate of the cube is a cell
+
+    def is_compact(k, ox, oy, oz):
+        key = (k, ox, oy, oz)
+        if key not in compact:
+            s = 1 << k
+            compact[key] = all((ox + a, oy + b, oz + c) in cells
+                               for c in range(s) for b in range(s) for a in range(s))
+        return compact[key]
+
+    covered = set()
     first, level = [], []
-    i = 0
-    while i < n:
+    for i, (cx, cy, cz) in enumerate(coords):
+        if (cx, cy, cz) in covered:
+            continue
         k_found = 0
         for k in range(kmax, 0, -1):
-            size = 8 ** k
-            base = int(keys[i]) & ~(size - 1)
-            j = pos_of.get(base)
-            if j is None or j + size - 1 >= n:
-                continue
-            if int(keys[j + size - 1]) == base + size - 1:
+            s = 1 << k
+            if is_compact(k, cx // s * s, cy // s * s, cz // s * s):
                 k_found = k
                 break
-        base = int(keys[i]) & ~(8 ** k_found - 1)
-        assert pos_of[base] == i, "cells of a compact cube are consecutive: the walk always lands on its first cell"
+        s = 1 << k_found
+        ox, oy, oz = cx // s * s, cy // s * s, cz // s * s
+        covered.update((ox + a, oy + b, oz + c) for c in range(s) for b in range(s) for a in range(s))
         first.append(i)
         level.append(k_found)
-        i += 8 ** k_found
     return np.asarray(first, dtype=np.int64), np.asarray(level, dtype=np.int32)
 
 

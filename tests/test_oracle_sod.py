@@ -191,3 +191,53 @@ def test_first_order_limit_is_monotone(oracle):
     rho = U[0, 0, 2, 2, :]
     assert np.all(np.diff(rho) <= 1e-14)
     assert rho.max() <= 1.0 + 1e-14 and rho.min() >= 0.125 - 1e-14
+
+
+# ---- O0 rule (ii) ACROSS patches (the outflow clamp that lands in a sibling: edge and corner regions) ----
+
+def _tiled(U1, n):
+    """The single-patch level data [nf, 1, N, N, N] cut into (N/n)^3 patches of n^3 (Morton order)."""
+    N = U1.shape[2]
+    origin = wk.morton_patch_origins(N // n, N // n, N // n, n)
+    return wk.split_into_patches(U1[:, 0], n, origin), origin
+
+
+def test_outflow_ghosts_across_siblings_are_the_edge_padding_of_the_domain(oracle):
+    """fill_ghosts on a 2x2x2 tiling of an outflow box, all three ghost layers, faces + edges + corners,
+    against the definition written with a library routine: the level-global array extended by
+    numpy.pad(mode='edge') (= clamp of the global index), cut at every patch.  A genuinely 3-D random field,
+    so a wrong source cell in any region of any patch fails; bitwise."""
+    n, g, N = 16, 3, 32
+    rng = np.random.default_rng([wk.SEED, 77])
+    G = rng.standard_normal((5, N, N, N))
+    origin = wk.morton_patch_origins(2, 2, 2, n)
+    U = wk.split_into_patches(G, n, origin)
+    Ug = oracle.ghosted(U, g)
+    mask = oracle.fill_ghosts(Ug, g, origin, (N, N, N), (1,) * 6, False)
+    assert mask.all()
+    P = np.pad(G, ((0, 0), (g, g), (g, g), (g, g)), mode="edge")
+    for p, (ox, oy, oz) in enumerate(origin):
+        assert np.array_equal(Ug[:, p], P[:, oz:oz + n + 2 * g, oy:oy + n + 2 * g, ox:ox + n + 2 * g]), p
+    # mixed faces: outflow in x only, periodic in y and z = edge padding in x, wrap padding in y, z
+    mask = oracle.fill_ghosts(Ug, g, origin, (N, N, N), (1, 1, 0, 0, 0, 0), False)
+    P = np.pad(np.pad(G, ((0, 0), (g, g), (g, g), (0, 0)), mode="wrap"), ((0, 0), (0, 0), (0, 0), (g, g)), mode="edge")
+    for p, (ox, oy, oz) in enumerate(origin):
+        assert np.array_equal(Ug[:, p], P[:, oz:oz + n + 2 * g, oy:oy + n + 2 * g, ox:ox + n + 2 * g]), p
+
+
+@pytest.mark.parametrize("axis", [0, 2])
+def test_sod_tiled_as_eight_patches_is_bitwise_the_single_patch_run(oracle, sod32, axis):
+    """Config 1 cut into 2x2x2 patches of 16^3 with the same outflow faces: 20 steps give bit for bit the
+    single-32^3-patch result of test_sod_l1_error_config1 (every cell sees the same stencil values, so any
+    difference is a ghost cell taken from the wrong place)."""
+    wl = wk.config1_sod(n=32, axis=axis)
+    lev = wl.levels[0]
+    U, origin = _tiled(lev.U, 16)
+    Ug = oracle.ghosted(U, lev.g)
+    for _ in range(20):
+        oracle.fill_ghosts(Ug, lev.g, origin, lev.domain_cells, lev.bc, False)
+        sm = oracle.smax(Ug, lev.g, wl.gamma)
+        Ug = oracle.step(Ug, lev.g, wl.cfl * (1.0 / 32) / sm, 1.0 / 32, wl.gamma, wl.limiter, wl.riemann)["U"]
+    got = wk.configs.join_patches(oracle.interior(Ug, lev.g), origin, (32, 32, 32))
+    ref = sod32[0] if axis == 0 else run_sod(oracle, 32, nsteps=20, axis=axis)[0]
+    assert np.array_equal(got, ref[:, 0])
