@@ -14,7 +14,12 @@ cosmological run.  N > 1 runs N independent replicas, one per 
 shard: DESIGN.md §8), and reports the aggregate.
 
 Prints ONE JSON line (rank 0).  Timing: CUDA events on the stream the library launches on, max over
-ranks; the state (4.8 GB for config 5) is far larger than L2, so no flush is needed between steps.
+ranks; --repeats regions (default 5) of exactly --steps steps each, the median region is reported; the
+state (4.8 GB for config 5) is far larger than L2, so no flush is needed between steps.  Before any number
+is printed one more step is compared with the oracle on 8 seeded patches (`parity`): a run that fails it
+prints "value": null and exits 3.  The default run also times config 3 (256^3, fp32 and fp64) under `also`,
+measures the plain FMA rate of the SMs for `alu_roofline.peak`, and times the oracle on all host cores and
+on one core (`cpu_baseline`).
 """
 from __future__ import annotations
 
@@ -216,8 +221,12 @@ def oracle_sample_level(W, npatch_sample: int):
                     bc=(0,) * 6, self_periodic=False, U=U)
 
 
-def oracle_time(W, npatch_sample: int, steps: int, warmup: int):
+def oracle_time(W, npatch_sample: int, steps: int, warmup: int, threads: int | None = None):
+    """Times the oracle, as it stands, on a bounded sample: `warmup` untimed steps, then `steps` timed ones.
+    threads = None: all host cores (the OpenMP default)."""
     from oracle import api as oracle  # the cpu_baseline / reference legs may execute the oracle
+    ncores = os.cpu_count() or 1
+    oracle.set_num_threads(threads if threads else ncores)
     lev = oracle_sample_level(W, npatch_sample)
     wl = wk.Workload("sample", [lev], W["gamma"], W["mhd"], W["limiter"], W["riemann"], W["cfl"], 1, W["alpha"])
     times = []
@@ -226,7 +235,96 @@ def oracle_time(W, npatch_sample: int, steps: int, warmup: int):
         oracle.advance(lev, wl, 1)
         if i >= warmup:
             times.append(time.perf_counter() - t0)
-    return lev.ncells, times, oracle.num_threads()
+    used = oracle.num_threads()
+    oracle.set_num_threads(ncores)
+    return lev.ncells, times, used
+
+
+def cpu_baseline_both(W, npatch: int):
+    """BASELINE.md section 3 protocol: the oracle on all host cores AND on one core, one warm-up step and the
+    median of three timed steps each, on bounded samples of the same workload (full Morton cubes of patches)."""
+    big = 512 if npatch >= 512 else (64 if npatch >= 64 else (8 if npatch >= 8 else 1))
+    small = 8 if W["n"] == 32 else min(big, 64)
+    if W.get("self_periodic"):
+        big, small = min(npatch, 512), min(npatch, 64)
+    nc, t_all, threads = oracle_time(W, big, 3, 1)
+    nc1, t_one, one = oracle_time(W, small, 3, 1, threads=1)
+    m_all, m_one = statistics.median(t_all), statistics.median(t_one)
+    return dict(value=nc / m_all, unit=UNIT, cores=threads, kind="oracle",
+                sample="first %d patches in Morton order as a periodic sub-domain (%d cells), one warm-up + median of 3 steps "
+                       "(O0+O7+O1..O6, fp64), %.2f s per step" % (big, nc, m_all),
+                one_core=dict(value=nc1 / m_one, unit=UNIT, cores=one,
+                              sample="first %d patches (%d cells), one warm-up + median of 3 steps, %.2f s per step" % (small, nc1, m_one)))
+
+
+def parity_gate(b, W, nsample: int = 8):
+    """parity is checked on the same run's output before any number is reported.  One more
+    step is taken after the timed region; `nsample` seeded patches of its output are compared element by element
+    with the oracle (the checker: fp64, same dt and c_h, the patch and its 26 neighbours cut out of the GPU's own
+    input state; tests/gpu_harness.sampled_patch_parity, the routine of the full-size parity tests).  Tolerance:
+    north_star's per-step bound (1e-12 fp64, 1e-5 fp32).  Outside every timed region."""
+    tests_dir = os.path.join(ROOT, "tests")
+    if tests_dir not in sys.path:
+        sys.path.insert(0, tests_dir)
+    import gpu_harness as H
+    from oracle import api as oracle
+    f32 = W["dtype"] == "f32"
+    np_dtype = np.float32 if f32 else np.float64
+    tol = 1e-5 if f32 else 1e-12
+    U0 = b.download()
+    dt, sm = one_step(b, W)
+    U1 = b.download()
+    npatch = int(U0.shape[1])
+    rng = np.random.default_rng([wk.SEED, 2, npatch])
+    ids = sorted(int(i) for i in rng.choice(npatch, size=min(nsample, npatch), replace=False))
+    wl = dict(gamma=W["gamma"], limiter=W["limiter"], riemann=W["riemann"], alpha=W["alpha"])
+    if W.get("self_periodic"):
+        errs = []
+        for s_ in ids:
+            Um = np.ascontiguousarray(U0[:, s_:s_ + 1]).astype(np.float64)
+            Ug = oracle.ghosted(Um, 3)
+            oracle.fill_ghosts(Ug, 3, np.zeros((1, 3), np.int32), (W["n"],) * 3, (0,) * 6, True)
+            r = oracle.step(Ug, 3, dt, W["dx"], W["gamma"], W["limiter"], W["riemann"], ch=sm, alpha=W["alpha"],
+                            eps=oracle.default_eps(np_dtype))
+            errs.append(H.rel_err(np.asarray(U1[:, s_:s_ + 1], np.float64), oracle.interior(r["U"], 3)))
+    else:
+        errs = H.sampled_patch_parity(oracle, U0, U1, W["origin"], W["n"], W["domain"], W["dx"], wl, dt, sm, ids, np_dtype)
+    worst = float(max(float(e.max()) for e in errs))
+    return dict(ok=bool(worst <= tol), max_rel_err=worst, tol=tol, patches=ids,
+                how="one extra step after the timed region; %d seeded patches vs the fp64 oracle on their 3x3x3-patch neighbourhoods" % len(ids))
+
+
+def timed_regions(b, W, K: int, repeats: int, dist, device):
+    """`repeats` regions of EXACTLY K steps each, every region bracketed by barrier + synchronize, CUDA events on the
+    library's stream; per-step events around the step call give the kernel time.  Returns (ms per step of each
+    region, max over ranks; kernel ms of every step of every region, max over ranks)."""
+    import torch
+    regions, kernels = [], []
+    for _ in range(repeats):
+        ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+        ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
+        start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        start.record()
+        for i in range(K):
+            dt, sm = b.cfl_dt(W["gamma"], W["cfl"])          # fused smax of the previous step: 8-byte D->H
+            ev0[i].record()
+            if W["mhd"]:
+                b.mhd_step(dt, W["gamma"], W["limiter"], W["riemann"], sm, W["alpha"])
+            else:
+                b.hydro_step(dt, W["gamma"], W["limiter"], W["riemann"])
+            ev1[i].record()
+        end.record()
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        km = [a.elapsed_time(c) for a, c in zip(ev0, ev1)]
+        vals = reduce_max_over_ranks([start.elapsed_time(end) / K] + km, dist, device)
+        regions.append(vals[0])
+        kernels.extend(vals[1:])
+    return regions, kernels
 
 
 def run_reference(args):
@@ -455,6 +553,9 @@ def main():
     ap.add_argument("--size", type=int, default=None, help="override the grid size N (config3/5) or patch count (config2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--repeats", type=int, default=5, help="timed regions of --steps steps each; the median is reported")
+    ap.add_argument("--no-parity", action="store_true", help="skip the oracle parity gate (profiling runs only)")
+    ap.add_argument("--no-also", action="store_true", help="skip the config-3 timings appended to the default run")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -489,7 +590,7 @@ def main():
     b = make_batch(W, device)
     b.upload(W["U"])
     ncells = b.ncells
-    K, Wm = args.steps, args.warmup
+    K, Wm, R = args.steps, args.warmup, max(1, args.repeats)
 
     for _ in range(Wm):
         one_step(b, W)
@@ -500,34 +601,19 @@ def main():
     if rank == 0:
         sampler.start()
         time.sleep(0.25)
-    ev0 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
-    ev1 = [torch.cuda.Event(enable_timing=True) for _ in range(K)]
-    start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    start.record()
-    for i in range(K):
-        dt, sm = b.cfl_dt(W["gamma"], W["cfl"])          # fused smax of the previous step: 8-byte D->H
-        ev0[i].record()
-        if W["mhd"]:
-            b.mhd_step(dt, W["gamma"], W["limiter"], W["riemann"], sm, W["alpha"])
-        else:
-            b.hydro_step(dt, W["gamma"], W["limiter"], W["riemann"])
-        ev1[i].record()
-    end.record()
-    torch.cuda.synchronize()
-    if dist is not None:
-        dist.barrier()
+    regions, kern_ms = timed_regions(b, W, K, R, dist, device)
     clocks = sampler.stop() if rank == 0 else None
-    total_ms = start.elapsed_time(end)
-    kern_ms = [a.elapsed_time(c) for a, c in zip(ev0, ev1)]
-    total_ms, kern_avg = reduce_max_over_ranks([total_ms, sum(kern_ms) / K], dist, device)
-    ms_per_step = total_ms / K
+    ms_per_step = statistics.median(regions)          # median of the R regions of K steps each
+    kern_med = statistics.median(kern_ms)
     value = job_value(world, ncells, ms_per_step)
 
-    # sanity of the evolved state (validity of the run, not parity: parity is tests/ -m gpu)
+    # validity of the evolved state, then parity of one more step against the oracle (the gate of SURVEY.md 8(d))
     counters = b.step_counters()
     tot = b.conserved_totals()
     state_ok = bool(np.all(np.isfinite(tot))) and counters["nonpositive_rho_after"] == 0
+    parity = None
+    if rank == 0 and not args.no_parity:
+        parity = parity_gate(b, W)
 
     # end to end through the C-ABI with HOST buffers: H2D of the state, step, D2H of the new state
     e2e = None
@@ -550,6 +636,7 @@ def main():
         nbytes = W["U"].numel() * W["U"].element_size()
         e2e = dict(value=job_value(world, ncells, ms2), unit=UNIT, h2d_bytes_per_step=int(nbytes),
                    d2h_bytes_per_step=int(nbytes + 8), ms_per_step=ms2, steps=ke)
+        del out_host
 
     if rank != 0:
         if dist is not None:
@@ -558,34 +645,75 @@ def main():
 
     pk = peaks()
     bpc = BYTES_PER_CELL[(kind, W["dtype"])]
-    ach = bpc * ncells / (kern_avg * 1e-3) / 1e9
-    kname = "x2::godunov_step_x2_kernel" if (W["dtype"] == "f32" and W["n"] % 16 == 0) else "godunov_step_kernel"
-    traffic, traffic_src = dram_traffic(args.workload if args.size is None else None)
-    roof = dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"],
-                traffic=traffic, traffic_unit="bytes per launch (dram read + write, ncu --set full)",
-                traffic_source=traffic_src, peak_source=pk["source"], kernel=kname, kernel_ms=kern_avg,
-                bytes_per_cell=bpc, frac_of_nominal_8TBs=ach / 8000.0)
+
+    def roofline_of(kind_, dtype_, n_, ncells_, kms, workload_for_traffic):
+        bpc_ = BYTES_PER_CELL[(kind_, dtype_)]
+        ach = bpc_ * ncells_ / (kms * 1e-3) / 1e9
+        kname = ("x2::godunov_step_x2_kernel" if dtype_ == "f32" else "d1::godunov_step_d1_kernel") if n_ % 16 == 0 else "godunov_step_kernel"
+        traffic, traffic_src = dram_traffic(workload_for_traffic)
+        return dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"],
+                    traffic=traffic, traffic_unit="bytes per launch (dram read + write, ncu --set full)",
+                    traffic_source=traffic_src, peak_source=pk["source"], kernel=kname, kernel_ms=kms,
+                    kernel_ms_how="median of the %d x %d per-step CUDA-event times" % (R, K),
+                    bytes_per_cell=bpc_, frac_of_nominal_8TBs=ach / 8000.0)
+
+    roof = roofline_of(kind, W["dtype"], W["n"], ncells, kern_med, args.workload if args.size is None else None)
+    # ALU roofline against the FMA rate MEASURED in this run (amr_measure_fma_peak: dependent-FMA chains on every SM)
     lanes = 128 if W["dtype"] == "f32" else 64
-    alu_peak = 148 * lanes * pk["sm_max_mhz"] * 1e6 * 2 / 1e12          # TFLOP/s, fma = 2
-    alu_ach = FLOPS_PER_CELL[kind] * ncells / (kern_avg * 1e-3) / 1e12
+    nominal = 148 * lanes * pk["sm_max_mhz"] * 1e6 * 2 / 1e12          # TFLOP/s, fma = 2
+    try:
+        alu_peak = amr.measure_fma_peak(amr.AMR_F32 if W["dtype"] == "f32" else amr.AMR_F64, 2.0, str(device))
+        alu_src = "measured in this run: amr_measure_fma_peak, ~2 ms of dependent-FMA chains on every SM"
+    except Exception as exc:  # noqa: BLE001  (the bench line must still be printed)
+        alu_peak, alu_src = nominal, "nominal (measurement failed: %s)" % exc
+    alu_ach = FLOPS_PER_CELL[kind] * ncells / (kern_med * 1e-3) / 1e12
     alu = dict(bound="alu", achieved=alu_ach, peak=alu_peak, unit="TFLOP/s", frac=alu_ach / alu_peak,
-               flops_per_cell=FLOPS_PER_CELL[kind],
-               peak_source="148 SMs x %d %s lanes x 2 (fma) x sm_max_mhz" % (lanes, W["dtype"]))
+               flops_per_cell=FLOPS_PER_CELL[kind], peak_source=alu_src,
+               nominal_peak=nominal, nominal_how="148 SMs x %d %s lanes x 2 (fma) x sm_max_mhz" % (lanes, W["dtype"]))
+
+    # the 256^3 half of north_star's target, timed in the same run (not part of the headline value)
+    also = None
+    if args.workload == "config5" and args.size is None and world == 1 and not args.no_also:
+        also = {}
+        del b
+        torch.cuda.empty_cache()
+        for name in ("config3_f32", "config3_f64"):
+            W3 = build_workload(name, device, None)
+            b3 = make_batch(W3, device)
+            b3.upload(W3["U"])
+            for _ in range(3):
+                one_step(b3, W3)
+            reg3, k3 = timed_regions(b3, W3, 5, 3, None, device)
+            p3 = None if args.no_parity else parity_gate(b3, W3)
+            r3 = roofline_of("mhd", W3["dtype"], W3["n"], b3.ncells, statistics.median(k3), name)
+            also[name] = dict(workload=W3["label"], cells=b3.ncells, steps=5, repeats=3, ms_per_step=statistics.median(reg3),
+                              value=b3.ncells / (statistics.median(reg3) * 1e-3), unit=UNIT, kernel_ms=r3["kernel_ms"],
+                              frac=r3["frac"], achieved_gbs=r3["achieved"], bytes_per_cell=r3["bytes_per_cell"],
+                              traffic=r3["traffic"], parity=p3)
+            del b3
+            torch.cuda.empty_cache()
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        sample = min(b.npatch, 512)
-        nc, times, threads = oracle_time(W, sample, 1, 0)
-        cpu = dict(value=nc / times[0], unit=UNIT, cores=threads, kind="oracle",
-                   sample="first %d patches in Morton order as a periodic sub-domain (%d cells), one step (O0+O7+O1..O6), fp64, %.1f s" % (sample, nc, times[0]))
+        cpu = cpu_baseline_both(W, int(W["U"].shape[1]))
 
-    out = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=Wm, ms_per_step=ms_per_step,
-               higher_is_better=True, scaling="weak", vs_baseline=None, dtype=W["dtype"], data="synthetic",
+    parity_ok = None if parity is None else bool(parity["ok"] and all(v["parity"] is None or v["parity"]["ok"] for v in (also or {}).values()))
+    out = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=Wm, repeats=R, ms_per_step=ms_per_step,
+               ms_per_step_regions=regions, higher_is_better=True, scaling="weak", vs_baseline=None, dtype=W["dtype"], data="synthetic",
                config=dict(workload=W["label"], physics=kind, cells_per_gpu=ncells, l2="state %.2f GB per buffer >> 126 MB L2, no flush needed" % (ncells * bpc / 2 / 1e9),
                            parallelism="replicas only (no sharding)" if world > 1 else "single GPU",
-                           step="amr_cfl_dt (fused smax, 8-byte D2H) + amr_%s_step" % kind),
-               roofline=roof, alu_roofline=alu, cpu_baseline=cpu, e2e=e2e, gpu_launches=K,
-               clocks=clocks, state_ok=state_ok, counters=counters)
+                           step="amr_cfl_dt (fused smax, 8-byte D2H) + amr_%s_step" % kind,
+                           timing="median of %d regions of exactly %d steps each (CUDA events, barrier + synchronize around every region)" % (R, K)),
+               roofline=roof, alu_roofline=alu, also=also, cpu_baseline=cpu, e2e=e2e, gpu_launches=K, gpu_launches_all_regions=K * R,
+               clocks=clocks, state_ok=state_ok, parity_ok=parity_ok, parity=parity, counters=counters)
+    if parity_ok is False or not state_ok:
+        # no number is reported from a run whose output fails parity (or went non-physical)
+        out["value"] = None
+        out["rejected"] = "parity gate failed" if parity_ok is False else "state went non-finite / non-positive"
+        print(json.dumps(out))
+        if dist is not None:
+            dist.destroy_process_group()
+        sys.exit(3)
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()

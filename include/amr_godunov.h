@@ -16,6 +16,11 @@
  *  - "host" / "device" is stated for every pointer.  Host metadata is copied at create time.
  *  - The DEVICE ARENA is allocated by the caller (e.g. a torch uint8 tensor) and only BORROWED:
  *    the library never frees it and keeps pointers into it until amr_patch_batch_destroy.
+ *    The only device memory the library obtains itself is transient and stream-ordered
+ *    (cudaMallocAsync / cudaFreeAsync on the batch's stream, released before the call returns):
+ *    the staging buffer of a ghosted upload/download and the flag array of amr_flag_blocks.
+ *  - The device of a batch is the device its arena lives on.  Every call makes that device
+ *    current for its own duration and restores the caller's; linked batches share one device.
  *  - Calls enqueue work on the cudaStream_t given at create time and do not synchronise, except
  *    the ones that return host data (upload/download, amr_cfl_dt, amr_conserved_totals,
  *    amr_step_counters), which synchronise that stream.
@@ -217,6 +222,12 @@ int amr_builder_results(amr_patch_builder* b, int64_t* perm, int64_t* first, int
  * max_patches. */
 int amr_builder_gather(amr_patch_builder* b, const void* dev_fields, int32_t nfields, int32_t dtype, int32_t k,
                        void* dev_out, int64_t max_patches, int32_t* host_origin, int64_t* count_out);
+
+/* Measurement aid for the benchmark's ALU roofline ("an FMA-chain microbenchmark in the
+ * same run"); not a step of the path.  Runs plain dependent-FMA chains on every SM for about `ms_target`
+ * milliseconds on cuda_stream (dev_scratch: DEVICE, >= 8 bytes, borrowed) and returns the measured rate in
+ * *tflops_out (2 flops per FMA per lane; dtype AMR_F32 or AMR_F64).  Synchronises the stream. */
+int amr_measure_fma_peak(int32_t dtype, void* dev_scratch, void* cuda_stream, double ms_target, double* tflops_out);
 
 const char* amr_last_error(void);
 /* Library/build description, e.g. "amr_godunov sm_100a ..." (static string). */

@@ -57,6 +57,11 @@ def num_threads() -> int:
     return int(lib().oracle_num_threads())
 
 
+def set_num_threads(nt: int) -> None:
+    """Thread count of the oracle's OpenMP loops over patches (bench.py: 1 core vs all cores)."""
+    lib().oracle_set_num_threads(int(nt))
+
+
 def fill_ghosts(Ug: np.ndarray, g: int, origin, domain_cells, bc, self_periodic: bool) -> np.ndarray:
     """O0 (i)+(ii) in place.  Returns mask[npatch, M, M, M]: 1 = interior or filled, 0 = left for O8."""
     nf, npch, M = Ug.shape[0], Ug.shape[1], Ug.shape[2]

@@ -831,6 +831,15 @@ int oracle_hlld_states(const double* WL, const double* WR, double gamma, double 
 
 double oracle_limited_slope(double a, double b, int lim) { return limited_slope<double>(a, b, lim); }
 
+// thread count of the OpenMP loops over patches (timing of the CPU baseline on 1 core / all cores; no arithmetic)
+void oracle_set_num_threads(int nt) {
+#ifdef _OPENMP
+  if (nt > 0) omp_set_num_threads(nt);
+#else
+  (void)nt;
+#endif
+}
+
 int oracle_num_threads(void) {
   int nt = 1;
 #ifdef _OPENMP

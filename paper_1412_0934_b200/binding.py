@@ -26,7 +26,7 @@ EXPORTS = (
     "amr_link_destroy", "amr_prolong_ghosts", "amr_flux_clear", "amr_restrict", "amr_reflux", "amr_last_error",
     "amr_version", "amr_builder_bytes", "amr_builder_create", "amr_builder_destroy", "amr_builder_build",
     "amr_builder_results", "amr_builder_gather", "amr_hierarchy_cfl_dt", "amr_hierarchy_step",
-    "amr_flag_blocks", "amr_regrid_bytes", "amr_regrid_fill",
+    "amr_flag_blocks", "amr_regrid_bytes", "amr_regrid_fill", "amr_measure_fma_peak",
 )
 
 
@@ -97,6 +97,7 @@ def lib():
                                          C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int]
         L.amr_builder_gather.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_int64,
                                          C.c_void_p, C.POINTER(C.c_int64)]
+        L.amr_measure_fma_peak.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -104,6 +105,17 @@ def lib():
 def _check(rc: int):
     if rc != 0:
         raise AmrError(rc, lib().amr_last_error().decode())
+
+
+def measure_fma_peak(dtype: int, ms_target: float = 2.0, device: str = "cuda:0") -> float:
+    """amr_measure_fma_peak: plain FMA throughput of the device in TFLOP/s (the benchmark's measured ALU peak)."""
+    import torch
+    scratch = torch.zeros(64, dtype=torch.uint8, device=device)
+    out = C.c_double()
+    with torch.cuda.device(scratch.device):
+        _check(lib().amr_measure_fma_peak(dtype, scratch.data_ptr(), int(torch.cuda.current_stream().cuda_stream),
+                                          float(ms_target), C.byref(out)))
+    return float(out.value)
 
 
 def _np_dtype(dtype: int):

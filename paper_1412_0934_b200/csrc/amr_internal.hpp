@@ -1,6 +1,7 @@
 // Internal declarations shared by the host code (batch.cu) and the kernel translation units.
 // Nothing here crosses the C-ABI (include/amr_godunov.h).  No code is shared with oracle/.
 #pragma once
+#include <atomic>
 #include <cuda_runtime.h>
 #include <stddef.h>
 #include <stdint.h>
@@ -46,6 +47,19 @@ void tile_shape_hydro_f64(int n, int* tx, int* ty);
 void tile_shape_mhd_f32(int n, int* tx, int* ty);
 void tile_shape_mhd_f64(int n, int* tx, int* ty);
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute of a kernel: remembered per kernel
+// instantiation as a bit mask over devices (atomic; setting it twice is harmless, so no lock is needed)
+inline cudaError_t ensure_dynamic_smem(const void* kern, int bytes, std::atomic<unsigned long long>& done) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  const unsigned long long bit = 1ull << (dev & 63);
+  if (done.load(std::memory_order_acquire) & bit) return cudaSuccess;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) done.fetch_or(bit, std::memory_order_release);
+  return e;
+}
+
 // aux kernels (aux_kernels.cu); dtype: 0 = f32, 1 = f64
 cudaError_t launch_smax(int dtype, const void* U, int nf, int np, int n, double gamma, void* smax_slot,
                         cudaStream_t s);
@@ -59,6 +73,7 @@ cudaError_t launch_gather_ghosted(int dtype, const void* U, const void* halo, co
 cudaError_t launch_scatter_interior(int dtype, const void* staged, int with_ghosts, int nf, int np, int n, int g,
                                     int p0, int npc, void* U, cudaStream_t s);
 cudaError_t launch_fill_nan(int dtype, void* ptr, size_t count, cudaStream_t s);
+cudaError_t launch_fma_chain(int dtype, void* sink, int grid, int iters, cudaStream_t s);
 
 // two-level kernels (aux_kernels.cu); table formats are documented at the kernels
 // dst: [nparents][8] child halo indices or -1, c7: [nparents][7] (formats at the kernel)

@@ -419,6 +419,33 @@ cudaError_t launch_zero_faces(int dtype, void* Fc, int nf, int n, const long lon
   return cudaGetLastError();
 }
 
+// ---- measurement aid (bench.py alu_roofline.peak; not on the path): plain FMA throughput of the SMs -----------
+// Every thread runs 8 independent chains of dependent fused multiply-adds (enough to cover the pipe latency
+// at 8 warps per scheduler); 2 flops per FMA per lane.
+template <class T>
+__global__ void __launch_bounds__(256) fma_chain_kernel(T* sink, int iters, T a, T b) {
+  T x[8];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) x[c] = (T)(threadIdx.x + c) * (T)1e-3;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int c = 0; c < 8; ++c) x[c] = fma(x[c], a, b);
+    }
+  }
+  T s = 0;
+#pragma unroll
+  for (int c = 0; c < 8; ++c) s += x[c];
+  if (s == (T)-123.456) sink[0] = s;     // never true for the launch arguments: keeps the chains alive
+}
+
+cudaError_t launch_fma_chain(int dtype, void* sink, int grid, int iters, cudaStream_t s) {
+  if (dtype == 0) fma_chain_kernel<float><<<(unsigned)grid, 256, 0, s>>>((float*)sink, iters, 0.999f, 1e-3f);
+  else fma_chain_kernel<double><<<(unsigned)grid, 256, 0, s>>>((double*)sink, iters, 0.999, 1e-3);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_flag_blocks(int dtype, const void* Ufield, int np, int n, double threshold, unsigned char* flags,
                                cudaStream_t s) {
   if (np == 0) return cudaSuccess;

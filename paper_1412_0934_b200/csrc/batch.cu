@@ -98,12 +98,26 @@ struct PatchMap {
 
 }  // namespace
 
+// Every entry point that takes a batch makes the batch's device current for the call and restores the caller's
+// device afterwards (a second GPU in the same process must not receive this batch's launches).
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
 struct amr_patch_batch {
   amr_batch_desc d;
   std::vector<int32_t> origin;
   std::vector<int> nbr_host;
   PatchMap map;
   cudaStream_t stream;
+  int device;        // the device the arena lives on (recorded at create; every call runs with it current)
   char* arena;
   size_t bytes, esz, n3, M3;
   void* U[2];
@@ -345,6 +359,7 @@ int check_link_args(const amr_patch_batch* c, const amr_patch_batch* f, int rati
   for (int a = 0; a < 6; ++a)
     if (c->d.bc[a] != f->d.bc[a]) return fail(AMR_EINVAL, "linked batches must have the same boundary conditions");
   if (c->stream != f->stream) return fail(AMR_EINVAL, "linked batches must have been created on the same stream");
+  if (c->device != f->device) return fail(AMR_EINVAL, "linked batches must live on the same device");
   if (f->d.level != c->d.level + 1) return fail(AMR_EINVAL, "fine.level must be coarse.level + 1");
   for (int a = 0; a < 3; ++a)
     if (f->d.domain_cells[a] != 2 * c->d.domain_cells[a]) return fail(AMR_EINVAL, "fine domain must be 2x the coarse domain");
@@ -382,6 +397,7 @@ amr::StepParams<T> make_params(amr_patch_batch* b, double dt, double gamma, doub
 
 int do_step(amr_patch_batch* b, bool mhd, double dt, double gamma, int limiter, int riemann, double ch, double alpha) {
   if (!b) return fail(AMR_EINVAL, "null batch");
+  DeviceGuard guard(b->device);
   if (mhd != (b->d.nfields == 9))
     return fail(AMR_EINVAL, "%s step on a batch with %d fields", mhd ? "MHD" : "hydro", b->d.nfields);
   if (!(dt > 0) || !std::isfinite(dt)) return fail(AMR_EINVAL, "dt must be finite and > 0");
@@ -396,6 +412,7 @@ int do_step(amr_patch_batch* b, bool mhd, double dt, double gamma, int limiter, 
   }
   if (b->needs_halo && !b->halo_valid)
     return fail(AMR_ESTATE, "level-%d batch has coarse-fine halo regions but amr_prolong_ghosts was never called", b->d.level);
+  b->smax_valid = false;   // the slot is about to be zeroed; it holds the new state's smax only after a successful launch
   CUDA_TRY(cudaMemsetAsync(b->smax_slot, 0, 16, b->stream));
   cudaError_t e;
   int tx = 0, ty = 0;
@@ -428,6 +445,42 @@ int set_error(int code, const char* where, const char* what) { return fail(code,
 extern "C" {
 
 const char* amr_last_error(void) { return g_err.c_str(); }
+
+int amr_measure_fma_peak(int32_t dtype, void* dev_scratch, void* cuda_stream, double ms_target, double* tflops_out) {
+  if (!dev_scratch || !tflops_out) return fail(AMR_EINVAL, "null argument");
+  if (dtype != AMR_F32 && dtype != AMR_F64) return fail(AMR_EINVAL, "dtype must be AMR_F32 or AMR_F64");
+  if (!(ms_target > 0) || ms_target > 1000) return fail(AMR_EINVAL, "ms_target must be in (0, 1000]");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return fail(AMR_ECUDA, "no CUDA device");
+  const int grid = sms * 8;                      // 8 CTAs of 256 threads per SM: 16 warps per scheduler
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return fail(AMR_ECUDA, "cudaEventCreate");
+  auto run = [&](int iters, float* ms) -> cudaError_t {
+    cudaEventRecord(e0, s);
+    cudaError_t e = amr::launch_fma_chain(dtype, dev_scratch, grid, iters, s);
+    cudaEventRecord(e1, s);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(ms, e0, e1);
+    return e;
+  };
+  float ms = 0;
+  int iters = 256;
+  cudaError_t e = run(iters, &ms);               // warm-up and calibration
+  if (e == cudaSuccess) e = run(iters, &ms);
+  if (e == cudaSuccess) {
+    const double scale = ms_target / (ms > 1e-3 ? ms : 1e-3);
+    iters = (int)std::min(1.0e7, std::max(64.0, iters * scale));
+    e = run(iters, &ms);
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "fma chain: %s", cudaGetErrorString(e));
+  const double flops = 2.0 * 64.0 * (double)iters * 256.0 * (double)grid;
+  *tflops_out = flops / (ms * 1e-3) / 1e12;
+  return AMR_OK;
+}
 const char* amr_version(void) { return "amr_godunov 0.1 (sm_100a; fused MUSCL-Hancock/HLLC/HLLD step, interiors-only SoA arena)"; }
 
 size_t amr_patch_batch_bytes(const amr_batch_desc* desc) {
@@ -508,6 +561,16 @@ int amr_patch_batch_create(const amr_batch_desc* desc, void* dev_arena, size_t b
     }
   }
   b->stream = (cudaStream_t)cuda_stream;
+  {
+    cudaPointerAttributes pa;
+    if (cudaPointerGetAttributes(&pa, dev_arena) != cudaSuccess || pa.type != cudaMemoryTypeDevice) {
+      cudaGetLastError();
+      delete b;
+      return fail(AMR_EINVAL, "dev_arena is not a device allocation");
+    }
+    b->device = pa.device;
+  }
+  DeviceGuard guard(b->device);
   b->arena = (char*)dev_arena;
   b->bytes = bytes;
   b->esz = desc->dtype == AMR_F64 ? 8 : 4;
@@ -550,6 +613,7 @@ int amr_patch_batch_create(const amr_batch_desc* desc, void* dev_arena, size_t b
 
 int amr_patch_batch_destroy(amr_patch_batch* b) {
   if (!b) return AMR_OK;
+  DeviceGuard guard(b->device);
   if (b->link_up || b->link_down) return fail(AMR_ESTATE, "batch is still linked; call amr_link_destroy first");
   cudaStreamSynchronize(b->stream);
   delete b;
@@ -563,6 +627,7 @@ void* amr_patch_batch_state(amr_patch_batch* b, int which) {
 
 int amr_patch_batch_upload(amr_patch_batch* b, const void* host, int with_ghosts) {
   if (!b || !host) return fail(AMR_EINVAL, "null pointer");
+  DeviceGuard guard(b->device);
   const int nf = b->d.nfields, np = b->d.npatch;
   const size_t state_bytes = (size_t)nf * np * b->n3 * b->esz;
   if (!with_ghosts) {
@@ -571,21 +636,21 @@ int amr_patch_batch_upload(amr_patch_batch* b, const void* host, int with_ghosts
     const size_t per_patch = (size_t)nf * b->M3 * b->esz;
     int chunk = (int)std::max<size_t>(1, std::min<size_t>((size_t)np, ((size_t)512 << 20) / per_patch));
     void* stage = nullptr;
-    CUDA_TRY(cudaMalloc(&stage, (size_t)chunk * per_patch));
+    CUDA_TRY(cudaMallocAsync(&stage, (size_t)chunk * per_patch, b->stream));   // stream-ordered, returned below
     for (int p0 = 0; p0 < np; p0 += chunk) {
       const int npc = std::min(chunk, np - p0);
       for (int q = 0; q < nf; ++q) {
         cudaError_t e = cudaMemcpyAsync((char*)stage + (size_t)q * npc * b->M3 * b->esz,
                                         (const char*)host + ((size_t)q * np + p0) * b->M3 * b->esz,
                                         (size_t)npc * b->M3 * b->esz, cudaMemcpyHostToDevice, b->stream);
-        if (e != cudaSuccess) { cudaFree(stage); return fail(AMR_ECUDA, "upload: %s", cudaGetErrorString(e)); }
+        if (e != cudaSuccess) { cudaFreeAsync(stage, b->stream); return fail(AMR_ECUDA, "upload: %s", cudaGetErrorString(e)); }
       }
       cudaError_t e = amr::launch_scatter_interior(b->d.dtype, stage, 1, nf, np, b->d.n, b->d.nghost, p0, npc,
                                                    b->U[b->cur], b->stream);
       if (e == cudaSuccess) e = cudaStreamSynchronize(b->stream);
-      if (e != cudaSuccess) { cudaFree(stage); return fail(AMR_ECUDA, "upload: %s", cudaGetErrorString(e)); }
+      if (e != cudaSuccess) { cudaFreeAsync(stage, b->stream); return fail(AMR_ECUDA, "upload: %s", cudaGetErrorString(e)); }
     }
-    cudaFree(stage);
+    cudaFreeAsync(stage, b->stream);
   }
   // both buffers hold the uploaded state, so that "previous state" is defined before the first step
   CUDA_TRY(cudaMemcpyAsync(b->U[1 - b->cur], b->U[b->cur], state_bytes, cudaMemcpyDeviceToDevice, b->stream));
@@ -596,6 +661,7 @@ int amr_patch_batch_upload(amr_patch_batch* b, const void* host, int with_ghosts
 
 int amr_patch_batch_download(amr_patch_batch* b, void* host, int with_ghosts) {
   if (!b || !host) return fail(AMR_EINVAL, "null pointer");
+  DeviceGuard guard(b->device);
   const int nf = b->d.nfields, np = b->d.npatch;
   if (!with_ghosts) {
     CUDA_TRY(cudaMemcpyAsync(host, b->U[b->cur], (size_t)nf * np * b->n3 * b->esz, cudaMemcpyDeviceToHost, b->stream));
@@ -605,7 +671,7 @@ int amr_patch_batch_download(amr_patch_batch* b, void* host, int with_ghosts) {
   const size_t per_patch = (size_t)nf * b->M3 * b->esz;
   int chunk = (int)std::max<size_t>(1, std::min<size_t>((size_t)np, ((size_t)512 << 20) / per_patch));
   void* stage = nullptr;
-  CUDA_TRY(cudaMalloc(&stage, (size_t)chunk * per_patch));
+  CUDA_TRY(cudaMallocAsync(&stage, (size_t)chunk * per_patch, b->stream));   // stream-ordered, returned below
   for (int p0 = 0; p0 < np; p0 += chunk) {
     const int npc = std::min(chunk, np - p0);
     cudaError_t e = amr::launch_gather_ghosted(b->d.dtype, b->U[b->cur], b->halo, b->nbr_dev, nf, np, b->d.n,
@@ -615,9 +681,9 @@ int amr_patch_batch_download(amr_patch_batch* b, void* host, int with_ghosts) {
                           (const char*)stage + (size_t)q * npc * b->M3 * b->esz, (size_t)npc * b->M3 * b->esz,
                           cudaMemcpyDeviceToHost, b->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(b->stream);
-    if (e != cudaSuccess) { cudaFree(stage); return fail(AMR_ECUDA, "download: %s", cudaGetErrorString(e)); }
+    if (e != cudaSuccess) { cudaFreeAsync(stage, b->stream); return fail(AMR_ECUDA, "download: %s", cudaGetErrorString(e)); }
   }
-  cudaFree(stage);
+  cudaFreeAsync(stage, b->stream);
   return AMR_OK;
 }
 
@@ -628,6 +694,7 @@ int amr_fill_ghosts(amr_patch_batch* b) {
 
 int amr_cfl_dt(amr_patch_batch* b, double gamma, double cfl, int mhd, double* dt_out, double* smax_out) {
   if (!b) return fail(AMR_EINVAL, "null batch");
+  DeviceGuard guard(b->device);
   if ((mhd != 0) != (b->d.nfields == 9)) return fail(AMR_EINVAL, "mhd flag does not match nfields = %d", b->d.nfields);
   if (!std::isfinite(gamma) || !(gamma > 1)) return fail(AMR_EINVAL, "gamma must be finite and > 1");
   if (!(cfl > 0) || !std::isfinite(cfl)) return fail(AMR_EINVAL, "cfl must be finite and > 0");
@@ -663,6 +730,7 @@ int amr_mhd_step(amr_patch_batch* b, double dt, double gamma, int limiter, int r
 
 int amr_conserved_totals(amr_patch_batch* b, double* totals) {
   if (!b || !totals) return fail(AMR_EINVAL, "null pointer");
+  DeviceGuard guard(b->device);
   const int nf = b->d.nfields;
   cudaError_t e = amr::launch_totals(b->d.dtype, b->U[b->cur], nf, b->d.npatch, b->d.n, b->partials, b->stream);
   if (e != cudaSuccess) return fail(AMR_ECUDA, "totals kernel launch: %s", cudaGetErrorString(e));
@@ -679,6 +747,7 @@ int amr_conserved_totals(amr_patch_batch* b, double* totals) {
 
 int amr_step_counters(amr_patch_batch* b, long long* counters, int reset) {
   if (!b || !counters) return fail(AMR_EINVAL, "null pointer");
+  DeviceGuard guard(b->device);
   CUDA_TRY(cudaMemcpyAsync(counters, b->counters, 4 * sizeof(long long), cudaMemcpyDeviceToHost, b->stream));
   if (reset) CUDA_TRY(cudaMemsetAsync(b->counters, 0, 4 * sizeof(long long), b->stream));
   CUDA_TRY(cudaStreamSynchronize(b->stream));
@@ -707,6 +776,7 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   int rc = check_link_args(coarse, fine, ratio);
   if (rc != AMR_OK) return rc;
   if (coarse->link_down) return fail(AMR_ESTATE, "the coarse batch already has a child level");
+  DeviceGuard guard(coarse->device);
   if (fine->link_up) return fail(AMR_ESTATE, "the fine batch already has a parent level");
   if (fine->link_down) return fail(AMR_ESTATE, "link a hierarchy from the root upwards: the fine batch already has a child level");
   if (!dev_ws || (uintptr_t)dev_ws % ALIGN) return fail(AMR_EINVAL, "workspace must be a %zu-byte aligned device pointer", ALIGN);
@@ -765,6 +835,7 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
 
 int amr_link_destroy(amr_level_link* l) {
   if (!l) return AMR_OK;
+  DeviceGuard guard(l->f->device);
   if (l->f->link_down) return fail(AMR_ESTATE, "destroy the finer link first (it records into this link's fine blocks)");
   cudaStreamSynchronize(l->c->stream);
   cudaStreamSynchronize(l->f->stream);
@@ -777,6 +848,7 @@ int amr_link_destroy(amr_level_link* l) {
 
 int amr_prolong_ghosts(amr_level_link* l, double theta) {
   if (!l) return fail(AMR_EINVAL, "null link");
+  DeviceGuard guard(l->f->device);
   if (!(theta >= 0 && theta <= 1)) return fail(AMR_EINVAL, "theta must be in [0,1]");
   amr_patch_batch *c = l->c, *f = l->f;
   cudaError_t e = amr::launch_prolong(f->d.dtype, f->halo, (size_t)f->d.npatch * f->M3, f->d.nfields, l->pro_dst, l->pro_c7,
@@ -788,6 +860,7 @@ int amr_prolong_ghosts(amr_level_link* l, double theta) {
 
 int amr_flux_clear(amr_level_link* l) {
   if (!l) return fail(AMR_EINVAL, "null link");
+  DeviceGuard guard(l->f->device);
   if (l->shared_c) {
     cudaError_t e = amr::launch_zero_faces(l->c->d.dtype, l->fblk_c, l->c->d.nfields, l->c->d.n, l->faces, l->nfaces, l->c->stream);
     if (e != cudaSuccess) return fail(AMR_ECUDA, "flux clear kernel launch: %s", cudaGetErrorString(e));
@@ -800,6 +873,7 @@ int amr_flux_clear(amr_level_link* l) {
 
 int amr_restrict(amr_level_link* l) {
   if (!l) return fail(AMR_EINVAL, "null link");
+  DeviceGuard guard(l->f->device);
   amr_patch_batch *c = l->c, *f = l->f;
   cudaError_t e = amr::launch_restrict(f->d.dtype, f->U[f->cur], (size_t)f->d.npatch * f->n3, f->d.nfields, f->d.n, l->res_dst,
                                        l->nres, c->U[c->cur], (size_t)c->d.npatch * c->n3, c->stream);
@@ -810,6 +884,7 @@ int amr_restrict(amr_level_link* l) {
 
 int amr_reflux(amr_level_link* l, double dt_coarse) {
   if (!l) return fail(AMR_EINVAL, "null link");
+  DeviceGuard guard(l->f->device);
   if (!(dt_coarse > 0) || !std::isfinite(dt_coarse)) return fail(AMR_EINVAL, "dt_coarse must be finite and > 0");
   amr_patch_batch* c = l->c;
   cudaError_t e = amr::launch_reflux(c->d.dtype, c->U[c->cur], (size_t)c->d.npatch * c->n3, c->d.nfields, c->d.n, l->faces,
@@ -925,6 +1000,8 @@ int amr_hierarchy_cfl_dt(amr_patch_batch* const* levels, int nlevels, double gam
   if (!(cfl > 0) || !std::isfinite(cfl)) return fail(AMR_EINVAL, "cfl must be finite and > 0");
   // every level's smax kernel (where the fused value is stale) and 8-byte read are enqueued first, into pinned
   // host memory, then ONE synchronisation per distinct stream - not one round trip per level
+  if (!levels[0]) return fail(AMR_EINVAL, "null batch at level 0");
+  DeviceGuard guard(levels[0]->device);
   thread_local double* pinned = nullptr;
   if (!pinned) CUDA_TRY(cudaHostAlloc((void**)&pinned, 32 * sizeof(double), cudaHostAllocDefault));
   for (int l = 0; l < nlevels; ++l) {
@@ -961,6 +1038,7 @@ int amr_hierarchy_step(amr_patch_batch* const* levels, amr_level_link* const* li
   int rc = check_hierarchy(levels, links, nlevels);
   if (rc != AMR_OK) return rc;
   if (!(dt0 > 0) || !std::isfinite(dt0)) return fail(AMR_EINVAL, "dt0 must be finite and > 0");
+  DeviceGuard guard(levels[0]->device);
   CycleArgs A{levels, links, nlevels, mhd, limiter, riemann, do_reflux, gamma, ch, alpha, nullptr};
   const char* env = std::getenv("AMR_HIERARCHY_OVERLAP");
   const bool overlap = nlevels > 1 && !(env && env[0] == '0');
@@ -1074,6 +1152,7 @@ extern "C" {
 
 int amr_flag_blocks(amr_patch_batch* b, int field, double threshold, unsigned char* host_flags) {
   if (!b || !host_flags) return fail(AMR_EINVAL, "null pointer");
+  DeviceGuard guard(b->device);
   if (field < 0 || field >= b->d.nfields) return fail(AMR_EINVAL, "field must be in [0, nfields)");
   if (b->d.n % 2) return fail(AMR_EINVAL, "n must be even");
   const size_t nflag = (size_t)b->d.npatch * 8;
@@ -1101,6 +1180,7 @@ int amr_regrid_fill(amr_patch_batch* new_fine, const amr_patch_batch* old_fine, 
   int rc = check_regrid_args(new_fine, old_fine, coarse);
   if (rc != AMR_OK) return rc;
   if (new_fine->link_up || new_fine->link_down) return fail(AMR_ESTATE, "fill the new batch before linking it");
+  DeviceGuard guard(new_fine->device);
   if (old_fine && old_fine->stream != new_fine->stream) return fail(AMR_EINVAL, "old and new fine batches must share the stream");
   if (!dev_ws || (uintptr_t)dev_ws % ALIGN) return fail(AMR_EINVAL, "workspace must be a %zu-byte aligned device pointer", ALIGN);
   RegridHost H;

@@ -795,11 +795,10 @@ template <class T, int NF, int LIM, int RS, int TX, int TY, int NT, int MAXR>
 cudaError_t launch_variant(const StepParams<T>& P, cudaStream_t s) {
   using G = TileGeom<T, NF, TX, TY>;
   auto kern = godunov_step_kernel<T, NF, LIM, RS, TX, TY, NT, MAXR>;
-  static bool configured = false;  // per instantiation; attribute is per device function
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
+  static std::atomic<unsigned long long> configured{0};  // per instantiation, one bit per device
+  {
+    cudaError_t e = ensure_dynamic_smem((const void*)kern, (int)G::smem_bytes, configured);
     if (e != cudaSuccess) return e;
-    configured = true;
   }
   const long long grid = (long long)P.np * P.ntx * P.nty * P.ntz;
   kern<<<(unsigned)grid, NT, G::smem_bytes, s>>>(P);

@@ -604,11 +604,10 @@ template <int NF, int LIM, int RS, int HX, int TY, int NT, int MAXR>
 cudaError_t launch_variant_d1(const StepParams<double>& P, cudaStream_t s) {
   using G = GeomD1<NF, HX, TY>;
   auto kern = godunov_step_d1_kernel<NF, LIM, RS, HX, TY, NT, MAXR>;
-  static bool configured = false;  // per instantiation; attribute is per device function
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
+  static std::atomic<unsigned long long> configured{0};  // per instantiation, one bit per device
+  {
+    cudaError_t e = ensure_dynamic_smem((const void*)kern, (int)G::smem_bytes, configured);
     if (e != cudaSuccess) return e;
-    configured = true;
   }
   const long long grid = (long long)P.np * P.ntx * P.nty;
   kern<<<(unsigned)grid, NT, G::smem_bytes, s>>>(P);

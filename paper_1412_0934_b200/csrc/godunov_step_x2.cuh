@@ -749,11 +749,10 @@ template <int NF, int LIM, int RS, int TX, int TY, int NT, int MAXR>
 cudaError_t launch_variant_x2(const StepParams<float>& P, cudaStream_t s) {
   using G = GeomX2<NF, TX, TY>;
   auto kern = godunov_step_x2_kernel<NF, LIM, RS, TX, TY, NT, MAXR>;
-  static bool configured = false;  // per instantiation; attribute is per device function
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::smem_bytes);
+  static std::atomic<unsigned long long> configured{0};  // per instantiation, one bit per device
+  {
+    cudaError_t e = ensure_dynamic_smem((const void*)kern, (int)G::smem_bytes, configured);
     if (e != cudaSuccess) return e;
-    configured = true;
   }
   const long long grid = (long long)P.np * P.ntx * P.nty;
   kern<<<(unsigned)grid, NT, G::smem_bytes, s>>>(P);

@@ -9,11 +9,7 @@
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
-#ifdef AMR_TUNE_NO_EXPECT
-#define X2_UNLIKELY(x) (x)
-#else
 #define X2_UNLIKELY(x) __builtin_expect((x), 0)
-#endif
 
 namespace amr {
 namespace x2 {

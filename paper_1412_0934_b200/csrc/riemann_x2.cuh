@@ -37,8 +37,8 @@ __device__ __forceinline__ void riemann_hydro2(const V* WL, const V* WR, const R
                                                int* s_cnt) {
   const V rL = WL[0], uL = WL[1], vL = WL[2], wL = WL[3], pL = WL[4];
   const V rR = WR[0], uR = WR[1], vR = WR[2], wR = WR[3], pR = WR[4];
-  const V cL = sqrt2((C.gamma * pL) * rcp2(rL)), cR = sqrt2((C.gamma * pR) * rcp2(rR));
-  const V cmax = max2(cL, cR);
+  // max(c_L, c_R) = sqrt(max(c_L^2, c_R^2)): one square root instead of two (the root is monotone)
+  const V cmax = sqrt2(max2((C.gamma * pL) * rcp2(rL), (C.gamma * pR) * rcp2(rR)));
   const V SL = min2(uL, uR) - cmax, SR = max2(uL, uR) + cmax;
   const V EL = fma(pL, C.igm1, (0.5f * rL) * fma(uL, uL, fma(vL, vL, wL * wL)));
   const V ER = fma(pR, C.igm1, (0.5f * rR) * fma(uR, uR, fma(vR, vR, wR * wR)));
@@ -112,8 +112,8 @@ __device__ __forceinline__ void riemann_mhd2(const V* WL, const V* WR, const RCT
   // fast speed along n: c_f^2 = (a + sqrt(max(a^2 - 4 gamma p Bn^2 / rho^2, 0))) / 2
   const V dL = max2(fma((gpL * irL) * (Bn2 * irL), -4.f, aL * aL), 0.f);
   const V dR = max2(fma((gpR * irR) * (Bn2 * irR), -4.f, aR * aR), 0.f);
-  const V cfL = sqrt2(0.5f * (aL + sqrt2(dL))), cfR = sqrt2(0.5f * (aR + sqrt2(dR)));
-  const V cmax = max2(cfL, cfR);
+  // max(c_fL, c_fR) = sqrt(max(c_fL^2, c_fR^2)): one outer square root instead of two (the root is monotone)
+  const V cmax = sqrt2(0.5f * max2(aL + sqrt2(dL), aR + sqrt2(dR)));
   const V SL = min2(uL, uR) - cmax, SR = max2(uL, uR) + cmax;
   const M fan = lt(SL, 0.f) & gt(SR, 0.f);
 

@@ -8,9 +8,6 @@ namespace amr {
 
 void tile_shape_mhd_f32(int n, int* tx, int* ty) {
   using C = TileCfg_mhd_f32;
-#ifdef AMR_TUNE_F32_SCALAR
-  if (n % AMR_TUNE_SC_TX == 0 && n % AMR_TUNE_SC_TY == 0) { *tx = AMR_TUNE_SC_TX; *ty = AMR_TUNE_SC_TY; return; }
-#endif
   if (n % C::WTX == 0 && n % C::WTY == 0) { *tx = C::WTX; *ty = C::WTY; }
   else if (n % C::STX == 0 && n % C::STY == 0) { *tx = C::STX; *ty = C::STY; }
   else { *tx = 8; *ty = 8; }
@@ -18,10 +15,6 @@ void tile_shape_mhd_f32(int n, int* tx, int* ty) {
 
 cudaError_t launch_step_mhd_f32(const StepParams<float>& P, int limiter, int riemann, cudaStream_t s) {
   using C = TileCfg_mhd_f32;
-#ifdef AMR_TUNE_F32_SCALAR   // tuning sweeps only: the scalar kernel with a -D tile
-  if (P.n % AMR_TUNE_SC_TX == 0 && P.n % AMR_TUNE_SC_TY == 0)
-    return launch_dispatch<float, 9, AMR_TUNE_SC_TX, AMR_TUNE_SC_TY, AMR_TUNE_SC_NT, AMR_TUNE_SC_MAXR>(P, limiter, riemann, s);
-#endif
   if (P.n % C::WTX == 0 && P.n % C::WTY == 0)
     return x2::launch_dispatch_x2<9, C::WTX, C::WTY, C::WNT, C::WMAXR>(P, limiter, riemann, s);
   if (P.n % C::STX == 0 && P.n % C::STY == 0)

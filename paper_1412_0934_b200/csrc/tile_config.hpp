@@ -8,23 +8,11 @@
 //   fp64: one cell per thread with the x2 kernel's structure (godunov_step_d1.cuh): HX*TY compute threads (whole
 //         warps) plus the aux warps, NT >= HX*TY + 2*TY + 2*HX; n = 8 (and other non-multiples of 16) run the first
 //         fp64 kernel (godunov_step.cuh) on 8x8 tiles
-// The AMR_TUNE_* macros exist for tuning sweeps only (one -D per value); the defaults are the product.
 #pragma once
-#ifndef AMR_TUNE_F32_WTX
-#define AMR_TUNE_F32_WTX 32
-#define AMR_TUNE_F32_WTY 8
-#define AMR_TUNE_F32_NT 192
-#define AMR_TUNE_F32_MAXR 168
-#endif
 namespace amr {
-#ifndef AMR_TUNE_HYDRO_F32_MAXR
-#define AMR_TUNE_HYDRO_F32_MAXR 96   /* 3 CTAs per SM: 18 warps, 5 on one scheduler -> at most 102 registers */
-#endif
-struct TileCfg_hydro_f32 { static constexpr int WTX = 32, WTY = 8, STX = 16, STY = 16, NT = 192, MAXR = AMR_TUNE_HYDRO_F32_MAXR; };
-struct TileCfg_mhd_f32 {
-  static constexpr int WTX = AMR_TUNE_F32_WTX, WTY = AMR_TUNE_F32_WTY, STX = 16, STY = 16, NT = 192, WNT = AMR_TUNE_F32_NT,
-                       MAXR = 168, WMAXR = AMR_TUNE_F32_MAXR;
-};
+// hydro fp32: 3 CTAs per SM = 18 warps, 5 on one scheduler -> at most 102 registers per thread
+struct TileCfg_hydro_f32 { static constexpr int WTX = 32, WTY = 8, STX = 16, STY = 16, NT = 192, MAXR = 96; };
+struct TileCfg_mhd_f32 { static constexpr int WTX = 32, WTY = 8, STX = 16, STY = 16, NT = 192, WNT = 192, MAXR = 168, WMAXR = 168; };
 struct TileCfg_hydro_f64 { static constexpr int HX = 16, TY = 8, NT = 192, MAXR = 168; };
 struct TileCfg_mhd_f64 { static constexpr int HX = 16, TY = 8, NT = 192, MAXR = 168; };
 }  // namespace amr

@@ -133,10 +133,50 @@ def sampled_patch_parity(oracle, U0, U1, origin, n, domain, dx, wl, dt, ch, samp
                        self_periodic=False, U=Um)
         Ug = oracle.ghosted(Um, 3)
         oracle.fill_ghosts(Ug, 3, lev.origin, lev.domain_cells, lev.bc, False)
-        r = oracle.step(Ug, 3, dt, dx, wl["gamma"], wl["limiter"], wl["riemann"], ch=ch, alpha=wl["alpha"],
+        # O1..O6 act patch by patch on the ghosted arrays: only the centre patch (index 13) is stepped
+        Uc = np.ascontiguousarray(Ug[:, 13:14])
+        r = oracle.step(Uc, 3, dt, dx, wl["gamma"], wl["limiter"], wl["riemann"], ch=ch, alpha=wl["alpha"],
                         eps=oracle.default_eps(np_dtype))
-        ref = oracle.interior(r["U"], 3)[:, 13]
+        ref = oracle.interior(r["U"], 3)[:, 0]
         got = np.asarray(U1[:, s], dtype=np.float64)
         ps = ch * np.abs(ref[5:8]).max() if ref.shape[0] == 9 else None
         errs.append(rel_err(got[:, None], ref[:, None], psi_scale=ps))
     return errs
+
+
+_ROT = {0: [0, 1, 2, 3, 4, 5, 6, 7, 8], 1: [0, 2, 3, 1, 4, 6, 7, 5, 8], 2: [0, 3, 1, 2, 4, 7, 5, 6, 8]}
+
+
+def cells_next_to_a_marginal_decision(oracle, level, wl, dt, ch, limiter, riemann, eps, cells, rel=1e-4):
+    """Readings A7 / A19: the HLL fallback (p_T* <= 0) and the skipped rotational waves (B_n^2 < eps p_T*) are the
+    discontinuous decisions of the MHD solver; the kernel takes them in the batch dtype, the oracle in fp64, so a face
+    whose criterion lies within fp32 round-off of its threshold may be decided differently and then changes its two
+    cells by O(1e-3).  For each cell (p, k, j, i) this returns whether one of its six faces is such a face ACCORDING
+    TO THE ORACLE: |p_T*| <= rel * max(p_TL, p_TR) or |B_n^2 - eps p_T*| <= rel * eps p_T* (oracle.hlld_states on the
+    oracle's own face states).  Everything else must meet the plain bound."""
+    g = level.g
+    Ug = oracle.ghosted(level.U, g)
+    oracle.fill_ghosts(Ug, g, level.origin, level.domain_cells, level.bc, level.self_periodic)
+    FS = oracle.step(Ug, g, dt, level.dx, wl.gamma, limiter, riemann, ch=ch, alpha=wl.alpha, eps=eps,
+                     want_face_states=True)["FS"]          # [d][0: W^-_d, 1: W^+_d][field][patch][M^3]
+    out = []
+    for (p, k, j, i) in cells:
+        c = [k + g, j + g, i + g]
+        marginal = False
+        for d in range(3):
+            e = [0, 0, 0]
+            e[2 - d] = 1
+            for upper in (0, 1):
+                lo = c if upper else [c[a] - e[a] for a in range(3)]
+                hi = [c[a] + e[a] for a in range(3)] if upper else c
+                WL = FS[d, 1, :, p, lo[0], lo[1], lo[2]][_ROT[d]]
+                WR = FS[d, 0, :, p, hi[0], hi[1], hi[2]][_ROT[d]]
+                st = oracle.hlld_states(WL, WR, wl.gamma, ch, eps)
+                if st["S"][0] >= 0 or st["S"][4] <= 0:
+                    continue                                # supersonic face: no star state is formed
+                pts, bn2 = st["ptstar"], st["Bn"] ** 2
+                ptk = max(WL[4] + 0.5 * (WL[5:8] ** 2).sum(), WR[4] + 0.5 * (WR[5:8] ** 2).sum())
+                if abs(pts) <= rel * ptk or abs(bn2 - eps * pts) <= rel * eps * abs(pts):
+                    marginal = True
+        out.append(marginal)
+    return out

@@ -20,9 +20,10 @@ def H():
 
 
 def test_config5_full_size_sampled_fp32(oracle, H):
-    """Config 5 as bench.py runs it: 512^3 = 4096 patches of 32^3, MHD fp32, MC + HLLD + GLM.  Step 1 and
-    step 3 are checked on 12 seeded sample patches each against the fp64 oracle restarted from the GPU's own
-    input state of that step (A17: the fp32 bound is per step); conserved totals over all 3 steps."""
+    """Config 5 as bench.py runs it and as BASELINE.json states it: 512^3 = 4096 patches of 32^3, MHD fp32,
+    MC + HLLD + GLM, 10 steps.  EVERY step is checked on 64 seeded sample patches
+    against the fp64 oracle restarted from the GPU's own input state of that step (A17: the fp32 bound is per
+    step); conserved totals over all 10 steps."""
     import torch
     import paper_1412_0934_b200 as amr
     dev = torch.device("cuda:0")
@@ -37,21 +38,20 @@ def test_config5_full_size_sampled_fp32(oracle, H):
     tot0 = b.conserved_totals()
     rng = np.random.default_rng([wk.SEED, 5, 512])
     before = U0
-    for step in range(3):
+    worst = []
+    for step in range(10):
         dt, sm = b.cfl_dt(wlp["gamma"], wlp["cfl"])
         b.mhd_step(dt, wlp["gamma"], wlp["limiter"], wlp["riemann"], sm, wlp["alpha"])
-        if step in (0, 2):
-            after = b.download()
-            ids = rng.choice(npatch, size=12, replace=False)
-            errs = H.sampled_patch_parity(oracle, before, after, origin, 32, (512,) * 3, 1.0 / 512, wlp, dt, sm, ids, np.float32)
-            assert max(e.max() for e in errs) <= 1e-5, errs
-            before = after
-        elif step == 1:
-            before = b.download()
+        after = b.download()
+        ids = rng.choice(npatch, size=64, replace=False)
+        errs = H.sampled_patch_parity(oracle, before, after, origin, 32, (512,) * 3, 1.0 / 512, wlp, dt, sm, ids, np.float32)
+        worst.append(max(e.max() for e in errs))
+        assert worst[-1] <= 1e-5, (step, worst)
+        before = after
     tot = b.conserved_totals()
     absn = np.abs(U0.astype(np.float64)).sum(axis=(1, 2, 3, 4))
     grp = np.array([absn[0], absn[1:4].max(), absn[1:4].max(), absn[1:4].max(), absn[4], absn[5:8].max(), absn[5:8].max(), absn[5:8].max()])
-    assert (np.abs(tot - tot0)[:8] / grp).max() <= 1e-6       # fp32 round-off of 3 x 1.3e8 cell updates, summed in fp64
+    assert (np.abs(tot - tot0)[:8] / grp).max() <= 3e-6       # fp32 round-off of 10 x 1.3e8 cell updates, summed in fp64
     c = b.step_counters()
     assert c["nonpositive_rho_after"] == 0 and np.isfinite(tot).all()
 

@@ -196,6 +196,61 @@ def test_every_limiter_and_solver_fp32(oracle, H, nf, limiter, rs_exact, n):
     assert 0.95 * rc["hll_fallback_faces"] - 4 <= gc["hll_fallback_faces"] <= 1.10 * rc["hll_fallback_faces"] + 4
 
 
+def _config_shaped(kind, nf, n):
+    """64^3 config-shaped data on n^3 patches: config 3 (Orszag-Tang) or the config-5 recipe (Mach-3 turbulence,
+    beta = 100); nf = 5 takes the same gas without the field (E loses B^2/2)."""
+    wl = wk.config3_orszag_tang(N=64, n=n) if kind == "config3" else wk.config5_turbulence(N=64, n=n)
+    lev = wl.levels[0]
+    U = lev.U.copy()
+    if nf == 5:
+        U[4] -= 0.5 * (U[5] ** 2 + U[6] ** 2 + U[7] ** 2)
+        U = np.ascontiguousarray(U[:5])
+        wl = wk.Workload(wl.name + "_hydro", [lev], wl.gamma, False, wl.limiter, wk.configs.RS_HLLC, wl.cfl, 1, 0.0)
+    lev.U = U.astype(np.float32).astype(np.float64)
+    return wl
+
+
+@pytest.mark.parametrize("kind", ["config3", "config5"])
+@pytest.mark.parametrize("nf", [5, 9])
+@pytest.mark.parametrize("limiter", [0, 1, 2])
+@pytest.mark.parametrize("rs_exact", [False, True])
+@pytest.mark.parametrize("n", [16, 32])
+def test_every_limiter_and_solver_fp32_at_the_plain_bound(oracle, H, kind, nf, limiter, rs_exact, n):
+    """north_star's fp32 bound, plain: one step of EVERY (limiter x Riemann solver x hydro/MHD) on config-shaped
+    data (config 3's Orszag-Tang vortex and config 5's turbulence at 64^3, n = 16 and n = 32 patches) within
+    1e-5 of the fp64 oracle started from the fp32-rounded data (A17) -- no allowance for the oracle's own fp32
+    error and no quantile; the only cells excused are those the ORACLE shows to touch a face within round-off
+    of a discontinuous decision (see below).  (The white-noise cases above stay as stress tests with their
+    documented bound.)  Event counters as the oracle's."""
+    wl = _config_shaped(kind, nf, n)
+    lev = wl.levels[0]
+    rs = (wk.configs.RS_HLLD if nf == 9 else wk.configs.RS_HLLC) if rs_exact else wk.configs.RS_HLL
+    ref = oracle.advance(lev, wl, 1, limiter=limiter, riemann_solver=rs, eps=oracle.default_eps(np.float32))
+    got = H.gpu_advance(lev, wl, 1, np_dtype=np.float32, limiter=limiter, riemann=rs)
+    ps = _psi_scale(ref["U"], ref["smaxs"][0]) if nf == 9 else None
+    # per cell: the largest error over the field groups, each normalised as in rel_err (A18)
+    e_cell = np.zeros(got["U"].shape[1:])
+    for grp in H.field_groups(nf):
+        den = np.abs(ref["U"][grp]).max()
+        if grp == [8]:
+            den = max(den, ps)
+        e_cell = np.maximum(e_cell, np.abs(got["U"][grp].astype(np.float64) - ref["U"][grp]).max(axis=0) / den)
+    bad = np.argwhere(e_cell > TOL32)
+    # The one allowance (A7 / A19, measured: config 5 at 64^3 with minmod + HLLD has ONE face with p_T* = -9e-8 p_T,
+    # which the oracle sends to the HLL fallback and fp32 arithmetic does not): a cell may miss the bound only if
+    # the oracle itself says one of its faces sits within fp32 round-off of a discontinuous decision; at most 4.
+    assert len(bad) <= 4, (len(bad), e_cell.max())
+    if len(bad):
+        assert nf == 9 and rs == wk.configs.RS_HLLD, (bad, e_cell.max())
+        ok = H.cells_next_to_a_marginal_decision(oracle, lev, wl, ref["dts"][0], ref["smaxs"][0], limiter, rs,
+                                                 oracle.default_eps(np.float32), bad)
+        assert all(ok), (bad, ok, e_cell[tuple(bad.T)])
+    assert abs(got["dts"][0] - ref["dts"][0]) <= 4e-6 * ref["dts"][0]
+    gc, rc = got["counters"], ref["counters"][0]
+    assert gc["nonpositive_rho_after"] == rc["nonpositive_rho_after"] == 0
+    assert abs(gc["positivity_fallback_cells"] - rc["positivity_fallback_cells"]) <= 2 + 0.02 * rc["positivity_fallback_cells"]
+
+
 @pytest.mark.parametrize("n,npx", [(24, 2), (48, 1), (64, 1)])
 @pytest.mark.parametrize("nf", [5, 9])
 def test_other_patch_sizes_fp32(oracle, H, n, npx, nf):
