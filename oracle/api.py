@@ -92,6 +92,27 @@ def step(Ug: np.ndarray, g: int, dt: float, dx: float, gamma: float, limiter: in
     return dict(U=out, counters=dict(zip(CNT_NAMES, cnt.tolist())), F=F, FS=FS)
 
 
+def ppm_parabola(a5) -> tuple:
+    """PPM steps P1 + P2 of one cell from its five-point stencil (a_{i-2} .. a_{i+2}): (aL, aR)."""
+    a5 = np.ascontiguousarray(a5, dtype=np.float64)
+    aL, aR = C.c_double(), C.c_double()
+    lib().oracle_ppm_parabola(_p(a5), C.byref(aL), C.byref(aR))
+    return float(aL.value), float(aR.value)
+
+
+def ppm_sweep(Ug: np.ndarray, g: int, d: int, dt: float, dx: float, gamma: float, riemann: int):
+    """One PPM sweep (P1..P5) along direction d (0 = x, 1 = y, 2 = z) on every patch; hydro only.  Returns
+    dict(U=ghosted array with updated interiors (ghosts copied from the input), counters=...)."""
+    nf, npch, M = Ug.shape[0], Ug.shape[1], Ug.shape[2]
+    out = Ug.copy()
+    cnt = np.zeros(4, dtype=np.int64)
+    rc = lib().oracle_ppm_sweep(_dt(Ug), _p(Ug), _p(out), npch, M - 2 * g, g, nf, int(d), C.c_double(dt),
+                                C.c_double(dx), C.c_double(gamma), int(riemann), _p(cnt))
+    if rc != 0:
+        raise ValueError("oracle_ppm_sweep rejected its arguments")
+    return dict(U=out, counters=dict(zip(CNT_NAMES, cnt.tolist())))
+
+
 def smax(Ug: np.ndarray, g: int, gamma: float) -> float:
     """O7: max over interior cells and directions of |v_d| + c_d."""
     nf, npch, M = Ug.shape[0], Ug.shape[1], Ug.shape[2]
@@ -167,6 +188,32 @@ def advance(level, wl, nsteps: int, dtype=np.float64, dt_fixed: Optional[float] 
         dts.append(dt)
         smaxs.append(sm)
         counters.append(r["counters"])
+    return dict(U=interior(Ug, g), dts=dts, smaxs=smaxs, counters=counters)
+
+
+PPM_ORDERS = ((0, 1, 2), (2, 1, 0))     # sweep order 0: x-y-z, order 1: z-y-x
+
+
+def ppm_advance(level, wl, nsteps: int, dtype=np.float64, dt_fixed: Optional[float] = None,
+                riemann_solver: Optional[int] = None):
+    """Single-level PPM evolution as the harness sequences it: every step = O0 ghost fill, O7 smax ->
+    dt = cfl dx / smax, then three sweeps in the order x-y-z on even steps and z-y-x on odd steps, the ghost
+    cells refilled (O0) before every sweep.  Returns dict(U=final interior, dts, smaxs, counters)."""
+    g = level.g
+    Ug = ghosted(level.U, g, dtype)
+    rs = wl.riemann if riemann_solver is None else riemann_solver
+    dts, smaxs, counters = [], [], []
+    for step_no in range(nsteps):
+        fill_ghosts(Ug, g, level.origin, level.domain_cells, level.bc, level.self_periodic)
+        sm = smax(Ug, g, wl.gamma)
+        dt = dt_fixed if dt_fixed is not None else wl.cfl * level.dx / sm
+        for d in PPM_ORDERS[step_no % 2]:
+            fill_ghosts(Ug, g, level.origin, level.domain_cells, level.bc, level.self_periodic)
+            r = ppm_sweep(Ug, g, d, dt, level.dx, wl.gamma, rs)
+            Ug = r["U"]
+            counters.append(r["counters"])
+        dts.append(dt)
+        smaxs.append(sm)
     return dict(U=interior(Ug, g), dts=dts, smaxs=smaxs, counters=counters)
 
 

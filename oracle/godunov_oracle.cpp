@@ -474,6 +474,158 @@ int step_all(const T* Uin, T* Uout, T* Fout, T* FSout, const Geom& G, const Step
   return 0;
 }
 
+// ------------------------------------------------------------------------------------------
+// PPM (SURVEY.md 8(f1); PAPER.md:43 "the Piecewise Parabolic Method, PPM [9]", :76 "the PLM/PPM hydro
+// solver, have been ported to NVIDIA's CUDA").  The paper gives no formula; reading R-PPM of DESIGN.md
+// section 13: Colella & Woodward 1984 in the direct Eulerian, dimensionally split form (as in Enzo), hydro
+// only, primitive variables (rho, u, v, w, p) with u along the sweep, WITHOUT the optional dissipation of
+// CW84 section 4 (no contact steepening, no flattening, no artificial viscosity), and with the boundary's
+// HLL / HLLC flux (O5) in place of CW84's two-shock solver.  One sweep along direction d:
+//   P1  interface values, CW84 (1.6)-(1.8) on a uniform grid:
+//         da_i  = (a_{i+1} - a_{i-1}) / 2
+//         dm_i  = min(|da_i|, 2|a_i - a_{i-1}|, 2|a_{i+1} - a_i|) sgn(da_i)  if (a_{i+1}-a_i)(a_i-a_{i-1}) > 0, else 0
+//         a_{i+1/2} = a_i + (a_{i+1} - a_i)/2 - (dm_{i+1} - dm_i)/6 ;   aL_i = a_{i-1/2}, aR_i = a_{i+1/2}
+//   P2  monotonisation, CW84 (1.10):
+//         (aR-a)(a-aL) <= 0                          -> aL = aR = a
+//         (aR-aL)(a-(aL+aR)/2) >  (aR-aL)^2/6        -> aL = 3a - 2aR
+//         (aR-aL)(a-(aL+aR)/2) < -(aR-aL)^2/6        -> aR = 3a - 2aL
+//       then  Da = aR - aL,  a6 = 6(a - (aL+aR)/2)
+//   P3  averages over the domain of dependence of a wave of speed lambda, CW84 (1.12), s = |lambda| dt/dx:
+//         towards the upper face: Ip(s) = aR - s/2 (Da - (1 - 2s/3) a6)
+//         towards the lower face: Im(s) = aL + s/2 (Da + (1 - 2s/3) a6)
+//   P4  characteristic tracing, CW84 section 3 (3.5)-(3.7), written with the eigenvectors of the primitive
+//       system at the cell centre (c = sqrt(gamma p / rho); waves lambda_- = u-c, lambda_0 = u, lambda_+ = u+c):
+//       upper-face state W^+ : reference = Ip(max(lambda_+,0) dt/dx) of every variable; for every wave k with
+//         lambda_k > 0 subtract  [l_k . (ref - Ip_k)] r_k ,  Ip_k = Ip(lambda_k dt/dx)
+//       lower-face state W^- : reference = Im(max(-lambda_-,0) dt/dx); for every wave k with lambda_k < 0
+//         subtract  [l_k . (ref - Im_k)] r_k ,  Im_k = Im(-lambda_k dt/dx)
+//       on (rho, u, p):  l_- = (0, -rho/(2c), 1/(2c^2)), r_- = (1, -c/rho, c^2);  l_0 = (1, 0, -1/c^2),
+//       r_0 = (1, 0, 0);  l_+ = (0, rho/(2c), 1/(2c^2)), r_+ = (1, c/rho, c^2);  the transverse velocities
+//       ride on lambda_0: v^+ = Ip_0(v) if u > 0 else ref, v^- = Im_0(v) if u < 0 else ref.
+//       A cell whose traced rho or p is <= 0 (or non-finite) uses its cell-centre W for both states (counted).
+//   P5  flux at the lower face of cell i from (W^+_{i-1}, W^-_i) with O5's HLL / HLLC;  U_i -= dt/dx (F_{i+1/2} - F_{i-1/2}).
+// A step is three sweeps, x-y-z (order 0) or z-y-x (order 1), the ghost cells refilled before every sweep
+// (sequenced by oracle/api.py).  Needs g >= 3 ghost layers along the sweep (reading A11).
+// ------------------------------------------------------------------------------------------
+template <class T>
+void ppm_parabola(T am2, T am1, T a0, T ap1, T ap2, T* aL, T* aR) {
+  auto dm = [](T l, T c, T r) {
+    const T da = T(0.5) * (r - l);
+    if ((r - c) * (c - l) > 0) {
+      const T m = std::min(std::min(std::fabs(da), T(2) * std::fabs(c - l)), T(2) * std::fabs(r - c));
+      return da > 0 ? m : -m;
+    }
+    return T(0);
+  };
+  const T dmm = dm(am2, am1, a0), dm0 = dm(am1, a0, ap1), dmp = dm(a0, ap1, ap2);
+  T l = am1 + T(0.5) * (a0 - am1) - (dm0 - dmm) / T(6);   // a_{i-1/2}
+  T r = a0 + T(0.5) * (ap1 - a0) - (dmp - dm0) / T(6);    // a_{i+1/2}
+  if ((r - a0) * (a0 - l) <= 0) { l = a0; r = a0; }
+  else {
+    const T d = r - l, m = a0 - T(0.5) * (l + r);
+    if (d * m > d * d / T(6)) l = T(3) * a0 - T(2) * r;
+    else if (-(d * d) / T(6) > d * m) r = T(3) * a0 - T(2) * l;
+  }
+  *aL = l; *aR = r;
+}
+
+template <class T>
+void ppm_sweep_patch(const T* Uin, T* Uout, const Geom& G, int p, int d, T dt, T dx, T gamma, int solver,
+                     std::vector<T>& W, std::vector<T>& Wm, std::vector<T>& Wp, std::vector<T>& F, long long* cnt) {
+  const int n = G.n, M = G.M;
+  const size_t M3 = G.M3();
+  const size_t str[3] = {1, (size_t)M, (size_t)M * M};
+  const size_t sd = str[d];
+  const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
+  primitives(Uin, G, p, gamma, W.data());      // W[q*M3 + c], q = rho, vx, vy, vz, p
+  const int qu = 1 + d, qv = 1 + t1, qw = 1 + t2;
+  const int order[5] = {0, qu, qv, qw, 4};     // (rho, u, v, w, p) in sweep order
+  const T lam = dt / dx;
+  int lo[3] = {0, 0, 0}, hi[3] = {n - 1, n - 1, n - 1};
+  lo[d] = -1; hi[d] = n;
+  // P1-P4 on the interior grown by one cell along d
+  for (int k = lo[2]; k <= hi[2]; ++k)
+    for (int j = lo[1]; j <= hi[1]; ++j)
+      for (int i = lo[0]; i <= hi[0]; ++i) {
+        const size_t c = G.cell(i, j, k);
+        T a[5], aL[5], aR[5], Da[5], a6[5];
+        for (int m = 0; m < 5; ++m) {
+          const T* w = W.data() + (size_t)order[m] * M3;
+          a[m] = w[c];
+          ppm_parabola<T>(w[c - 2 * sd], w[c - sd], w[c], w[c + sd], w[c + 2 * sd], &aL[m], &aR[m]);
+          Da[m] = aR[m] - aL[m];
+          a6[m] = T(6) * (a[m] - T(0.5) * (aL[m] + aR[m]));
+        }
+        auto Ip = [&](int m, T s) { return aR[m] - T(0.5) * s * (Da[m] - (T(1) - T(2) * s / T(3)) * a6[m]); };
+        auto Im = [&](int m, T s) { return aL[m] + T(0.5) * s * (Da[m] + (T(1) - T(2) * s / T(3)) * a6[m]); };
+        const T rho = a[0], u = a[1], pr = a[4];
+        const T cs = std::sqrt(gamma * pr / rho);
+        const T lk[3] = {u - cs, u, u + cs};
+        T wp[5], wm[5];
+        {  // upper-face state
+          const T sref = std::max(lk[2], T(0)) * lam;
+          T ref[5];
+          for (int m = 0; m < 5; ++m) { ref[m] = Ip(m, sref); wp[m] = ref[m]; }
+          for (int kx = 0; kx < 3; ++kx) {
+            if (!(lk[kx] > 0)) continue;
+            const T s = lk[kx] * lam;
+            const T dr = ref[0] - Ip(0, s), du = ref[1] - Ip(1, s), dp = ref[4] - Ip(4, s);
+            if (kx == 0) { const T b = -rho / (T(2) * cs) * du + dp / (T(2) * cs * cs); wp[0] -= b; wp[1] -= b * (-cs / rho); wp[4] -= b * cs * cs; }
+            else if (kx == 2) { const T b = rho / (T(2) * cs) * du + dp / (T(2) * cs * cs); wp[0] -= b; wp[1] -= b * (cs / rho); wp[4] -= b * cs * cs; }
+            else { wp[0] -= dr - dp / (cs * cs); wp[2] = Ip(2, s); wp[3] = Ip(3, s); }
+          }
+        }
+        {  // lower-face state
+          const T sref = std::max(-lk[0], T(0)) * lam;
+          T ref[5];
+          for (int m = 0; m < 5; ++m) { ref[m] = Im(m, sref); wm[m] = ref[m]; }
+          for (int kx = 0; kx < 3; ++kx) {
+            if (!(lk[kx] < 0)) continue;
+            const T s = -lk[kx] * lam;
+            const T dr = ref[0] - Im(0, s), du = ref[1] - Im(1, s), dp = ref[4] - Im(4, s);
+            if (kx == 0) { const T b = -rho / (T(2) * cs) * du + dp / (T(2) * cs * cs); wm[0] -= b; wm[1] -= b * (-cs / rho); wm[4] -= b * cs * cs; }
+            else if (kx == 2) { const T b = rho / (T(2) * cs) * du + dp / (T(2) * cs * cs); wm[0] -= b; wm[1] -= b * (cs / rho); wm[4] -= b * cs * cs; }
+            else { wm[0] -= dr - dp / (cs * cs); wm[2] = Im(2, s); wm[3] = Im(3, s); }
+          }
+        }
+        const bool ok = (wp[0] > 0) && (wp[4] > 0) && (wm[0] > 0) && (wm[4] > 0) && std::isfinite(wp[0]) &&
+                        std::isfinite(wp[4]) && std::isfinite(wm[0]) && std::isfinite(wm[4]);
+        if (!ok) {
+          if (cnt) cnt[CNT_POSITIVITY]++;
+          for (int m = 0; m < 5; ++m) wp[m] = wm[m] = a[m];
+        }
+        for (int m = 0; m < 5; ++m) { Wp[(size_t)m * M3 + c] = wp[m]; Wm[(size_t)m * M3 + c] = wm[m]; }   // sweep order
+      }
+  // P5: flux through the lower d-face of every cell 0..n along d
+  lo[d] = 0; hi[d] = n;
+  for (int k = lo[2]; k <= hi[2]; ++k)
+    for (int j = lo[1]; j <= hi[1]; ++j)
+      for (int i = lo[0]; i <= hi[0]; ++i) {
+        const size_t c = G.cell(i, j, k), cl = c - sd;
+        T WL[5], WR[5], Fr[5];
+        for (int m = 0; m < 5; ++m) { WL[m] = Wp[(size_t)m * M3 + cl]; WR[m] = Wm[(size_t)m * M3 + c]; }
+        riemann_hydro<T>(WL, WR, gamma, solver, Fr, cnt);
+        for (int m = 0; m < 5; ++m) F[(size_t)m * M3 + c] = Fr[m];     // (rho, m_n, m_t1, m_t2, E)
+      }
+  // update (interior), components back in (x, y, z) order
+  for (int m = 0; m < 5; ++m) {
+    const T* u = Uin + G.fld(order[m], p);
+    T* un = Uout + G.fld(order[m], p);
+    const T* f = F.data() + (size_t)m * M3;
+    for (int k = 0; k < n; ++k)
+      for (int j = 0; j < n; ++j)
+        for (int i = 0; i < n; ++i) {
+          const size_t c = G.cell(i, j, k);
+          un[c] = u[c] - lam * (f[c + sd] - f[c]);
+        }
+  }
+  if (cnt)
+    for (int k = 0; k < n; ++k)
+      for (int j = 0; j < n; ++j)
+        for (int i = 0; i < n; ++i)
+          if (!(Uout[G.fld(0, p) + G.cell(i, j, k)] > 0)) cnt[CNT_NEG_STATE]++;
+}
+
 // O7: max over interior cells and directions of |v_d| + c_d
 template <class T>
 double smax_all(const T* U, const Geom& G, T gamma) {
@@ -802,6 +954,38 @@ void oracle_composite_totals(int dtype, const void* Uc, int npc, int n, int g, i
   Geom Gc = make_geom(npc, n, g, nf, originc, domc, nullptr, 0);
   if (dtype == 1) composite_totals<double>((const double*)Uc, Gc, (const double*)Uf, Gf, dx0, out);
   else composite_totals<float>((const float*)Uc, Gc, (const float*)Uf, Gf, dx0, out);
+}
+
+// One PPM sweep (hydro, nf = 5) along direction d of every patch; Uout's ghosts are the caller's.
+int oracle_ppm_sweep(int dtype, const void* Uin, void* Uout, int np, int n, int g, int nf, int d, double dt,
+                     double dx, double gamma, int riemann, long long* counters) {
+  if (nf != 5 || g < 3 || n < 4 || d < 0 || d > 2 || (riemann != RS_HLL && riemann != RS_HLLC)) return -1;
+  Geom G = make_geom(np, n, g, nf, nullptr, nullptr, nullptr, 0);
+  const size_t M3 = G.M3();
+  long long tot[4] = {0, 0, 0, 0};
+  auto run = [&](auto tag) {
+    using T = decltype(tag);
+    const T* in = (const T*)Uin;
+    T* out = (T*)Uout;
+#pragma omp parallel
+    {
+      std::vector<T> W(5 * M3), Wm(5 * M3), Wp(5 * M3), F(5 * M3);
+      long long cnt[4] = {0, 0, 0, 0};
+#pragma omp for schedule(dynamic, 1)
+      for (int p = 0; p < np; ++p)
+        ppm_sweep_patch<T>(in, out, G, p, d, (T)dt, (T)dx, (T)gamma, riemann, W, Wm, Wp, F, cnt);
+#pragma omp critical
+      for (int q = 0; q < 4; ++q) tot[q] += cnt[q];
+    }
+  };
+  if (dtype == 1) run(double(0)); else run(float(0));
+  if (counters) for (int q = 0; q < 4; ++q) counters[q] = tot[q];
+  return 0;
+}
+
+// P1 + P2 of one cell from its five-point stencil (pins of the reconstruction)
+void oracle_ppm_parabola(const double* a5, double* aL, double* aR) {
+  ppm_parabola<double>(a5[0], a5[1], a5[2], a5[3], a5[4], aL, aR);
 }
 
 // Single-face Riemann solvers (fp64) for the pins P7/P8.  nf = 5: hydro; nf = 9: MHD.
