@@ -116,6 +116,18 @@ int amr_mhd_step(amr_patch_batch* b, double dt, double gamma, int limiter, int r
                  double alpha);
 
 /* Sum over interior cells of each field (double accumulation, deterministic).  totals: host [nfields]. */
+/* PPM hydro (SURVEY.md 8(f1); PAPER.md:43 "the Piecewise Parabolic Method, PPM [9]", :76 "the PLM/PPM hydro solver,
+ * have been ported to NVIDIA's CUDA").  Reading R-PPM: Colella & Woodward 1984, direct
+ * Eulerian, dimensionally split, primitive variables, no optional dissipation, HLL | HLLC flux.
+ * amr_hydro_sweep_ppm: ONE sweep along dir (0 = x, 1 = y, 2 = z) over every patch: reads the current state (3 halo
+ * cells along dir gathered through the neighbour table: sibling / periodic / outflow / prolongation halo), writes the
+ * other buffer, swaps.  amr_hydro_step_ppm: the three sweeps of a step, order 0 = x-y-z, 1 = z-y-x (alternate them
+ * step by step).  nfields must be 5, nghost >= 3, n <= 64; the batch must not be linked (no flux registers are
+ * recorded: AMR_ESTATE).  No CFL value is fused: the next amr_cfl_dt runs the standalone reduction.  Event counters
+ * as for amr_hydro_step (a positivity fallback uses the cell-centre state for both traced states). */
+int amr_hydro_sweep_ppm(amr_patch_batch* b, double dt, double gamma, int riemann, int dir);
+int amr_hydro_step_ppm(amr_patch_batch* b, double dt, double gamma, int riemann, int order);
+
 int amr_conserved_totals(amr_patch_batch* b, double* totals);
 
 /* Event counters accumulated since the last call with reset != 0.  counters: host [4] (AMR_CNT_*).

@@ -26,7 +26,8 @@ EXPORTS = (
     "amr_link_destroy", "amr_prolong_ghosts", "amr_flux_clear", "amr_restrict", "amr_reflux", "amr_last_error",
     "amr_version", "amr_builder_bytes", "amr_builder_create", "amr_builder_destroy", "amr_builder_build",
     "amr_builder_results", "amr_builder_gather", "amr_hierarchy_cfl_dt", "amr_hierarchy_step",
-    "amr_flag_blocks", "amr_regrid_bytes", "amr_regrid_fill", "amr_measure_fma_peak",
+    "amr_flag_blocks", "amr_regrid_bytes", "amr_regrid_fill", "amr_measure_fma_peak", "amr_hydro_sweep_ppm",
+    "amr_hydro_step_ppm",
 )
 
 
@@ -97,6 +98,8 @@ def lib():
                                          C.c_double, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int]
         L.amr_builder_gather.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_int64,
                                          C.c_void_p, C.POINTER(C.c_int64)]
+        L.amr_hydro_sweep_ppm.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int]
+        L.amr_hydro_step_ppm.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int]
         L.amr_measure_fma_peak.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         _lib = L
     return _lib
@@ -212,6 +215,12 @@ class PatchBatch:
 
     def hydro_step(self, dt: float, gamma: float, limiter: int, riemann: int):
         _check(lib().amr_hydro_step(self._h, dt, gamma, limiter, riemann))
+
+    def hydro_sweep_ppm(self, dt: float, gamma: float, riemann: int, direction: int):
+        _check(lib().amr_hydro_sweep_ppm(self._h, dt, gamma, riemann, direction))
+
+    def hydro_step_ppm(self, dt: float, gamma: float, riemann: int, order: int = 0):
+        _check(lib().amr_hydro_step_ppm(self._h, dt, gamma, riemann, order))
 
     def mhd_step(self, dt: float, gamma: float, limiter: int, riemann: int, ch: float, alpha: float):
         _check(lib().amr_mhd_step(self._h, dt, gamma, limiter, riemann, ch, alpha))

@@ -18,6 +18,7 @@
 
 #include "../../include/amr_godunov.h"
 #include "amr_internal.hpp"
+#include "ppm_params.hpp"
 
 namespace {
 
@@ -726,6 +727,49 @@ int amr_hydro_step(amr_patch_batch* b, double dt, double gamma, int limiter, int
 
 int amr_mhd_step(amr_patch_batch* b, double dt, double gamma, int limiter, int riemann, double ch, double alpha) {
   return do_step(b, true, dt, gamma, limiter, riemann, ch, alpha);
+}
+
+int amr_hydro_sweep_ppm(amr_patch_batch* b, double dt, double gamma, int riemann, int dir) {
+  if (!b) return fail(AMR_EINVAL, "null batch");
+  DeviceGuard guard(b->device);
+  if (b->d.nfields != 5) return fail(AMR_EINVAL, "PPM is the hydro scheme: the batch has %d fields", b->d.nfields);
+  if (!(dt > 0) || !std::isfinite(dt)) return fail(AMR_EINVAL, "dt must be finite and > 0");
+  if (!std::isfinite(gamma) || !(gamma > 1)) return fail(AMR_EINVAL, "gamma must be finite and > 1");
+  if (riemann != AMR_RS_HLL && riemann != AMR_RS_HLLC) return fail(AMR_EINVAL, "PPM sweep takes HLL or HLLC");
+  if (dir < 0 || dir > 2) return fail(AMR_EINVAL, "dir must be 0 (x), 1 (y) or 2 (z)");
+  if (b->d.nghost < 3) return fail(AMR_EINVAL, "PPM needs nghost >= 3 (reading A11)");
+  if (b->d.n > 64) return fail(AMR_EINVAL, "PPM sweeps are instantiated for n <= 64");
+  if (b->link_up || b->link_down)
+    return fail(AMR_ESTATE, "PPM sweeps record no flux registers: the batch must not be linked");
+  if (b->needs_halo && !b->halo_valid)
+    return fail(AMR_ESTATE, "level-%d batch has coarse-fine halo regions but its halo was never filled", b->d.level);
+  cudaError_t e;
+  if (b->d.dtype == AMR_F32) {
+    amr::ppm::SweepParams<float> P;
+    P.Uin = (const float*)b->U[b->cur]; P.Uout = (float*)b->U[1 - b->cur]; P.halo = (const float*)b->halo;
+    P.nbr = b->nbr_dev; P.counters = b->counters; P.np = b->d.npatch; P.n = b->d.n; P.g = b->d.nghost;
+    P.dtdx = (float)(dt / b->d.dx); P.gamma = (float)gamma; P.gm1 = (float)(gamma - 1); P.igm1 = (float)(1.0 / (gamma - 1));
+    e = amr::launch_ppm_sweep_f32(P, riemann, dir, b->stream);
+  } else {
+    amr::ppm::SweepParams<double> P;
+    P.Uin = (const double*)b->U[b->cur]; P.Uout = (double*)b->U[1 - b->cur]; P.halo = (const double*)b->halo;
+    P.nbr = b->nbr_dev; P.counters = b->counters; P.np = b->d.npatch; P.n = b->d.n; P.g = b->d.nghost;
+    P.dtdx = dt / b->d.dx; P.gamma = gamma; P.gm1 = gamma - 1; P.igm1 = 1.0 / (gamma - 1);
+    e = amr::launch_ppm_sweep_f64(P, riemann, dir, b->stream);
+  }
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "PPM sweep kernel launch: %s", cudaGetErrorString(e));
+  b->cur = 1 - b->cur;
+  b->smax_valid = false;   // the sweeps fuse no CFL reduction: amr_cfl_dt runs the standalone one
+  return AMR_OK;
+}
+
+int amr_hydro_step_ppm(amr_patch_batch* b, double dt, double gamma, int riemann, int order) {
+  if (order != 0 && order != 1) return fail(AMR_EINVAL, "order must be 0 (x-y-z) or 1 (z-y-x)");
+  for (int i = 0; i < 3; ++i) {
+    const int rc = amr_hydro_sweep_ppm(b, dt, gamma, riemann, order ? 2 - i : i);
+    if (rc != AMR_OK) return rc;
+  }
+  return AMR_OK;
 }
 
 int amr_conserved_totals(amr_patch_batch* b, double* totals) {

@@ -34,6 +34,22 @@ def gpu_advance(level, wl, nsteps, np_dtype=np.float64, dt_fixed=None, limiter=N
     return dict(U=b.download(), dts=dts, smaxs=smaxs, counters=b.step_counters(), batch=b)
 
 
+def gpu_ppm_advance(level, wl, nsteps, np_dtype=np.float64, dt_fixed=None, riemann=None):
+    """PPM in the order of oracle.api.ppm_advance: amr_cfl_dt -> dt, then amr_hydro_step_ppm with the sweep order
+    x-y-z on even steps, z-y-x on odd steps (the halo is gathered inside every sweep)."""
+    b = amr.PatchBatch.from_level(level, gpu_dtype(np_dtype))
+    rs = wl.riemann if riemann is None else riemann
+    dts, smaxs = [], []
+    for step_no in range(nsteps):
+        dt, sm = b.cfl_dt(wl.gamma, wl.cfl)
+        if dt_fixed is not None:
+            dt = dt_fixed
+        b.hydro_step_ppm(dt, wl.gamma, rs, step_no % 2)
+        dts.append(dt)
+        smaxs.append(sm)
+    return dict(U=b.download(), dts=dts, smaxs=smaxs, counters=b.step_counters(), batch=b)
+
+
 def gpu_two_level_step(wl, np_dtype=np.float64, do_reflux=True):
     """O9 in the order of oracle.api.two_level_step."""
     lc, lf = wl.levels
