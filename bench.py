@@ -2,7 +2,7 @@
 """Benchmark of the per-patch Godunov hydro/MHD update (BASELINE.json metric: cell-updates/s and % of
 the HBM roofline).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config5|config3_f32|config3_f64|config2]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config5|config3_f32|config3_f64|config2|hydro_f32|hydro_ppm_f32|...]
   python bench.py --impl reference ...      # the CPU oracle on the host cores (the tier's reference arm)
 
 A "step" is one pass of the whole hot path over the batch: amr_cfl_dt (O7, fused into the previous
@@ -47,7 +47,7 @@ UNIT = "cell-updates/s"
 BYTES_PER_CELL = {("hydro", "f32"): 40, ("hydro", "f64"): 80, ("mhd", "f32"): 72, ("mhd", "f64"): 144}
 # algorithmic floating-point operations per cell-update (add/sub/mul/min/max/abs/compare = 1,
 # fma = 2, div and sqrt = 1; each face once, no halo recomputation), MC limiter, HLLC / HLLD+GLM
-FLOPS_PER_CELL = {"hydro": 600, "mhd": 1700}
+FLOPS_PER_CELL = {"hydro": 600, "mhd": 1700, "hydro_ppm": 1200}   # PPM: ~400 per cell and sweep (5 parabolas, tracing, HLLC), +-20 %
 
 
 def peaks():
@@ -167,6 +167,20 @@ def build_workload(name: str, device, size: int | None):
         return dict(U=host, origin=origin, n=32, dx=1.0 / N, domain=(N, N, N), mhd=False, dtype=name[-3:], gamma=5.0 / 3.0,
                     limiter=wk.configs.LIM_MC, riemann=wk.configs.RS_HLLC, cfl=0.3, alpha=0.0,
                     label="hydro: %d^3 cells, %d patches of 32^3, Mach-3 turbulence (config-5 recipe without B), hydro %s, MC+HLLC" % (N, origin.shape[0], name[-3:]))
+    if name in ("hydro_ppm_f32", "hydro_ppm_f64"):
+        # the next row of the scope table: the same gas as hydro_f32 (config-5 recipe without B,
+        # Mach-1 here: PPM is run without CW84's optional flattening), advanced with the split PPM sweeps (HLLC)
+        N = size or (512 if name.endswith("f32") else 256)
+        U, origin = wk.turbulence_patches_torch(N, 32, device, mach=1.0)
+        U[4] -= 0.5 * (U[5] ** 2 + U[6] ** 2 + U[7] ** 2)
+        dt = torch.float32 if name.endswith("f32") else torch.float64
+        host = torch.empty((5,) + tuple(U.shape[1:]), dtype=dt, pin_memory=True)
+        host.copy_(U[:5])
+        del U
+        torch.cuda.empty_cache()
+        return dict(U=host, origin=origin, n=32, dx=1.0 / N, domain=(N, N, N), mhd=False, dtype=name[-3:], gamma=5.0 / 3.0,
+                    limiter=wk.configs.LIM_MC, riemann=wk.configs.RS_HLLC, cfl=0.3, alpha=0.0, scheme="ppm",
+                    label="hydro PPM: %d^3 cells, %d patches of 32^3, Mach-1 turbulence (config-5 recipe without B), hydro %s, PPM + HLLC, 3 sweeps per step" % (N, origin.shape[0], name[-3:]))
     if name in ("config3_f32", "config3_f64"):
         N = size or 256
         w = wk.config3_orszag_tang(N=N)
@@ -199,6 +213,10 @@ def make_batch(W, device):
 
 def one_step(b, W):
     dt, sm = b.cfl_dt(W["gamma"], W["cfl"])
+    if W.get("scheme") == "ppm":
+        W["_step_no"] = W.get("_step_no", 0) + 1
+        b.hydro_step_ppm(dt, W["gamma"], W["riemann"], (W["_step_no"] - 1) % 2)
+        return dt, sm
     if W["mhd"]:
         b.mhd_step(dt, W["gamma"], W["limiter"], W["riemann"], sm, W["alpha"])
     else:
@@ -278,7 +296,24 @@ def parity_gate(b, W, nsample: int = 8):
     rng = np.random.default_rng([wk.SEED, 2, npatch])
     ids = sorted(int(i) for i in rng.choice(npatch, size=min(nsample, npatch), replace=False))
     wl = dict(gamma=W["gamma"], limiter=W["limiter"], riemann=W["riemann"], alpha=W["alpha"])
-    if W.get("self_periodic"):
+    if W.get("scheme") == "ppm":
+        # three sweeps with the ghost cells refilled before each: the whole 3x3x3 mini-level is swept (what enters
+        # from beyond it travels 3 cells per sweep and never reaches the centre patch)
+        order = oracle.PPM_ORDERS[(W["_step_no"] - 1) % 2]
+        n = W["n"]
+        where = {tuple(int(v) for v in o): i for i, o in enumerate(np.asarray(W["origin"]))}
+        dom = np.asarray(W["domain"])
+        mini = np.array([[i * n, j * n, k * n] for k in range(3) for j in range(3) for i in range(3)], np.int32)
+        errs = []
+        for s_ in ids:
+            o = np.asarray(W["origin"][s_])
+            sel = [where[tuple(int(v) for v in (o + (mo - n)) % dom)] for mo in mini]
+            Ug = oracle.ghosted(np.ascontiguousarray(U0[:, sel]).astype(np.float64), 3)
+            for d in order:
+                oracle.fill_ghosts(Ug, 3, mini, (3 * n,) * 3, (0,) * 6, False)
+                Ug = oracle.ppm_sweep(Ug, 3, d, dt, W["dx"], W["gamma"], W["riemann"])["U"]
+            errs.append(H.rel_err(np.asarray(U1[:, s_:s_ + 1], np.float64), oracle.interior(Ug, 3)[:, 13:14]))
+    elif W.get("self_periodic"):
         errs = []
         for s_ in ids:
             Um = np.ascontiguousarray(U0[:, s_:s_ + 1]).astype(np.float64)
@@ -311,7 +346,10 @@ def timed_regions(b, W, K: int, repeats: int, dist, device):
         for i in range(K):
             dt, sm = b.cfl_dt(W["gamma"], W["cfl"])          # fused smax of the previous step: 8-byte D->H
             ev0[i].record()
-            if W["mhd"]:
+            if W.get("scheme") == "ppm":
+                W["_step_no"] = W.get("_step_no", 0) + 1
+                b.hydro_step_ppm(dt, W["gamma"], W["riemann"], (W["_step_no"] - 1) % 2)
+            elif W["mhd"]:
                 b.mhd_step(dt, W["gamma"], W["limiter"], W["riemann"], sm, W["alpha"])
             else:
                 b.hydro_step(dt, W["gamma"], W["limiter"], W["riemann"])
@@ -648,8 +686,10 @@ def main():
 
     def roofline_of(kind_, dtype_, n_, ncells_, kms, workload_for_traffic):
         bpc_ = BYTES_PER_CELL[(kind_, dtype_)]
-        ach = bpc_ * ncells_ / (kms * 1e-3) / 1e9
         kname = ("x2::godunov_step_x2_kernel" if dtype_ == "f32" else "d1::godunov_step_d1_kernel") if n_ % 16 == 0 else "godunov_step_kernel"
+        if workload_for_traffic is not None and str(workload_for_traffic).startswith("hydro_ppm"):
+            bpc_, kname = 3 * bpc_, "ppm::ppm_sweep_kernel (three launches per step: every value read and written once per sweep)"
+        ach = bpc_ * ncells_ / (kms * 1e-3) / 1e9
         traffic, traffic_src = dram_traffic(workload_for_traffic)
         return dict(bound="hbm", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s", frac=ach / pk["hbm_gbs"],
                     traffic=traffic, traffic_unit="bytes per launch (dram read + write, ncu --set full)",
@@ -657,7 +697,8 @@ def main():
                     kernel_ms_how="median of the %d x %d per-step CUDA-event times" % (R, K),
                     bytes_per_cell=bpc_, frac_of_nominal_8TBs=ach / 8000.0)
 
-    roof = roofline_of(kind, W["dtype"], W["n"], ncells, kern_med, args.workload if args.size is None else None)
+    roof = roofline_of(kind, W["dtype"], W["n"], ncells, kern_med,
+                       args.workload if (args.size is None or W.get("scheme") == "ppm") else None)
     # ALU roofline against the FMA rate MEASURED in this run (amr_measure_fma_peak: dependent-FMA chains on every SM)
     lanes = 128 if W["dtype"] == "f32" else 64
     nominal = 148 * lanes * pk["sm_max_mhz"] * 1e6 * 2 / 1e12          # TFLOP/s, fma = 2
@@ -666,9 +707,10 @@ def main():
         alu_src = "measured in this run: amr_measure_fma_peak, ~2 ms of dependent-FMA chains on every SM"
     except Exception as exc:  # noqa: BLE001  (the bench line must still be printed)
         alu_peak, alu_src = nominal, "nominal (measurement failed: %s)" % exc
-    alu_ach = FLOPS_PER_CELL[kind] * ncells / (kern_med * 1e-3) / 1e12
+    fkind = "hydro_ppm" if W.get("scheme") == "ppm" else kind
+    alu_ach = FLOPS_PER_CELL[fkind] * ncells / (kern_med * 1e-3) / 1e12
     alu = dict(bound="alu", achieved=alu_ach, peak=alu_peak, unit="TFLOP/s", frac=alu_ach / alu_peak,
-               flops_per_cell=FLOPS_PER_CELL[kind], peak_source=alu_src,
+               flops_per_cell=FLOPS_PER_CELL[fkind], peak_source=alu_src,
                nominal_peak=nominal, nominal_how="148 SMs x %d %s lanes x 2 (fma) x sm_max_mhz" % (lanes, W["dtype"]))
 
     # the 256^3 half of north_star's target, timed in the same run (not part of the headline value)
@@ -702,7 +744,8 @@ def main():
                ms_per_step_regions=regions, higher_is_better=True, scaling="weak", vs_baseline=None, dtype=W["dtype"], data="synthetic",
                config=dict(workload=W["label"], physics=kind, cells_per_gpu=ncells, l2="state %.2f GB per buffer >> 126 MB L2, no flush needed" % (ncells * bpc / 2 / 1e9),
                            parallelism="replicas only (no sharding)" if world > 1 else "single GPU",
-                           step="amr_cfl_dt (fused smax, 8-byte D2H) + amr_%s_step" % kind,
+                           step=("amr_cfl_dt (standalone smax reduction) + amr_hydro_step_ppm (x-y-z / z-y-x sweeps, alternating)" if W.get("scheme") == "ppm"
+                                 else "amr_cfl_dt (fused smax, 8-byte D2H) + amr_%s_step" % kind),
                            timing="median of %d regions of exactly %d steps each (CUDA events, barrier + synchronize around every region)" % (R, K)),
                roofline=roof, alu_roofline=alu, also=also, cpu_baseline=cpu, e2e=e2e, gpu_launches=K, gpu_launches_all_regions=K * R,
                clocks=clocks, state_ok=state_ok, parity_ok=parity_ok, parity=parity, counters=counters)
