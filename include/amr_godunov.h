@@ -69,6 +69,9 @@ typedef struct {
   int32_t domain_cells[3]; /* extent of this level's index space (multiples of n) */
   int32_t bc[6];           /* xlo,xhi,ylo,yhi,zlo,zhi: AMR_BC_* */
   int32_t self_periodic;   /* 1: every patch is its own periodic neighbour (config 2); origin ignored */
+  int32_t nactive;         /* 0 = npatch.  Sharding over GPUs: only the first
+                              nactive patches are OWNED - stepped, reduced (smax, totals) - the patches behind them are
+                              read-only copies of remote patches (halo sources), refreshed by amr_patch_batch_import */
 } amr_batch_desc;
 
 /* Bytes of device arena amr_patch_batch_create needs for this desc (0 on an invalid desc). */
@@ -116,6 +119,16 @@ int amr_mhd_step(amr_patch_batch* b, double dt, double gamma, int limiter, int r
                  double alpha);
 
 /* Sum over interior cells of each field (double accumulation, deterministic).  totals: host [nfields]. */
+/* Halo exchange of a level sharded over GPUs (SURVEY.md 8(f4); PAPER.md:70 "16 GPUs", :72 "one GPU per computing
+ * node ... communicating through the network").  dev_pairs: DEVICE, int32 [count][2] =
+ * (slot in the packed array, patch index in the batch), borrowed for the call.
+ * amr_patch_batch_export copies the CURRENT state of the listed patches into dev_packed[field][count][n^3] (what a
+ * rank sends); amr_patch_batch_import copies dev_packed[field][count][n^3] into the listed patches of the current
+ * state (what a rank receives into its read-only copies; the fused smax stays valid: it covers owned patches only).
+ * Both only enqueue on the batch's stream. */
+int amr_patch_batch_export(amr_patch_batch* b, const int32_t* dev_pairs, int32_t count, void* dev_packed);
+int amr_patch_batch_import(amr_patch_batch* b, const int32_t* dev_pairs, int32_t count, const void* dev_packed);
+
 /* PPM hydro (SURVEY.md 8(f1); PAPER.md:43 "the Piecewise Parabolic Method, PPM [9]", :76 "the PLM/PPM hydro solver,
  * have been ported to NVIDIA's CUDA").  Reading R-PPM: Colella & Woodward 1984, direct
  * Eulerian, dimensionally split, primitive variables, no optional dissipation, HLL | HLLC flux.

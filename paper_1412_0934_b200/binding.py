@@ -27,7 +27,7 @@ EXPORTS = (
     "amr_version", "amr_builder_bytes", "amr_builder_create", "amr_builder_destroy", "amr_builder_build",
     "amr_builder_results", "amr_builder_gather", "amr_hierarchy_cfl_dt", "amr_hierarchy_step",
     "amr_flag_blocks", "amr_regrid_bytes", "amr_regrid_fill", "amr_measure_fma_peak", "amr_hydro_sweep_ppm",
-    "amr_hydro_step_ppm",
+    "amr_hydro_step_ppm", "amr_patch_batch_export", "amr_patch_batch_import",
 )
 
 
@@ -40,7 +40,8 @@ class AmrError(RuntimeError):
 class _Desc(C.Structure):
     _fields_ = [("npatch", C.c_int32), ("n", C.c_int32), ("nghost", C.c_int32), ("nfields", C.c_int32),
                 ("dtype", C.c_int32), ("level", C.c_int32), ("dx", C.c_double), ("origin", C.c_void_p),
-                ("domain_cells", C.c_int32 * 3), ("bc", C.c_int32 * 6), ("self_periodic", C.c_int32)]
+                ("domain_cells", C.c_int32 * 3), ("bc", C.c_int32 * 6), ("self_periodic", C.c_int32),
+                ("nactive", C.c_int32)]
 
 
 _lib = None
@@ -100,6 +101,8 @@ def lib():
                                          C.c_void_p, C.POINTER(C.c_int64)]
         L.amr_hydro_sweep_ppm.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int]
         L.amr_hydro_step_ppm.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int]
+        L.amr_patch_batch_export.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
+        L.amr_patch_batch_import.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p]
         L.amr_measure_fma_peak.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         _lib = L
     return _lib
@@ -139,7 +142,8 @@ class PatchBatch:
 
     def __init__(self, npatch: int, n: int, nfields: int, dtype: int, dx: float, origin=None,
                  domain_cells: Sequence[int] = (0, 0, 0), bc: Sequence[int] = (0,) * 6, self_periodic: bool = False,
-                 nghost: int = 3, level: int = 0, device: str = "cuda:0", stream: Optional[int] = None):
+                 nghost: int = 3, level: int = 0, device: str = "cuda:0", stream: Optional[int] = None,
+                 nactive: int = 0):
         import torch  # device memory + stream only
         self._torch = torch
         L = lib()
@@ -154,6 +158,8 @@ class PatchBatch:
         d.domain_cells[:] = [int(v) for v in domain_cells]
         d.bc[:] = [int(v) for v in bc]
         d.self_periodic = int(bool(self_periodic))
+        d.nactive = int(nactive)
+        self.nactive = int(nactive) if nactive else int(npatch)
         self.npatch, self.n, self.nghost, self.nfields, self.dtype, self.dx, self.level = npatch, n, nghost, nfields, dtype, dx, level
         nbytes = L.amr_patch_batch_bytes(C.byref(d))
         if nbytes == 0:
@@ -201,6 +207,14 @@ class PatchBatch:
             out = np.empty(self._shape(with_ghosts), dtype=self.np_dtype)
         _check(lib().amr_patch_batch_download(self._h, _host_ptr(out), int(with_ghosts)))
         return out
+
+    def export_patches(self, dev_pairs, count: int, dev_packed):
+        """amr_patch_batch_export: dev_pairs int32 [count, 2] = (slot, patch), dev_packed [nfields, count, n^3]
+        (device tensors)."""
+        _check(lib().amr_patch_batch_export(self._h, dev_pairs.data_ptr(), int(count), dev_packed.data_ptr()))
+
+    def import_patches(self, dev_pairs, count: int, dev_packed):
+        _check(lib().amr_patch_batch_import(self._h, dev_pairs.data_ptr(), int(count), dev_packed.data_ptr()))
 
     def state_ptr(self, which: int = 0) -> int:
         return int(lib().amr_patch_batch_state(self._h, which))

@@ -26,7 +26,8 @@ struct StepParams {
   const int* fblk_of;  // device, [np] block index or -1 (nullptr if fblk is)
   unsigned long long* counters;  // device [4]
   void* smax;          // device, one T-sized slot (bit pattern ordered as unsigned), pre-zeroed
-  int np, n, g;
+  int np, n, g;        // np = patches in the arena (strides); the grid covers the first np_active of them
+  int np_active;
   int ntx, nty, ntz, zc;  // tiles per patch along x,y,z; planes per z-chunk
   T dtdx;              // dt/dx
   T hdtdx;             // dt/(2 dx)
@@ -61,10 +62,10 @@ inline cudaError_t ensure_dynamic_smem(const void* kern, int bytes, std::atomic<
 }
 
 // aux kernels (aux_kernels.cu); dtype: 0 = f32, 1 = f64
-cudaError_t launch_smax(int dtype, const void* U, int nf, int np, int n, double gamma, void* smax_slot,
+cudaError_t launch_smax(int dtype, const void* U, int nf, int np, int np_active, int n, double gamma, void* smax_slot,
                         cudaStream_t s);
 constexpr int TOTALS_BLOCKS = 256;
-cudaError_t launch_totals(int dtype, const void* U, int nf, int np, int n, double* partials /*[nf][TOTALS_BLOCKS]*/,
+cudaError_t launch_totals(int dtype, const void* U, int nf, int np, int np_active, int n, double* partials /*[nf][TOTALS_BLOCKS]*/,
                           cudaStream_t s);
 // interiors [nf][np][n^3] (device) -> ghosted [nf][npc][(n+2g)^3] (device) for patches [p0, p0+npc)
 cudaError_t launch_gather_ghosted(int dtype, const void* U, const void* halo, const int* nbr, int nf, int np,
@@ -93,6 +94,8 @@ cudaError_t launch_flag_blocks(int dtype, const void* Ufield, int np, int n, dou
                                cudaStream_t s);
 cudaError_t launch_copy_patches(int dtype, void* Unew, size_t fs_new, const void* Uold, size_t fs_old, const void* pairs,
                                 int npairs, int nf, int n, cudaStream_t s);
+cudaError_t launch_copy_patches_in(int dtype, void* U, size_t fs, const void* packed, size_t fs_packed, const void* pairs,
+                                   int npairs, int nf, int n, cudaStream_t s);
 cudaError_t launch_prolong_patches(int dtype, void* Unew, size_t fs_new, int nf, int n, const int* born, const long long* c7,
                                    int nparents, const void* Uc, size_t fs_c, cudaStream_t s);
 

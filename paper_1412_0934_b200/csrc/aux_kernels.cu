@@ -20,13 +20,13 @@ template <> __device__ __forceinline__ void atomic_max_slot<double>(void* slot, 
 
 // ---- O7 standalone: grid-stride over interior cells, warp-shuffle max, one atomic per CTA ----------
 template <class T, int NF>
-__global__ void __launch_bounds__(256) smax_kernel(const T* __restrict__ U, size_t ncell, T gamma, T gm1,
+__global__ void __launch_bounds__(256) smax_kernel(const T* __restrict__ U, size_t ncell, size_t fstride, T gamma, T gm1,
                                                    void* slot) {
   T m = T(0);
   for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < ncell; c += (size_t)gridDim.x * blockDim.x) {
     T u[NF];
 #pragma unroll
-    for (int q = 0; q < NF; ++q) u[q] = __ldg(U + (size_t)q * ncell + c);
+    for (int q = 0; q < NF; ++q) u[q] = __ldg(U + (size_t)q * fstride + c);
     m = max_(m, signal_speed<T, NF>(u, gamma, gm1));
   }
 #pragma unroll
@@ -43,9 +43,9 @@ __global__ void __launch_bounds__(256) smax_kernel(const T* __restrict__ U, size
 
 // ---- conserved totals: fixed grid, fixed per-thread order, tree reduce -> deterministic ------------
 template <class T>
-__global__ void __launch_bounds__(256) totals_kernel(const T* __restrict__ U, size_t ncell, double* partials) {
+__global__ void __launch_bounds__(256) totals_kernel(const T* __restrict__ U, size_t ncell, size_t fstride, double* partials) {
   const int q = blockIdx.y;
-  const T* u = U + (size_t)q * ncell;
+  const T* u = U + (size_t)q * fstride;
   double s = 0.0;
   for (size_t c = (size_t)blockIdx.x * 256 + threadIdx.x; c < ncell; c += (size_t)gridDim.x * 256) s += (double)u[c];
   __shared__ double red[256];
@@ -316,26 +316,26 @@ inline unsigned grid_for(size_t work, int block, unsigned cap = 148 * 16) {
 
 }  // namespace
 
-cudaError_t launch_smax(int dtype, const void* U, int nf, int np, int n, double gamma, void* slot, cudaStream_t s) {
-  const size_t ncell = (size_t)np * n * n * n;
+cudaError_t launch_smax(int dtype, const void* U, int nf, int np, int np_active, int n, double gamma, void* slot, cudaStream_t s) {
+  const size_t ncell = (size_t)np_active * n * n * n, fstride = (size_t)np * n * n * n;
   const unsigned grid = grid_for(ncell, 256, 148 * 8);
   if (dtype == 0) {
     const float g = (float)gamma, gm1 = (float)(gamma - 1.0);
-    if (nf == 5) smax_kernel<float, 5><<<grid, 256, 0, s>>>((const float*)U, ncell, g, gm1, slot);
-    else smax_kernel<float, 9><<<grid, 256, 0, s>>>((const float*)U, ncell, g, gm1, slot);
+    if (nf == 5) smax_kernel<float, 5><<<grid, 256, 0, s>>>((const float*)U, ncell, fstride, g, gm1, slot);
+    else smax_kernel<float, 9><<<grid, 256, 0, s>>>((const float*)U, ncell, fstride, g, gm1, slot);
   } else {
     const double g = gamma, gm1 = gamma - 1.0;
-    if (nf == 5) smax_kernel<double, 5><<<grid, 256, 0, s>>>((const double*)U, ncell, g, gm1, slot);
-    else smax_kernel<double, 9><<<grid, 256, 0, s>>>((const double*)U, ncell, g, gm1, slot);
+    if (nf == 5) smax_kernel<double, 5><<<grid, 256, 0, s>>>((const double*)U, ncell, fstride, g, gm1, slot);
+    else smax_kernel<double, 9><<<grid, 256, 0, s>>>((const double*)U, ncell, fstride, g, gm1, slot);
   }
   return cudaGetLastError();
 }
 
-cudaError_t launch_totals(int dtype, const void* U, int nf, int np, int n, double* partials, cudaStream_t s) {
-  const size_t ncell = (size_t)np * n * n * n;
+cudaError_t launch_totals(int dtype, const void* U, int nf, int np, int np_active, int n, double* partials, cudaStream_t s) {
+  const size_t ncell = (size_t)np_active * n * n * n, fstride = (size_t)np * n * n * n;
   dim3 grid(TOTALS_BLOCKS, nf);
-  if (dtype == 0) totals_kernel<float><<<grid, 256, 0, s>>>((const float*)U, ncell, partials);
-  else totals_kernel<double><<<grid, 256, 0, s>>>((const double*)U, ncell, partials);
+  if (dtype == 0) totals_kernel<float><<<grid, 256, 0, s>>>((const float*)U, ncell, fstride, partials);
+  else totals_kernel<double><<<grid, 256, 0, s>>>((const double*)U, ncell, fstride, partials);
   return cudaGetLastError();
 }
 
@@ -461,6 +461,26 @@ cudaError_t launch_copy_patches(int dtype, void* Unew, size_t fs_new, const void
   const int n3 = n * n * n;
   if (dtype == 0) copy_patches_kernel<float><<<grid, 256, 0, s>>>((float*)Unew, fs_new, (const float*)Uold, fs_old, (const int2*)pairs, n3);
   else copy_patches_kernel<double><<<grid, 256, 0, s>>>((double*)Unew, fs_new, (const double*)Uold, fs_old, (const int2*)pairs, n3);
+  return cudaGetLastError();
+}
+
+// the same copy with the roles of the pair swapped: pairs[e] = (slot in the packed source, patch in the destination)
+template <class T>
+__global__ void __launch_bounds__(256) copy_patches_in_kernel(T* __restrict__ U, size_t fs, const T* __restrict__ packed,
+                                                              size_t fs_packed, const int2* __restrict__ pairs, int n3) {
+  const int2 pr = pairs[blockIdx.x];
+  const T* src = packed + (size_t)blockIdx.y * fs_packed + (size_t)pr.x * n3;
+  T* dst = U + (size_t)blockIdx.y * fs + (size_t)pr.y * n3;
+  for (int r = threadIdx.x; r < n3; r += blockDim.x) dst[r] = src[r];
+}
+
+cudaError_t launch_copy_patches_in(int dtype, void* U, size_t fs, const void* packed, size_t fs_packed, const void* pairs,
+                                   int npairs, int nf, int n, cudaStream_t s) {
+  if (npairs == 0) return cudaSuccess;
+  const dim3 grid((unsigned)npairs, (unsigned)nf);
+  const int n3 = n * n * n;
+  if (dtype == 0) copy_patches_in_kernel<float><<<grid, 256, 0, s>>>((float*)U, fs, (const float*)packed, fs_packed, (const int2*)pairs, n3);
+  else copy_patches_in_kernel<double><<<grid, 256, 0, s>>>((double*)U, fs, (const double*)packed, fs_packed, (const int2*)pairs, n3);
   return cudaGetLastError();
 }
 

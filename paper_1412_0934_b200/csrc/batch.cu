@@ -58,6 +58,7 @@ bool desc_ok(const amr_batch_desc* d, std::string* why) {
   if (d->dtype != AMR_F32 && d->dtype != AMR_F64) return bad("dtype must be AMR_F32 or AMR_F64");
   if (!(d->dx > 0) || !std::isfinite(d->dx)) return bad("dx must be finite and > 0");
   if (d->level < 0) return bad("level < 0");
+  if (d->nactive < 0 || d->nactive > d->npatch) return bad("nactive must be in [0, npatch]");
   {  // the step kernel keeps per-field element offsets (interiors and ghosted halo buffer) in 32 bits
     const double M = d->n + 2.0 * d->nghost;
     if ((double)d->npatch * M * M * M > 2.0e9) return bad("more than 2e9 (ghosted) cells in one batch");
@@ -118,6 +119,7 @@ struct amr_patch_batch {
   std::vector<int> nbr_host;
   PatchMap map;
   cudaStream_t stream;
+  int nactive;       // the first nactive patches are stepped / reduced; the rest are read-only copies of remote patches (sharding)
   int device;        // the device the arena lives on (recorded at create; every call runs with it current)
   char* arena;
   size_t bytes, esz, n3, M3;
@@ -380,6 +382,7 @@ amr::StepParams<T> make_params(amr_patch_batch* b, double dt, double gamma, doub
   P.counters = b->counters;
   P.smax = b->smax_slot;
   P.np = b->d.npatch;
+  P.np_active = b->nactive;
   P.n = b->d.n;
   P.g = b->d.nghost;
   const T dtT = (T)dt, dxT = (T)b->d.dx;
@@ -508,6 +511,8 @@ int amr_patch_batch_create(const amr_batch_desc* desc, void* dev_arena, size_t b
   b->d = *desc;
   b->d.origin = nullptr;
   const int np = desc->npatch, n = desc->n;
+  const int nactive = desc->nactive > 0 ? desc->nactive : np;
+  b->nactive = nactive;
   b->origin.assign((size_t)np * 3, 0);
   if (desc->self_periodic) {
     for (int a = 0; a < 3; ++a) b->d.domain_cells[a] = n;
@@ -555,6 +560,7 @@ int amr_patch_batch_create(const amr_batch_desc* desc, void* dev_arena, size_t b
         const int src = m.at(q[0], q[1], q[2]);
         int e;
         if (src >= 0) e = src | (mode << amr::NBR_MODE_SHIFT);
+        else if (p >= nactive) e = p;   // a read-only copy of a remote patch is never stepped: its halo is never gathered
         else if (desc->level > 0) { e = amr::NBR_FROM_HALO; b->needs_halo = true; }
         else { delete b; return fail(AMR_EINVAL, "root-level patch %d has no neighbour in region %d", p, r); }
         b->nbr_host[(size_t)p * 27 + r] = e;
@@ -701,7 +707,7 @@ int amr_cfl_dt(amr_patch_batch* b, double gamma, double cfl, int mhd, double* dt
   if (!(cfl > 0) || !std::isfinite(cfl)) return fail(AMR_EINVAL, "cfl must be finite and > 0");
   if (!(b->smax_valid && b->smax_gamma == gamma)) {
     CUDA_TRY(cudaMemsetAsync(b->smax_slot, 0, 16, b->stream));
-    cudaError_t e = amr::launch_smax(b->d.dtype, b->U[b->cur], b->d.nfields, b->d.npatch, b->d.n, gamma, b->smax_slot, b->stream);
+    cudaError_t e = amr::launch_smax(b->d.dtype, b->U[b->cur], b->d.nfields, b->d.npatch, b->nactive, b->d.n, gamma, b->smax_slot, b->stream);
     if (e != cudaSuccess) return fail(AMR_ECUDA, "smax kernel launch: %s", cudaGetErrorString(e));
     b->smax_valid = true;
     b->smax_gamma = gamma;
@@ -729,6 +735,26 @@ int amr_mhd_step(amr_patch_batch* b, double dt, double gamma, int limiter, int r
   return do_step(b, true, dt, gamma, limiter, riemann, ch, alpha);
 }
 
+int amr_patch_batch_export(amr_patch_batch* b, const int32_t* dev_pairs, int32_t count, void* dev_packed) {
+  if (!b || (count > 0 && (!dev_pairs || !dev_packed))) return fail(AMR_EINVAL, "null pointer");
+  if (count < 0) return fail(AMR_EINVAL, "count < 0");
+  DeviceGuard guard(b->device);
+  cudaError_t e = amr::launch_copy_patches(b->d.dtype, dev_packed, (size_t)count * b->n3, b->U[b->cur],
+                                           (size_t)b->d.npatch * b->n3, dev_pairs, count, b->d.nfields, b->d.n, b->stream);
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "export kernel launch: %s", cudaGetErrorString(e));
+  return AMR_OK;
+}
+
+int amr_patch_batch_import(amr_patch_batch* b, const int32_t* dev_pairs, int32_t count, const void* dev_packed) {
+  if (!b || (count > 0 && (!dev_pairs || !dev_packed))) return fail(AMR_EINVAL, "null pointer");
+  if (count < 0) return fail(AMR_EINVAL, "count < 0");
+  DeviceGuard guard(b->device);
+  cudaError_t e = amr::launch_copy_patches_in(b->d.dtype, b->U[b->cur], (size_t)b->d.npatch * b->n3, dev_packed,
+                                              (size_t)count * b->n3, dev_pairs, count, b->d.nfields, b->d.n, b->stream);
+  if (e != cudaSuccess) return fail(AMR_ECUDA, "import kernel launch: %s", cudaGetErrorString(e));
+  return AMR_OK;
+}
+
 int amr_hydro_sweep_ppm(amr_patch_batch* b, double dt, double gamma, int riemann, int dir) {
   if (!b) return fail(AMR_EINVAL, "null batch");
   DeviceGuard guard(b->device);
@@ -747,13 +773,13 @@ int amr_hydro_sweep_ppm(amr_patch_batch* b, double dt, double gamma, int riemann
   if (b->d.dtype == AMR_F32) {
     amr::ppm::SweepParams<float> P;
     P.Uin = (const float*)b->U[b->cur]; P.Uout = (float*)b->U[1 - b->cur]; P.halo = (const float*)b->halo;
-    P.nbr = b->nbr_dev; P.counters = b->counters; P.np = b->d.npatch; P.n = b->d.n; P.g = b->d.nghost;
+    P.nbr = b->nbr_dev; P.counters = b->counters; P.np = b->d.npatch; P.np_active = b->nactive; P.n = b->d.n; P.g = b->d.nghost;
     P.dtdx = (float)(dt / b->d.dx); P.gamma = (float)gamma; P.gm1 = (float)(gamma - 1); P.igm1 = (float)(1.0 / (gamma - 1));
     e = amr::launch_ppm_sweep_f32(P, riemann, dir, b->stream);
   } else {
     amr::ppm::SweepParams<double> P;
     P.Uin = (const double*)b->U[b->cur]; P.Uout = (double*)b->U[1 - b->cur]; P.halo = (const double*)b->halo;
-    P.nbr = b->nbr_dev; P.counters = b->counters; P.np = b->d.npatch; P.n = b->d.n; P.g = b->d.nghost;
+    P.nbr = b->nbr_dev; P.counters = b->counters; P.np = b->d.npatch; P.np_active = b->nactive; P.n = b->d.n; P.g = b->d.nghost;
     P.dtdx = dt / b->d.dx; P.gamma = gamma; P.gm1 = gamma - 1; P.igm1 = 1.0 / (gamma - 1);
     e = amr::launch_ppm_sweep_f64(P, riemann, dir, b->stream);
   }
@@ -776,7 +802,7 @@ int amr_conserved_totals(amr_patch_batch* b, double* totals) {
   if (!b || !totals) return fail(AMR_EINVAL, "null pointer");
   DeviceGuard guard(b->device);
   const int nf = b->d.nfields;
-  cudaError_t e = amr::launch_totals(b->d.dtype, b->U[b->cur], nf, b->d.npatch, b->d.n, b->partials, b->stream);
+  cudaError_t e = amr::launch_totals(b->d.dtype, b->U[b->cur], nf, b->d.npatch, b->nactive, b->d.n, b->partials, b->stream);
   if (e != cudaSuccess) return fail(AMR_ECUDA, "totals kernel launch: %s", cudaGetErrorString(e));
   std::vector<double> h((size_t)nf * amr::TOTALS_BLOCKS);
   CUDA_TRY(cudaMemcpyAsync(h.data(), b->partials, h.size() * sizeof(double), cudaMemcpyDeviceToHost, b->stream));
@@ -1054,7 +1080,7 @@ int amr_hierarchy_cfl_dt(amr_patch_batch* const* levels, int nlevels, double gam
     if ((mhd != 0) != (b->d.nfields == 9)) return fail(AMR_EINVAL, "mhd flag does not match nfields = %d", b->d.nfields);
     if (!(b->smax_valid && b->smax_gamma == gamma)) {
       CUDA_TRY(cudaMemsetAsync(b->smax_slot, 0, 16, b->stream));
-      cudaError_t e = amr::launch_smax(b->d.dtype, b->U[b->cur], b->d.nfields, b->d.npatch, b->d.n, gamma, b->smax_slot, b->stream);
+      cudaError_t e = amr::launch_smax(b->d.dtype, b->U[b->cur], b->d.nfields, b->d.npatch, b->nactive, b->d.n, gamma, b->smax_slot, b->stream);
       if (e != cudaSuccess) return fail(AMR_ECUDA, "smax kernel launch: %s", cudaGetErrorString(e));
       b->smax_valid = true;
       b->smax_gamma = gamma;

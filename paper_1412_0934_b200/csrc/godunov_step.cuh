@@ -800,7 +800,7 @@ cudaError_t launch_variant(const StepParams<T>& P, cudaStream_t s) {
     cudaError_t e = ensure_dynamic_smem((const void*)kern, (int)G::smem_bytes, configured);
     if (e != cudaSuccess) return e;
   }
-  const long long grid = (long long)P.np * P.ntx * P.nty * P.ntz;
+  const long long grid = (long long)P.np_active * P.ntx * P.nty * P.ntz;
   kern<<<(unsigned)grid, NT, G::smem_bytes, s>>>(P);
   cudaError_t le = cudaGetLastError();
   if (le != cudaSuccess) {

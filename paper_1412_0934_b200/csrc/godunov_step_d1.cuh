@@ -609,7 +609,7 @@ cudaError_t launch_variant_d1(const StepParams<double>& P, cudaStream_t s) {
     cudaError_t e = ensure_dynamic_smem((const void*)kern, (int)G::smem_bytes, configured);
     if (e != cudaSuccess) return e;
   }
-  const long long grid = (long long)P.np * P.ntx * P.nty;
+  const long long grid = (long long)P.np_active * P.ntx * P.nty;
   kern<<<(unsigned)grid, NT, G::smem_bytes, s>>>(P);
   cudaError_t le = cudaGetLastError();
   if (le != cudaSuccess) {

@@ -11,7 +11,7 @@ struct SweepParams {
   const T* halo;   // device, [5][np][(n+2g)^3] or nullptr
   const int* nbr;  // device, [np][27]
   unsigned long long* counters;
-  int np, n, g;
+  int np, np_active, n, g;   // np: patches in the arena (strides); the grid covers the first np_active
   T dtdx, gamma, gm1, igm1;
 };
 }  // namespace ppm

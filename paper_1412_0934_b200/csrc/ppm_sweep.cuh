@@ -248,7 +248,7 @@ cudaError_t launch_sweep_variant(const SweepParams<T>& P, cudaStream_t s) {
     cudaError_t e = ensure_dynamic_smem((const void*)kern, 160 * 1024, configured);
     if (e != cudaSuccess) return e;
   }
-  const dim3 grid((unsigned)(P.n * P.n / PB), (unsigned)P.np);
+  const dim3 grid((unsigned)(P.n * P.n / PB), (unsigned)P.np_active);
   const int nt = ((PB * (P.n + 2) + 31) / 32) * 32;
   kern<<<grid, nt, smem, s>>>(P);
   return cudaGetLastError();
