@@ -581,6 +581,76 @@ def run_hierarchy(args):
     print(json.dumps(out))
 
 
+class _SoloTransport:
+    """world = 1: nothing to exchange."""
+
+    def exchange(self, rank, sendbuf, recvbuf):
+        assert not sendbuf and not recvbuf
+
+    @staticmethod
+    def allreduce_max(v):
+        return float(v)
+
+
+def run_sharded(args):
+    """--sharded: ONE level cut over the ranks instead of N replicas: config 3
+    (256^3 Orszag-Tang, MHD; fp32 or fp64 by --workload config3_f32|config3_f64) or config 5 at --size, strong
+    scaling.  Per step every rank refreshes its read-only copies (amr_patch_batch_export -> NCCL isend/irecv ->
+    amr_patch_batch_import), all-reduces the signal speed and steps its owned patches.  With one GPU available only
+    world = 1 could be run here; the exchange is covered by tests/test_sharding.py (gloo) and
+    tests/test_gpu_sharding.py (emulated ranks, bitwise)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    import paper_1412_0934_b200 as amr
+    from paper_1412_0934_b200 import sharding as sh
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    name = args.workload if args.workload.startswith("config3") else "config3_f32"
+    f32 = name.endswith("f32")
+    w = wk.config3_orszag_tang(N=args.size or 256)
+    lev = w.levels[0]
+    plan = sh.make_plans(lev.origin, lev.n, lev.domain_cells, lev.bc, world)[rank]
+    shard = sh.ShardedBatch(plan, lev, amr.AMR_F32 if f32 else amr.AMR_F64, device=str(device))
+    tr = sh.DistTransport(dist) if dist is not None else _SoloTransport()
+    K, Wm = args.steps, args.warmup
+    for _ in range(Wm):
+        sh.sharded_step(shard, tr, w)
+    regions = []
+    for _ in range(max(1, args.repeats)):
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(K):
+            sh.sharded_step(shard, tr, w)
+        e1.record()
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        regions.append(reduce_max_over_ranks([e0.elapsed_time(e1) / K], dist, device)[0])
+    ms = statistics.median(regions)
+    nbytes = sum(len(v) for v in plan.send.values()) * lev.nfields * lev.n ** 3 * (4 if f32 else 8)
+    if rank == 0:
+        out = dict(metric=METRIC, value=lev.ncells / (ms * 1e-3), unit=UNIT, n_gpus=world, steps=K, warmup=Wm, repeats=len(regions),
+                   ms_per_step=ms, higher_is_better=True, scaling="strong", vs_baseline=None, dtype="f32" if f32 else "f64", data="synthetic",
+                   config=dict(workload="config3 sharded: %d^3 Orszag-Tang, %d patches of 16^3 cut into %d space-filling-curve ranges" % (lev.domain_cells[0], lev.npatch, world),
+                               parallelism="one level sharded over %d GPU(s): halo copies + all-reduce(max) per step" % world,
+                               halo_bytes_sent_per_step_rank0=int(nbytes), owned_patches_rank0=int(len(plan.owned)), copies_rank0=int(len(plan.ghost))),
+                   gpu_launches=K * (1 + len(plan.send) + len(plan.recv)))
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -594,9 +664,14 @@ def main():
     ap.add_argument("--repeats", type=int, default=5, help="timed regions of --steps steps each; the median is reported")
     ap.add_argument("--no-parity", action="store_true", help="skip the oracle parity gate (profiling runs only)")
     ap.add_argument("--no-also", action="store_true", help="skip the config-3 timings appended to the default run")
+    ap.add_argument("--sharded", action="store_true", help="one level cut over the ranks (strong scaling) instead of replicas")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
+    if args.sharded:
+        if args.impl == "reference":
+            raise SystemExit("the reference arm times the hot path on one host")
+        return run_sharded(args)
     if args.workload == "patch_builder":
         if args.impl == "reference":
             raise SystemExit("the reference arm times the hot path (config 2, 3, 5); the patch builder's oracle is timed in cpu_baseline")
