@@ -17,7 +17,9 @@
 // Rankine-Hugoniot closure), P8 HLLD(B=0) == HLLC and mhd(B=0) == hydro, P9 extruded
 // Orszag-Tang, P10 second-order convergence (density wave, circularly polarised Alfven wave),
 // P11 first-order limit, P12 predictor cross-check, P13 composite conservation, P14 prolongation
-// identities, P15 closed-form CFL, P16 brute force on a 4^3 patch.
+// identities, P15 closed-form CFL, P16 brute force on a 4^3 patch; round 2: the outflow clamp across sibling
+// patches against numpy.pad(mode='edge') and Sod tiled 2x2x2 bitwise (test_oracle_sod.py), fine patches on
+// non-periodic faces (boundary pressure force, clamped halo cells; test_oracle_amr.py), PPM (test_oracle_ppm.py).
 // Parity unpinned: long-time MHD behaviour (no printed values exist in PAPER.md).
 //
 // Array layout (host): U[field][patch][k][j][i] with ghosts, M = n + 2g per side, i fastest.
