@@ -19,8 +19,9 @@
 //   ring   three planes of primitives on the tile + radius-2 halo; the raw conserved pairs of plane k+2 arrive
 //          by 8-byte cp.async (LDGSTS.64) in the slot plane k-1 vacated and are converted in place by the aux
 //          thread that issued the copies
-//   XP     per x-face column: W^+_x of the odd cell left of a pair (scalar record), then that pair's lower
-//          x flux        YP   per y face: W^+_y of the pair below, then the y flux
+//   XP     per pair of x faces (left of a pair's even cell, between its cells): their left states (W^+_x of the left
+//          neighbour's odd cell - handed over by shuffle - and of the own even cell) as ONE pair record, then the two
+//          x fluxes        YP   per pair of y faces: W^+_y of the pair below (y solver's component order), then the fluxes
 //   UO     (m, E) of the cell awaiting its update (conversion overwrites them in the ring)
 //   SCR    private staging of each compute thread (face states between phases, own fluxes), which keeps a
 //          thread that carries two MHD cells within 168 registers (two CTAs per SM)
@@ -127,18 +128,16 @@ struct GeomX2 {
   static constexpr int NPX = HX + 2;                // pair columns of a ring row (one halo pair each side)
   static constexpr int RH = TY + 4;                 // ring rows
   static constexpr int REC = NF == 9 ? 20 : 12;     // floats per pair record (NF float2 + pad)
-  static constexpr int XREC = NF == 9 ? 12 : 6;     // floats per scalar record (NF floats + pad)
-  static constexpr int XVW = NF == 9 ? 4 : 2;
   static constexpr int SLOT = RH * NPX * REC;       // floats per ring plane
   static constexpr int NSLOT = 3;                   // planes k-1, k, k+1; plane k+2 lands in the slot k-1 vacates
   static constexpr int BLK = NF == 9 ? 5 : 3;       // float4 per staging block: NF pairs + 2 floats
-  static constexpr int NSCR = 3 * BLK + (NF == 9 ? 2 : 1);   // float4 of private staging per interior pair thread
+  static constexpr int NSCR = 3 * BLK;              // float4 of private staging per interior pair thread
   static constexpr int NI = HX * TY;                // interior pair threads
   static constexpr int NPRED = NI + 2 * TY + 2 * HX;
   static constexpr int NXP = TY * (HX + 1);
   static constexpr int NYP = (TY + 1) * HX;
   static constexpr int NCHUNK = RH * NPX;
-  static constexpr size_t smem_floats = (size_t)NSLOT * SLOT + (size_t)NXP * XREC + (size_t)NYP * REC + (size_t)2 * 2 * NI * 4 + (size_t)NSCR * NI * 4;
+  static constexpr size_t smem_floats = (size_t)NSLOT * SLOT + (size_t)NXP * REC + (size_t)NYP * REC + (size_t)2 * 2 * NI * 4 + (size_t)NSCR * NI * 4;
   static constexpr size_t smem_bytes = smem_floats * sizeof(float);
 };
 
@@ -235,7 +234,7 @@ __device__ __forceinline__ int predict_pair(const float* Wm, const float* Wc, co
 template <int NF, int LIM, int RS, int TX, int TY, int NT, int MAXR>
 __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__ StepParams<float> P) {
   using G = GeomX2<NF, TX, TY>;
-  constexpr int HX = G::HX, NPX = G::NPX, RH = G::RH, REC = G::REC, XREC = G::XREC, XVW = G::XVW;
+  constexpr int HX = G::HX, NPX = G::NPX, RH = G::RH, REC = G::REC;
   constexpr int SLOT = G::SLOT, NI = G::NI, NPRED = G::NPRED, NCHUNK = G::NCHUNK;
   constexpr int NA = NT - NI;                 // aux threads: ring pairs + the plane loader
   constexpr int LC = (NCHUNK + NA - 1) / NA;  // loader chunks (pairs of one ring plane) per aux thread
@@ -244,8 +243,8 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
 
   extern __shared__ __align__(16) unsigned char smem_raw[];
   float* const ring = reinterpret_cast<float*>(smem_raw);  // [3][RH][NPX][REC]
-  float* const XP = ring + G::NSLOT * SLOT;                // [TY][HX+1][XREC]
-  float* const YP = XP + G::NXP * XREC;                    // [TY+1][HX][REC]
+  float* const XP = ring + G::NSLOT * SLOT;                // [TY][HX+1][REC]
+  float* const YP = XP + G::NXP * REC;                     // [TY+1][HX][REC]
   float* const UO = YP + G::NYP * REC;                     // [2][2][NI][4]
   float4* const SCR = reinterpret_cast<float4*>(UO + 2 * 2 * NI * 4);  // [NSCR][NI] float4
   __shared__ int s_nbr[27];
@@ -287,8 +286,8 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
     // =================================== compute warps: interior pairs ===================================
     const int pj = tid / HX, pc = tid - pj * HX;                 // row, pair column: cells (2 pc, 2 pc + 1)
     const int rc = ((pj + 2) * NPX + pc + 1) * REC;              // ring record of this pair
-    float* const xpub = XP + (pj * (HX + 1) + pc + 1) * XREC;    // W^+_x of the odd cell, then the right neighbour's flux
-    float* const xsol = xpub - XREC;                             // left state of the lo face, then its flux
+    float* const xpub = XP + (pj * (HX + 1) + pc + 1) * REC;     // the right neighbour's x face pair: its left states, then its fluxes
+    float* const xsol = xpub - REC;                              // this pair's x faces (left of the even cell, between the cells)
     float* const ypub = YP + ((pj + 1) * HX + pc) * REC;         // W^+_y, then the upper pair's y fluxes
     float* const ysol = ypub - HX * REC;                         // W^+_y of the pair below, then this pair's y fluxes
     const int cell0 = p * n3 + (y0 + pj) * n + (x0 + 2 * pc);
@@ -298,11 +297,10 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
     // are staged in this thread's private shared-memory scratch (float4 j of thread tid at SCR[j*NI + tid]):
     // (blocks of BLK float4 = NF pairs + 2 floats: 5 for MHD, 3 for hydro)
     //   BZ      W^+_z of the previous plane (left state of the next z face)
-    //   BX      W^-_x pair + W^+_x of the even cell [0..1]; after the x solve: the x flux pair
-    //   BY      W^-_y pair + W^+_x of the even cell [2..3]; after the y solve: the y flux pair
-    //   BE      W^+_x of the even cell [4..NF-1]
+    //   BX      W^-_x pair (right states of the pair's two x faces); after the x solve: the x flux pair
+    //   BY      W^-_y pair in the y solver's component order (y, z, x); after the y solve: the y flux pair, same order
     float4* const sc = SCR + tid;
-    constexpr int BLK = G::BLK, BZ = 0, BX = BLK, BY = 2 * BLK, BE = 3 * BLK, NFULL = (NF - 1) / 2;
+    constexpr int BLK = G::BLK, BZ = 0, BX = BLK, BY = 2 * BLK, NFULL = (NF - 1) / 2;
     auto st_block = [&](int j0, const F2* a, float e0, float e1) {  // NF pairs + 2 floats -> BLK float4
 #pragma unroll
       for (int i = 0; i < NFULL; ++i) sc[(j0 + i) * NI] = make_float4(a[2 * i].v.x, a[2 * i].v.y, a[2 * i + 1].v.x, a[2 * i + 1].v.y);
@@ -337,27 +335,42 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
           const int nb = predict_pair<NF, LIM>(Wm, Wc, Wp, rc, NPX * REC, REC, P, ms, B2(true), ws, hx, hy, hz);
           if (mid) {
             npos += nb;
+            F2 o[9], r[9];
+#pragma unroll
+            for (int q = NF; q < 9; ++q) { o[q] = F2(0.f); r[q] = F2(0.f); ws[q] = F2(0.f); }
+            // x: the left states of this pair's two x faces are (W^+_x of the left neighbour's odd cell, W^+_x of the own
+            // even cell).  The neighbour's value arrives by shuffle (a row of pairs lies inside one warp), so every pair
+            // publishes ONE complete pair record, as it does for y.  First pair of a row: its left neighbour is the left
+            // ring pair (aux warp), which writes the .x halves itself; last pair of a row: the right ring pair's face
+            // needs this pair's odd cell, written here.
             {
-              float o[NF];
+              F2 wpx[NF];
 #pragma unroll
-              for (int q = 0; q < NF; ++q) o[q] = ws[q].v.y + hx[q].v.y;
-              sts_n<NF, XVW>(xpub, o);
+              for (int q = 0; q < NF; ++q) wpx[q] = ws[q] + hx[q];
+#pragma unroll
+              for (int q = 0; q < NF; ++q) o[q] = F2(__shfl_up_sync(0xffffffffu, wpx[q].v.y, 1), wpx[q].v.x);
+              if (pc != 0) sts_pairs<NF>(xsol, o);
+              else {
+#pragma unroll
+                for (int q = 0; q < NF; ++q) xsol[2 * q + 1] = wpx[q].v.x;
+              }
+              if (pc == HX - 1) {
+#pragma unroll
+                for (int q = 0; q < NF; ++q) xpub[2 * q] = wpx[q].v.y;
+              }
             }
-            F2 o[9];
-            float wpxl[9];
+            // y: W^+_y of this pair = left states of the upper pair's y faces, in the y solver's component order
 #pragma unroll
-            for (int q = 0; q < NF; ++q) { o[q] = ws[q] + hy[q]; wpxl[q] = ws[q].v.x + hx[q].v.x; }
-            sts_pairs<NF>(ypub, o);
-#pragma unroll
-            for (int q = NF; q < 9; ++q) { o[q] = F2(0.f); wpxl[q] = 0.f; ws[q] = F2(0.f); }
+            for (int q = 0; q < NF; ++q) o[q] = ws[q] + hy[q];
+            rot_in<NF, 1>(o, r);
+            sts_pairs<NF>(ypub, r);
 #pragma unroll
             for (int q = 0; q < NF; ++q) o[q] = ws[q] - hx[q];
-            st_block(BX, o, wpxl[0], wpxl[1]);
+            st_block(BX, o, 0.f, 0.f);
 #pragma unroll
             for (int q = 0; q < NF; ++q) o[q] = ws[q] - hy[q];
-            st_block(BY, o, wpxl[2], wpxl[3]);
-            sc[BE * NI] = make_float4(wpxl[4], wpxl[5], wpxl[6], wpxl[7]);
-            if (NF == 9) sc[(BE + 1) * NI] = make_float4(wpxl[8], 0.f, 0.f, 0.f);
+            rot_in<NF, 1>(o, r);
+            st_block(BY, r, 0.f, 0.f);
           }
           // z direction: left state of the face below = W^+_z of the previous plane (scratch), then this
           // plane's W^+_z takes its place
@@ -435,64 +448,35 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
       }
       cp_commit();
       if (mid) {
-        float wpxl[9];
-        F2 wmy[9];
-        {
-          const float4 v15 = sc[BE * NI];
-          wpxl[4] = v15.x; wpxl[5] = v15.y; wpxl[6] = v15.z; wpxl[7] = v15.w;
-          wpxl[8] = NF == 9 ? sc[(BE + 1) * NI].x : 0.f;
-        }
-        {
-          F2 wl[9], wmx[9], WL[9], WR[9], Fr[NF], fx[9];
-          ld_block(BX, wmx, wpxl[0], wpxl[1]);
-          ld_block(BY, wmy, wpxl[2], wpxl[3]);
-          {
-            float xl[NF];
-            lds_n<NF, XVW>(xsol, xl);
-#pragma unroll
-            for (int q = 0; q < NF; ++q) wl[q] = F2(xl[q], wpxl[q]);
-          }
-          rot_in<NF, 0>(wl, WL);
-          rot_in<NF, 0>(wmx, WR);
+        // d = 0: the pair's two x faces; d = 1: its two y faces.  ONE solver instance (the plane loop is bound by
+        // instruction fetch: profiles/r2a); operands and results in the solver's component order (identity for x,
+        // rotated for y), uniform pair records / staging blocks, so that nothing but two pointers differs per trip.
+#pragma unroll 1
+        for (int d = P.ntz - 1; d < 2; ++d) {   // ntz == 1: an opaque lower bound keeps the loop from being unrolled
+          float* const rec = d ? ysol : xsol;
+          const int bj = d ? BY : BX;
+          F2 WL[9], WR[9], Fr[9];
+          float e0, e1;
+          lds_pairs<NF>(rec, WL);
+          ld_block(bj, WR, e0, e1);
           riemann2<NF, RS>(WL, WR, RC, Fr, B2(true), s_cnt);
-          rot_out<NF, 0>(Fr, fx);
-          {
-            float o[NF];
 #pragma unroll
-            for (int q = 0; q < NF; ++q) o[q] = fx[q].v.x;
-            sts_n<NF, XVW>(xsol, o);
-#pragma unroll
-            for (int q = NF; q < 9; ++q) fx[q] = F2(0.f);
-            // private copy of both x fluxes -> scratch 5..9 (W^-_x is consumed).  Phase 3 must not read
-            // them back from xsol: the left neighbour overwrites that slot in ITS next phase 1, with no
-            // barrier in between
-            st_block(BX, fx, 0.f, 0.f);
-          }
+          for (int q = NF; q < 9; ++q) Fr[q] = F2(0.f);
+          sts_pairs<NF>(rec, Fr);         // for the left / lower neighbour's phase 3
+          st_block(bj, Fr, 0.f, 0.f);     // private copy for this thread's phase 3 (the neighbour overwrites rec in ITS
+                                          // next phase 1, with no barrier in between)
           // record the fluxes for the reflux: x faces 0 and n/2 are the even face of a pair
-          if (X2_UNLIKELY(blk >= 0) && (x0 + 2 * pc == 0 || x0 + 2 * pc == (n >> 1))) {
-            float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)((x0 + 2 * pc) == 0 ? 0 : ((x0 + 2 * pc) == n ? 2 : 1)) * n2 + (size_t)(kk * n + (y0 + pj)));
+          const int fidx = d ? y0 + pj : x0 + 2 * pc;
+          if (X2_UNLIKELY(blk >= 0) && (fidx == 0 || fidx == (n >> 1))) {
+            F2 f[NF];
+            if (d) rot_out<NF, 1>(Fr, f); else rot_out<NF, 0>(Fr, f);
+            float* dstF = P.fblk + ((size_t)blk * 3 + d) * NF * fsz + (size_t)(fidx == 0 ? 0 : 1) * n2 +
+                          (size_t)(d ? kk * n + (x0 + 2 * pc) : kk * n + (y0 + pj));
 #pragma unroll
-            for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, fx[q].v.x);
-          }
-        }
-        {
-          F2 wl[NF], WL[9], WR[9], Fr[NF], fy[NF];
-          lds_pairs<NF>(ysol, wl);
-          rot_in<NF, 1>(wl, WL);
-          rot_in<NF, 1>(wmy, WR);
-          riemann2<NF, RS>(WL, WR, RC, Fr, B2(true), s_cnt);
-          rot_out<NF, 1>(Fr, fy);
-          sts_pairs<NF>(ysol, fy);
-          {
-            F2 o[9];
-#pragma unroll
-            for (int q = 0; q < 9; ++q) o[q] = q < NF ? fy[q] : F2(0.f);
-            st_block(BY, o, 0.f, 0.f);  // private copy for phase 3 (same reason)
-          }
-          if (X2_UNLIKELY(blk >= 0) && (y0 + pj == 0 || y0 + pj == (n >> 1))) {
-            float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)((y0 + pj) == 0 ? 0 : ((y0 + pj) == n ? 2 : 1)) * n2 + (size_t)(kk * n + (x0 + 2 * pc)));
-#pragma unroll
-            for (int q = 0; q < NF; ++q) { atomicAdd(dstF + (size_t)q * fsz, fy[q].v.x); atomicAdd(dstF + (size_t)q * fsz + 1, fy[q].v.y); }
+            for (int q = 0; q < NF; ++q) {
+              atomicAdd(dstF + (size_t)q * fsz, f[q].v.x);
+              if (d) atomicAdd(dstF + (size_t)q * fsz + 1, f[q].v.y);
+            }
           }
         }
       }
@@ -504,17 +488,23 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
       // pair's y fluxes come from the slots this very thread overwrites with its W^+ in the next phase 1,
       // so no barrier is needed before that
       if (mid) {
-        float xr[NF], e0, e1;
-        F2 fu[NF], fx[9], fy[9];
-        lds_n<NF, XVW>(xpub, xr);
-        lds_pairs<NF>(ypub, fu);
+        float e0, e1;
+        F2 xr[NF], fu[NF], fx[9], fy[9], dy[NF], dyu[NF];
+        lds_pairs<NF>(xpub, xr);     // the right neighbour's x fluxes: its lo face is the face right of this pair's odd cell
+        lds_pairs<NF>(ypub, fu);     // the upper pair's y fluxes (y solver's component order)
         ld_block(BX, fx, e0, e1);
         ld_block(BY, fy, e0, e1);
 #pragma unroll
+        for (int q = 0; q < NF; ++q) dy[q] = fu[q] - fy[q];
+        rot_out<NF, 1>(dy, dyu);
+#pragma unroll
         for (int q = 0; q < NF; ++q) {
-          const F2 dfx = F2(fx[q].v.y - fx[q].v.x, xr[q] - fx[q].v.y);
-          dU[q] = (dfx + (fu[q] - fy[q])) + dU[q];
+          const F2 dfx = F2(fx[q].v.y - fx[q].v.x, xr[q].v.x - fx[q].v.y);
+          dU[q] = (dfx + dyu[q]) + dU[q];
         }
+        // xpub is the right neighbour's record: it rewrites it in its next phase 1.  Neighbours in x are lanes of the
+        // same warp (a row of pairs never straddles warps), so a warp-level fence orders the read before that write
+        __syncwarp();
       }
       float* tmp = Wm; Wm = Wc; Wc = Wp; Wp = tmp;
     }
@@ -639,7 +629,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
     const bool pred = at < 2 * TY + 2 * HX;
     const bool right = at < TY, left = pred && px == 0, top = pred && pj == TY, bottom = pred && pj == -1;
     const int rc = ((pj + 2) * NPX + px) * REC;
-    float* const xslot = XP + ((right || left) ? pj * (HX + 1) + (right ? HX : 0) : 0) * XREC;
+    float* const xslot = XP + ((right || left) ? pj * (HX + 1) + (right ? HX : 0) : 0) * REC;
     float* const yslot = YP + ((top || bottom) ? (top ? TY * HX : 0) + px - 1 : 0) * REC;
     F2 wm[NF];  // right ring: W^-_x (lo half real); top ring: W^-_y
 #pragma unroll
@@ -663,21 +653,23 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
         F2 ws[NF], hx[NF], hy[NF], hz[NF];
         predict_pair<NF, LIM>(Wm, Wc, Wp, rc, NPX * REC, REC, P, ms, B2(vlo, vhi), ws, hx, hy, hz);
         if (left) {
-          float o[NF];
+          // W^+_x of cell -1 = the .x halves of the first pair's left-state record (that pair writes the .y halves)
 #pragma unroll
-          for (int q = 0; q < NF; ++q) o[q] = ws[q].v.y + hx[q].v.y;
-          sts_n<NF, XVW>(xslot, o);
+          for (int q = 0; q < NF; ++q) xslot[2 * q] = ws[q].v.y + hx[q].v.y;
         } else if (bottom) {
-          F2 o[NF];
+          F2 o[NF], r[NF];
 #pragma unroll
           for (int q = 0; q < NF; ++q) o[q] = ws[q] + hy[q];
-          sts_pairs<NF>(yslot, o);
+          rot_in<NF, 1>(o, r);            // y solver's component order
+          sts_pairs<NF>(yslot, r);
         } else if (right) {
 #pragma unroll
           for (int q = 0; q < NF; ++q) wm[q] = ws[q] - hx[q];
         } else {
+          F2 o[NF];
 #pragma unroll
-          for (int q = 0; q < NF; ++q) wm[q] = ws[q] - hy[q];
+          for (int q = 0; q < NF; ++q) o[q] = ws[q] - hy[q];
+          rot_in<NF, 1>(o, wm);
         }
       }
       __syncthreads();
@@ -690,40 +682,28 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
         // ONE solver instance for the tile's last x faces (right ring: lo half real) and last y faces (top ring):
         // the kernel is bound by instruction fetch (profiles/r1c), these warps have the slack for the few moves
         // that bring the two roles' operands into the same registers
-        F2 WL[NF], WR[NF], Fr[NF];
-        if (right) {
-          float xl[NF];
-          lds_n<NF, XVW>(xslot, xl);
-          F2 wl[NF];
+        // (operands arrive in the solver's component order: identity for x, rotated for y)
+        F2 WL[NF], Fr[NF];
+        lds_pairs<NF>(right ? xslot : yslot, WL);
+        if (right) {   // only the lo face (TX - 1/2) is real: its left state is the .x half the last interior pair wrote
 #pragma unroll
-          for (int q = 0; q < NF; ++q) wl[q] = F2(xl[q], xl[q]);
-          rot_in<NF, 0>(wl, WL);
-          rot_in<NF, 0>(wm, WR);
-        } else {
-          F2 wl[NF];
-          lds_pairs<NF>(yslot, wl);
-          rot_in<NF, 1>(wl, WL);
-          rot_in<NF, 1>(wm, WR);
+          for (int q = 0; q < NF; ++q) WL[q] = F2(WL[q].v.x, WL[q].v.x);
         }
-        riemann2<NF, RS>(WL, WR, RC, Fr, B2(true, !right), s_cnt);
-        if (right) {
-          rot_out<NF, 0>(Fr, wm);
-          float o[NF];
-#pragma unroll
-          for (int q = 0; q < NF; ++q) o[q] = wm[q].v.x;
-          sts_n<NF, XVW>(xslot, o);
-          if (X2_UNLIKELY(blk >= 0) && x0 + TX == n) {  // the patch's last x face (a7)
+        riemann2<NF, RS>(WL, wm, RC, Fr, B2(true, !right), s_cnt);
+        sts_pairs<NF>(right ? xslot : yslot, Fr);
+        if (X2_UNLIKELY(blk >= 0)) {
+          if (right && x0 + TX == n) {  // the patch's last x face (a7)
+            F2 f[NF];
+            rot_out<NF, 0>(Fr, f);
             float* dstF = P.fblk + ((size_t)blk * 3 + 0) * NF * fsz + ((size_t)2 * n2 + (size_t)(kk * n + (y0 + pj)));
 #pragma unroll
-            for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, wm[q].v.x);
-          }
-        } else {
-          rot_out<NF, 1>(Fr, wm);
-          sts_pairs<NF>(yslot, wm);
-          if (X2_UNLIKELY(blk >= 0) && y0 + TY == n) {
+            for (int q = 0; q < NF; ++q) atomicAdd(dstF + (size_t)q * fsz, f[q].v.x);
+          } else if (!right && y0 + TY == n) {
+            F2 f[NF];
+            rot_out<NF, 1>(Fr, f);
             float* dstF = P.fblk + ((size_t)blk * 3 + 1) * NF * fsz + ((size_t)2 * n2 + (size_t)(kk * n + (x0 + 2 * (px - 1))));
 #pragma unroll
-            for (int q = 0; q < NF; ++q) { atomicAdd(dstF + (size_t)q * fsz, wm[q].v.x); atomicAdd(dstF + (size_t)q * fsz + 1, wm[q].v.y); }
+            for (int q = 0; q < NF; ++q) { atomicAdd(dstF + (size_t)q * fsz, f[q].v.x); atomicAdd(dstF + (size_t)q * fsz + 1, f[q].v.y); }
           }
         }
       }
