@@ -146,7 +146,7 @@ def build_workload(name: str, device, size: int | None):
     if name == "config5":
         N = size or 512
         U, origin = wk.turbulence_patches_torch(N, 32, device)
-        host = torch.empty(U.shape, dtype=torch.float32, pin_memory=True)
+        host = torch.empty(U.shape, dtype=torch.float32, pin_memory=torch.cuda.is_available())
         host.copy_(U)
         del U
         torch.cuda.empty_cache()
@@ -160,7 +160,7 @@ def build_workload(name: str, device, size: int | None):
         U, origin = wk.turbulence_patches_torch(N, 32, device)
         U[4] -= 0.5 * (U[5] ** 2 + U[6] ** 2 + U[7] ** 2)
         dt = torch.float32 if name.endswith("f32") else torch.float64
-        host = torch.empty((5,) + tuple(U.shape[1:]), dtype=dt, pin_memory=True)
+        host = torch.empty((5,) + tuple(U.shape[1:]), dtype=dt, pin_memory=torch.cuda.is_available())
         host.copy_(U[:5])
         del U
         torch.cuda.empty_cache()
@@ -174,7 +174,7 @@ def build_workload(name: str, device, size: int | None):
         U, origin = wk.turbulence_patches_torch(N, 32, device, mach=1.0)
         U[4] -= 0.5 * (U[5] ** 2 + U[6] ** 2 + U[7] ** 2)
         dt = torch.float32 if name.endswith("f32") else torch.float64
-        host = torch.empty((5,) + tuple(U.shape[1:]), dtype=dt, pin_memory=True)
+        host = torch.empty((5,) + tuple(U.shape[1:]), dtype=dt, pin_memory=torch.cuda.is_available())
         host.copy_(U[:5])
         del U
         torch.cuda.empty_cache()
@@ -186,7 +186,7 @@ def build_workload(name: str, device, size: int | None):
         w = wk.config3_orszag_tang(N=N)
         lev = w.levels[0]
         dt = torch.float32 if name.endswith("f32") else torch.float64
-        host = torch.empty(lev.U.shape, dtype=dt, pin_memory=True)
+        host = torch.empty(lev.U.shape, dtype=dt, pin_memory=torch.cuda.is_available())
         host.copy_(torch.from_numpy(lev.U))
         return dict(U=host, origin=lev.origin, n=16, dx=lev.dx, domain=lev.domain_cells, mhd=True, dtype=name[-3:],
                     gamma=w.gamma, limiter=w.limiter, riemann=w.riemann, cfl=w.cfl, alpha=w.alpha,
@@ -194,7 +194,7 @@ def build_workload(name: str, device, size: int | None):
     if name == "config2":
         w = wk.config2_random_patches(npatch=size or 512)
         lev = w.levels[0]
-        host = torch.empty(lev.U.shape, dtype=torch.float64, pin_memory=True)
+        host = torch.empty(lev.U.shape, dtype=torch.float64, pin_memory=torch.cuda.is_available())
         host.copy_(torch.from_numpy(lev.U))
         return dict(U=host, origin=None, n=16, dx=lev.dx, domain=(16, 16, 16), mhd=False, dtype="f64", gamma=w.gamma,
                     limiter=w.limiter, riemann=w.riemann, cfl=w.cfl, alpha=0.0, self_periodic=True,
@@ -483,7 +483,7 @@ def run_hierarchy(args):
     tdt = torch.float32 if f32 else torch.float64
     host = []
     for lv in wl.levels:
-        h = torch.empty(lv.U.shape, dtype=tdt, pin_memory=True)
+        h = torch.empty(lv.U.shape, dtype=tdt, pin_memory=torch.cuda.is_available())
         h.copy_(torch.from_numpy(lv.U))
         host.append(h)
     hier = amr.Hierarchy.from_workload(wl, amr.AMR_F32 if f32 else amr.AMR_F64)
@@ -732,7 +732,7 @@ def main():
     e2e = None
     if not args.no_e2e:
         ke = min(K, 3)
-        out_host = torch.empty(W["U"].shape, dtype=W["U"].dtype, pin_memory=True)
+        out_host = torch.empty(W["U"].shape, dtype=W["U"].dtype, pin_memory=torch.cuda.is_available())
         b.upload(W["U"]); one_step(b, W); b.download(out=out_host)   # warm
         torch.cuda.synchronize()
         if dist is not None:
