@@ -77,10 +77,12 @@ cudaError_t launch_fill_nan(int dtype, void* ptr, size_t count, cudaStream_t s);
 cudaError_t launch_fma_chain(int dtype, void* sink, int grid, int iters, cudaStream_t s);
 
 // two-level kernels (aux_kernels.cu); table formats are documented at the kernels
-// dst: [nparents][8] child halo indices or -1, c7: [nparents][7] (formats at the kernel)
-cudaError_t launch_prolong(int dtype, void* halo, size_t fs_halo, int nf, const long long* dst, const long long* c7,
-                           int ncells, const void* Ucold, const void* Ucnew, size_t fs_c, double theta,
-                           cudaStream_t s);
+// O8 without tables: parents resolved in the kernel through the coarse patch map (cmap, [cdims z][y][x], -1 = none),
+// the fine patches' origins and neighbour table (all device); bc: the six AMR_BC_* of the level pair (host)
+cudaError_t launch_prolong_halo(int dtype, void* halo, size_t fs_halo, int nf, int n, int g, int npf, const int* domf,
+                                const int* domc, const int* cdims, const int* bc, const int* forigin, const int* nbr,
+                                const int* cmap, const void* Ucold, const void* Ucnew, size_t fs_c, double theta,
+                                cudaStream_t s);
 cudaError_t launch_restrict(int dtype, const void* Uf, size_t fs_f, int nf, int n, const long long* dst, int nent,
                             void* Uc, size_t fs_c, cudaStream_t s);
 cudaError_t launch_reflux(int dtype, void* Uc, size_t fs_c, int nf, int n, const long long* faces, int nfaces,

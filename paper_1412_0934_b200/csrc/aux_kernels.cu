@@ -119,22 +119,64 @@ template <class T> __device__ __forceinline__ T minmod2(T a, T b) {
   return (lo > T(0) ? lo : T(0)) + (hi < T(0) ? hi : T(0));
 }
 
-// One thread per (fine patch, parent cell) entry e.  c7[e][7]: flat coarse interior indices: centre, x-, x+, y-,
-// y+, z-, z+.  dst[e][8]: flat index into one field of the halo buffer of child c = (pz, py, px) parity bits, or
-// -1 if that child is not a coarse-fine halo cell of the patch.  The slopes are computed once per parent.
+// O8 without tables (round 2: the host-built lists were 120 B per parent cell - 161 MB for a 944-patch level - and
+// 30-137 ms of host time per relink).  One thread per (fine patch p, parent position (li, lj, lk) in the patch's halo
+// box): the box spans the fine offsets -4 .. n+3, hp = n/2 + 4 parents per side, parent l <-> children 2(l-2), 2(l-2)+1
+// (patch origins and n are even, so a parent never straddles a region boundary).  A parent whose region no sibling
+// covers (neighbour table entry NBR_FROM_HALO) has its 7-point stencil resolved here through the coarse level's patch
+// map (periodic faces wrap; at an outflow face the fine cells take the prolongation AT the clamped in-domain cell,
+// parent and child parity of the clamped index; the +-1 stencil clamps like the coarse ghosts),
+// the minmod slopes are taken once, and the children inside the g halo layers are written.
+struct ProlongGeom {
+  int n, g, npf;
+  int domf[3], domc[3], cdims[3];
+  int per_lo[3], per_hi[3];   // 1 = periodic face
+};
+
 template <class T>
-__global__ void __launch_bounds__(128) prolong_kernel(T* __restrict__ halo, size_t fs_halo, int nf,
-                                                      const long long* __restrict__ dst,
-                                                      const long long* __restrict__ c7, int nparents,
-                                                      const T* __restrict__ Uold, const T* __restrict__ Unew,
-                                                      size_t fs_c, T theta) {
-  const int e = blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= nparents) return;
-  long long s[7], d[8];
+__global__ void __launch_bounds__(128) prolong_halo_kernel(T* __restrict__ halo, size_t fs_halo, int nf, ProlongGeom G,
+                                                           const int* __restrict__ forigin, const int* __restrict__ nbr,
+                                                           const int* __restrict__ cmap, const T* __restrict__ Uold,
+                                                           const T* __restrict__ Unew, size_t fs_c, T theta) {
+  const int n = G.n, g = G.g, hp = n / 2 + 4, hp3 = hp * hp * hp;
+  const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= (long long)G.npf * hp3) return;
+  const int p = (int)(e / hp3);
+  int r = (int)(e - (long long)p * hp3);
+  const int l[3] = {r % hp, (r / hp) % hp, r / (hp * hp)};
+  int reg = 0, C[3], forced[3];
+  const int pw[3] = {1, 3, 9};
 #pragma unroll
-  for (int k = 0; k < 7; ++k) s[k] = c7[(size_t)e * 7 + k];
+  for (int a = 0; a < 3; ++a) {
+    const int i0 = 2 * (l[a] - 2);                       // fine offset of child 0 along a
+    const int ra = i0 < 0 ? 0 : (i0 >= n ? 2 : 1);
+    reg += ra * pw[a];
+    int gi = forigin[3 * p + a] + i0;                    // even
+    forced[a] = -1;
+    if (gi < 0) {
+      if (G.per_lo[a]) gi += G.domf[a]; else { gi = 0; forced[a] = 0; }
+    } else if (gi >= G.domf[a]) {
+      if (G.per_hi[a]) gi -= G.domf[a]; else { gi = G.domf[a] - 1; forced[a] = 1; }
+    }
+    C[a] = gi >> 1;
+  }
+  if (reg == 13 || nbr[p * 27 + reg] != NBR_FROM_HALO) return;
+  auto coarse_flat = [&](int cx, int cy, int cz) -> long long {
+    int c[3] = {cx, cy, cz};
 #pragma unroll
-  for (int k = 0; k < 8; ++k) d[k] = dst[(size_t)e * 8 + k];
+    for (int a = 0; a < 3; ++a) {
+      if (c[a] < 0) c[a] = G.per_lo[a] ? c[a] + G.domc[a] : 0;
+      else if (c[a] >= G.domc[a]) c[a] = G.per_hi[a] ? c[a] - G.domc[a] : G.domc[a] - 1;
+    }
+    const int pc = cmap[((c[2] / n) * G.cdims[1] + c[1] / n) * G.cdims[0] + c[0] / n];   // nesting was checked at link time
+    return (long long)pc * n * n * n + ((long long)(c[2] % n) * n + (c[1] % n)) * n + (c[0] % n);
+  };
+  long long s[7];
+  s[0] = coarse_flat(C[0], C[1], C[2]);
+  s[1] = coarse_flat(C[0] - 1, C[1], C[2]); s[2] = coarse_flat(C[0] + 1, C[1], C[2]);
+  s[3] = coarse_flat(C[0], C[1] - 1, C[2]); s[4] = coarse_flat(C[0], C[1] + 1, C[2]);
+  s[5] = coarse_flat(C[0], C[1], C[2] - 1); s[6] = coarse_flat(C[0], C[1], C[2] + 1);
+  const int M = n + 2 * g;
   const T w0 = T(1) - theta;
   for (int q = 0; q < nf; ++q) {
     const T* a = Uold + (size_t)q * fs_c;
@@ -150,14 +192,18 @@ __global__ void __launch_bounds__(128) prolong_kernel(T* __restrict__ halo, size
     T sl[3];
 #pragma unroll
     for (int dd = 0; dd < 3; ++dd) sl[dd] = minmod2<T>(st[0] - st[1 + 2 * dd], st[2 + 2 * dd] - st[0]);
-    T* out = halo + (size_t)q * fs_halo;
+    T* out = halo + (size_t)q * fs_halo + (size_t)p * M * M * M;
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
-      if (d[c] < 0) continue;
+      const int i = 2 * (l[0] - 2) + (c & 1), j = 2 * (l[1] - 2) + ((c >> 1) & 1), k = 2 * (l[2] - 2) + ((c >> 2) & 1);
+      if (i < -g || i >= n + g || j < -g || j >= n + g || k < -g || k >= n + g) continue;
       T val = st[0];
 #pragma unroll
-      for (int dd = 0; dd < 3; ++dd) val += (((c >> dd) & 1) ? T(0.25) : T(-0.25)) * sl[dd];
-      out[d[c]] = val;
+      for (int dd = 0; dd < 3; ++dd) {
+        const int bit = forced[dd] >= 0 ? forced[dd] : ((c >> dd) & 1);
+        val += (bit ? T(0.25) : T(-0.25)) * sl[dd];
+      }
+      out[((size_t)(k + g) * M + (j + g)) * M + (i + g)] = val;
     }
   }
 }
@@ -370,17 +416,26 @@ cudaError_t launch_fill_nan(int dtype, void* ptr, size_t count, cudaStream_t s) 
   return cudaGetLastError();
 }
 
-cudaError_t launch_prolong(int dtype, void* halo, size_t fs_halo, int nf, const long long* dst, const long long* c7,
-                           int ncells, const void* Ucold, const void* Ucnew, size_t fs_c, double theta,
-                           cudaStream_t s) {
-  if (ncells == 0) return cudaSuccess;
-  const unsigned grid = (unsigned)((ncells + 127) / 128);
+cudaError_t launch_prolong_halo(int dtype, void* halo, size_t fs_halo, int nf, int n, int g, int npf, const int* domf,
+                                const int* domc, const int* cdims, const int* bc, const int* forigin, const int* nbr,
+                                const int* cmap, const void* Ucold, const void* Ucnew, size_t fs_c, double theta,
+                                cudaStream_t s) {
+  if (npf == 0) return cudaSuccess;
+  ProlongGeom G;
+  G.n = n; G.g = g; G.npf = npf;
+  for (int a = 0; a < 3; ++a) {
+    G.domf[a] = domf[a]; G.domc[a] = domc[a]; G.cdims[a] = cdims[a];
+    G.per_lo[a] = bc[2 * a] == 0; G.per_hi[a] = bc[2 * a + 1] == 0;   // AMR_BC_PERIODIC == 0
+  }
+  const int hp = n / 2 + 4;
+  const long long nthreads = (long long)npf * hp * hp * hp;
+  const unsigned grid = (unsigned)((nthreads + 127) / 128);
   if (dtype == 0)
-    prolong_kernel<float><<<grid, 128, 0, s>>>((float*)halo, fs_halo, nf, dst, c7, ncells, (const float*)Ucold,
-                                              (const float*)Ucnew, fs_c, (float)theta);
+    prolong_halo_kernel<float><<<grid, 128, 0, s>>>((float*)halo, fs_halo, nf, G, forigin, nbr, cmap, (const float*)Ucold,
+                                                    (const float*)Ucnew, fs_c, (float)theta);
   else
-    prolong_kernel<double><<<grid, 128, 0, s>>>((double*)halo, fs_halo, nf, dst, c7, ncells, (const double*)Ucold,
-                                               (const double*)Ucnew, fs_c, theta);
+    prolong_halo_kernel<double><<<grid, 128, 0, s>>>((double*)halo, fs_halo, nf, G, forigin, nbr, cmap, (const double*)Ucold,
+                                                     (const double*)Ucnew, fs_c, theta);
   return cudaGetLastError();
 }
 

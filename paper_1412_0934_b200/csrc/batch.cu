@@ -144,8 +144,7 @@ struct amr_level_link {
   amr_patch_batch *c, *f;
   char* ws;
   size_t bytes;
-  long long *pro_dst, *pro_c7;
-  int npro;
+  int *forg, *cmap;   // device: fine patch origins [npf][3], coarse patch map [z][y][x] (the prolongation resolves parents itself)
   long long* res_dst;
   int nres;
   long long* faces;  // all (direction, side) tables merged, sorted by coarse cell (stable in d*2+side)
@@ -159,14 +158,14 @@ struct amr_level_link {
 namespace {
 
 struct LinkHost {
-  std::vector<long long> pro_dst, pro_c7, res_dst, faces[6], faces_all;
+  std::vector<long long> res_dst, faces[6], faces_all;
   std::vector<int> fblk_of_c;
   int nblk_c = 0;
   bool identity_c = false;  // coarse blocks are per patch (block index = patch index)
 };
 
 struct LinkLayout {
-  size_t pro_dst, pro_c7, res_dst, faces, fblk_c, fblk_f, total, fblk_c_bytes, fblk_f_bytes;
+  size_t forg, cmap, res_dst, faces, fblk_c, fblk_f, total, fblk_c_bytes, fblk_f_bytes;
 };
 
 int wrapi(int v, int m) { return ((v % m) + m) % m; }
@@ -189,63 +188,32 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
     *out = (long long)pc * (long long)n3 + ((long long)(C[2] - oc[2]) * n + (C[1] - oc[1])) * n + (C[0] - oc[0]);
     return true;
   };
-  // O8 list: fine halo cells in regions no sibling covers, grouped by parent cell: one entry per (patch, parent)
-  // = 7 stencil indices (pro_c7) + the halo index of each of its 8 children that is needed, else -1 (pro_dst)
-  const int hp = n / 2 + 4;   // parent cells along one side of a patch's halo box (fine -g..n+g-1, g <= 4)
-  if (g > 4) return fail(AMR_EINVAL, "nghost > 4 is not supported by the prolongation tables");
-  std::vector<int> slot((size_t)hp * hp * hp);
-  {  // at most the parents of the halo shell per patch; untouched reserve costs nothing, regrowth copies do
-    const size_t h = (size_t)n / 2, shell = (size_t)hp * hp * hp - (h > 2 ? (h - 2) * (h - 2) * (h - 2) : 0);
-    H.pro_dst.reserve((size_t)f->d.npatch * shell * 8);
-    H.pro_c7.reserve((size_t)f->d.npatch * shell * 7);
-  }
+  // O8 needs no table: prolong_halo_kernel resolves the parents itself.  What the host still owes is the check of
+  // proper nesting: every halo region of a fine patch that no sibling covers (and its +-1 stencil) must lie inside
+  // coarse patches.  Checked per region at coarse-PATCH granularity: the region's parent cells, grown by one, span at
+  // most two coarse patches per axis.
+  if (g > 4) return fail(AMR_EINVAL, "nghost > 4 is not supported by the prolongation kernel");
   for (int p = 0; p < f->d.npatch; ++p) {
     const int* o = &f->origin[3 * p];
-    std::fill(slot.begin(), slot.end(), -1);
-    // region by region (27 neighbour regions of the patch; only those no sibling covers have entries)
     const int lo[3] = {-g, 0, n}, hi[3] = {0, n, n + g};
     for (int reg = 0; reg < 27; ++reg) {
-      const int rx = reg % 3, ry = (reg / 3) % 3, rz = reg / 9;
       if (reg == 13 || f->nbr_host[(size_t)p * 27 + reg] != amr::NBR_FROM_HALO) continue;
-    for (int k = lo[rz]; k < hi[rz]; ++k)
-      for (int j = lo[ry]; j < hi[ry]; ++j)
-        for (int i = lo[rx]; i < hi[rx]; ++i) {
-          // global fine index: periodic faces wrap, outflow faces clamp (O0 rule (ii): the halo cell takes the
-          // value of the clamped in-domain cell, which no fine patch covers, i.e. the prolongation AT that cell)
-          int gi[3] = {o[0] + i, o[1] + j, o[2] + k};
-          bool clamped = false;
-          for (int a = 0; a < 3; ++a) {
-            if (gi[a] < 0) {
-              if (f->d.bc[2 * a] == AMR_BC_PERIODIC) gi[a] += domf[a]; else { gi[a] = 0; clamped = true; }
-            } else if (gi[a] >= domf[a]) {
-              if (f->d.bc[2 * a + 1] == AMR_BC_PERIODIC) gi[a] -= domf[a]; else { gi[a] = domf[a] - 1; clamped = true; }
-            }
+      const int rr[3] = {reg % 3, (reg / 3) % 3, reg / 9};
+      int plo[3], phi[3];
+      for (int a = 0; a < 3; ++a) {
+        int flo = o[a] + lo[rr[a]], fhi = o[a] + hi[rr[a]] - 1;      // fine index range of the region along a
+        // beyond a periodic face: the wrapped range; beyond an outflow face: the clamped cell
+        if (flo < 0) { if (f->d.bc[2 * a] == AMR_BC_PERIODIC) { flo += domf[a]; fhi += domf[a]; } else { flo = fhi = 0; } }
+        else if (fhi >= domf[a]) { if (f->d.bc[2 * a + 1] == AMR_BC_PERIODIC) { flo -= domf[a]; fhi -= domf[a]; } else { flo = fhi = domf[a] - 1; } }
+        plo[a] = flo / 2 - 1;
+        phi[a] = fhi / 2 + 1;
+      }
+      for (int cz = plo[2]; cz <= phi[2]; cz += (cz == phi[2] ? 1 : std::min(n, phi[2] - cz)))
+        for (int cy = plo[1]; cy <= phi[1]; cy += (cy == phi[1] ? 1 : std::min(n, phi[1] - cy)))
+          for (int cx = plo[0]; cx <= phi[0]; cx += (cx == phi[0] ? 1 : std::min(n, phi[0] - cx))) {
+            long long dummy;
+            if (!coarse_flat(cx, cy, cz, &dummy)) return fail(AMR_EINVAL, "fine patch %d has a halo cell with no coarse parent", p);
           }
-          // patch origins and domain sizes are even: the parity of a fine cell inside its parent
-          const long long par = (long long)(gi[0] & 1) | ((long long)(gi[1] & 1) << 1) | ((long long)(gi[2] & 1) << 2);
-          const long long cell = (long long)p * (long long)M3 + ((long long)(k + g) * M + (j + g)) * M + (i + g);
-          // patch origins are even: the parent's position in the patch's halo box is floor(offset / 2) + 2.  Several
-          // clamped cells share one (parent, child), so each of them gets an entry of its own
-          const int li = ((i + 4) >> 1), lj = ((j + 4) >> 1), lk = ((k + 4) >> 1);
-          int own = -1;
-          int& sl = clamped ? own : slot[((size_t)lk * hp + lj) * hp + li];
-          if (sl < 0) {   // first child of this parent: resolve the 7-point stencil in the coarse batch
-            const int C[3] = {gi[0] / 2, gi[1] / 2, gi[2] / 2};
-            long long s7[7];
-            bool ok = coarse_flat(C[0], C[1], C[2], &s7[0]);
-            for (int a = 0; a < 3 && ok; ++a) {
-              int Cm[3] = {C[0], C[1], C[2]}, Cp[3] = {C[0], C[1], C[2]};
-              Cm[a] -= 1;
-              Cp[a] += 1;
-              ok = coarse_flat(Cm[0], Cm[1], Cm[2], &s7[1 + 2 * a]) && coarse_flat(Cp[0], Cp[1], Cp[2], &s7[2 + 2 * a]);
-            }
-            if (!ok) return fail(AMR_EINVAL, "fine patch %d has a halo cell with no coarse parent", p);
-            sl = (int)(H.pro_dst.size() / 8);
-            for (int q = 0; q < 8; ++q) H.pro_dst.push_back(-1);
-            for (int q = 0; q < 7; ++q) H.pro_c7.push_back(s7[q]);
-          }
-          H.pro_dst[(size_t)sl * 8 + (size_t)par] = cell;
-        }
     }
   }
   // O9(6) list: entry e = (p, ck, cj, ci)
@@ -338,8 +306,8 @@ thread_local LinkCache g_link_cache;
 LinkLayout make_link_layout(const amr_patch_batch* c, const amr_patch_batch* f, const LinkHost& H) {
   LinkLayout L;
   size_t off = 0;
-  L.pro_dst = off; off += up(H.pro_dst.size() * 8 + 8);
-  L.pro_c7 = off; off += up(H.pro_c7.size() * 8 + 8);
+  L.forg = off; off += up((size_t)f->d.npatch * 3 * sizeof(int) + 8);
+  L.cmap = off; off += up(c->map.idx.size() * sizeof(int) + 8);
   L.res_dst = off; off += up(H.res_dst.size() * 8 + 8);
   L.faces = off; off += up(H.faces_all.size() * 8 + 8);
   const size_t n = f->d.n, blk = 3 * (size_t)f->d.nfields * 3 * n * n * f->esz;
@@ -868,10 +836,9 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   amr_level_link* l = new (std::nothrow) amr_level_link();
   if (!l) return fail(AMR_ENOMEM, "out of host memory");
   l->c = coarse; l->f = fine; l->ws = (char*)dev_ws; l->bytes = bytes;
-  l->pro_dst = (long long*)(l->ws + L.pro_dst);
-  l->pro_c7 = (long long*)(l->ws + L.pro_c7);
+  l->forg = (int*)(l->ws + L.forg);
+  l->cmap = (int*)(l->ws + L.cmap);
   l->res_dst = (long long*)(l->ws + L.res_dst);
-  l->npro = (int)(H.pro_dst.size() / 8);
   l->nres = (int)H.res_dst.size();
   l->faces = (long long*)(l->ws + L.faces);
   l->nfaces = (int)(H.faces_all.size() / 4);
@@ -884,8 +851,8 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   auto h2d = [&](void* dst, const void* src, size_t nb) {
     return nb ? cudaMemcpyAsync(dst, src, nb, cudaMemcpyHostToDevice, s) : cudaSuccess;
   };
-  cudaError_t e = h2d(l->pro_dst, H.pro_dst.data(), H.pro_dst.size() * 8);
-  if (e == cudaSuccess) e = h2d(l->pro_c7, H.pro_c7.data(), H.pro_c7.size() * 8);
+  cudaError_t e = h2d(l->forg, fine->origin.data(), fine->origin.size() * sizeof(int));
+  if (e == cudaSuccess) e = h2d(l->cmap, coarse->map.idx.data(), coarse->map.idx.size() * sizeof(int));
   if (e == cudaSuccess) e = h2d(l->res_dst, H.res_dst.data(), H.res_dst.size() * 8);
   if (e == cudaSuccess) e = h2d(l->faces, H.faces_all.data(), H.faces_all.size() * 8);
   if (e == cudaSuccess && !l->shared_c) e = h2d(coarse->fblk_of, H.fblk_of_c.data(), H.fblk_of_c.size() * sizeof(int));
@@ -921,8 +888,10 @@ int amr_prolong_ghosts(amr_level_link* l, double theta) {
   DeviceGuard guard(l->f->device);
   if (!(theta >= 0 && theta <= 1)) return fail(AMR_EINVAL, "theta must be in [0,1]");
   amr_patch_batch *c = l->c, *f = l->f;
-  cudaError_t e = amr::launch_prolong(f->d.dtype, f->halo, (size_t)f->d.npatch * f->M3, f->d.nfields, l->pro_dst, l->pro_c7,
-                                      l->npro, c->U[1 - c->cur], c->U[c->cur], (size_t)c->d.npatch * c->n3, theta, f->stream);
+  cudaError_t e = amr::launch_prolong_halo(f->d.dtype, f->halo, (size_t)f->d.npatch * f->M3, f->d.nfields, f->d.n, f->d.nghost,
+                                           f->d.npatch, f->d.domain_cells, c->d.domain_cells, c->map.dims, f->d.bc, l->forg,
+                                           f->nbr_dev, l->cmap, c->U[1 - c->cur], c->U[c->cur], (size_t)c->d.npatch * c->n3,
+                                           theta, f->stream);
   if (e != cudaSuccess) return fail(AMR_ECUDA, "prolong kernel launch: %s", cudaGetErrorString(e));
   f->halo_valid = true;
   return AMR_OK;
@@ -1001,8 +970,10 @@ int stream_after(cudaStream_t waiter, cudaStream_t producer, cudaEvent_t ev) {
 // amr_prolong_ghosts(l, 0) reads after it): lets the fine level's first substep run beside the coarse step
 int prolong_from_current(amr_level_link* l) {
   amr_patch_batch *c = l->c, *f = l->f;
-  cudaError_t e = amr::launch_prolong(f->d.dtype, f->halo, (size_t)f->d.npatch * f->M3, f->d.nfields, l->pro_dst, l->pro_c7,
-                                      l->npro, c->U[c->cur], c->U[c->cur], (size_t)c->d.npatch * c->n3, 0.0, f->stream);
+  cudaError_t e = amr::launch_prolong_halo(f->d.dtype, f->halo, (size_t)f->d.npatch * f->M3, f->d.nfields, f->d.n, f->d.nghost,
+                                           f->d.npatch, f->d.domain_cells, c->d.domain_cells, c->map.dims, f->d.bc, l->forg,
+                                           f->nbr_dev, l->cmap, c->U[c->cur], c->U[c->cur], (size_t)c->d.npatch * c->n3, 0.0,
+                                           f->stream);
   if (e != cudaSuccess) return fail(AMR_ECUDA, "prolong kernel launch: %s", cudaGetErrorString(e));
   f->halo_valid = true;
   return AMR_OK;
