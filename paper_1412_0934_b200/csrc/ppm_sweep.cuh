@@ -118,7 +118,6 @@ __global__ void __launch_bounds__(PB * 66) ppm_sweep_kernel(const __grid_constan
   }
   __syncthreads();
 
-
   // ---- P1..P4: traced states of the cells -1 .. n ------------------------------------------------------------
   const bool active = true;
   {
@@ -159,22 +158,14 @@ __global__ void __launch_bounds__(PB * 66) ppm_sweep_kernel(const __grid_constan
         wp[0] -= (ref[0] - Ip(0, sg)) - (ref[4] - Ip(4, sg)) * ic2;
         wp[2] = Ip(2, sg); wp[3] = Ip(3, sg);
       }
-      if (lk[2] > T(0)) {
-        const T sg = lk[2] * lam;
-        const T b = T(0.5) * (roc * (ref[1] - Ip(1, sg)) + (ref[4] - Ip(4, sg)) * ic2);
-        wp[0] -= b; wp[1] -= b * cor; wp[4] -= b * c2;
-      }
+      // (the lambda_+ wave: its average IS the reference state, its correction is exactly zero)
     }
     {
       const T sref = rmax(-lk[0], T(0)) * lam;
       T ref[5];
 #pragma unroll
       for (int m = 0; m < 5; ++m) { ref[m] = Im(m, sref); wm[m] = ref[m]; }
-      if (lk[0] < T(0)) {
-        const T sg = -lk[0] * lam;
-        const T b = T(0.5) * (-roc * (ref[1] - Im(1, sg)) + (ref[4] - Im(4, sg)) * ic2);
-        wm[0] -= b; wm[1] += b * cor; wm[4] -= b * c2;
-      }
+      // (the lambda_- wave: its average IS the reference state, its correction is exactly zero)
       if (lk[1] < T(0)) {
         const T sg = -lk[1] * lam;
         wm[0] -= (ref[0] - Im(0, sg)) - (ref[4] - Im(4, sg)) * ic2;
