@@ -98,7 +98,9 @@ cudaError_t launch_copy_patches(int dtype, void* Unew, size_t fs_new, const void
                                 int npairs, int nf, int n, cudaStream_t s);
 cudaError_t launch_copy_patches_in(int dtype, void* U, size_t fs, const void* packed, size_t fs_packed, const void* pairs,
                                    int npairs, int nf, int n, cudaStream_t s);
-cudaError_t launch_prolong_patches(int dtype, void* Unew, size_t fs_new, int nf, int n, const int* born, const long long* c7,
-                                   int nparents, const void* Uc, size_t fs_c, cudaStream_t s);
+// born: int4 (new patch index, fine origin x, y, z) per new-born patch (device); cmap, domc, cdims, bc as launch_prolong_halo
+cudaError_t launch_prolong_patches(int dtype, void* Unew, size_t fs_new, int nf, int n, const int* domc, const int* cdims,
+                                   const int* bc, const void* born, const int* cmap, int nparents, const void* Uc,
+                                   size_t fs_c, cudaStream_t s);
 
 }  // namespace amr

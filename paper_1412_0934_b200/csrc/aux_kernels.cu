@@ -237,23 +237,39 @@ __global__ void __launch_bounds__(256) copy_patches_kernel(T* __restrict__ Unew,
   for (int r = threadIdx.x; r < n3; r += blockDim.x) dst[r] = src[r];
 }
 
-// new-born patches: one thread per coarse parent cell; born[b] = new patch index, c7[(b h^3 + r) 7 + .] = flat
-// coarse interior indices (centre, x-, x+, y-, y+, z-, z+) of parent r = (ck h + cj) h + ci.  The 8 children get
-// U_C -+ 1/4 minmod slopes, accumulated in the order x, y, z (as prolong_kernel, O8).
+// new-born patches, no tables (as prolong_halo_kernel): one thread per coarse parent cell; born[b] = (new patch index,
+// fine origin x, y, z).  The parent block of a patch ((n/2)^3 coarse cells from origin / 2) lies inside ONE coarse
+// patch; only the +-1 stencil can leave it, and it is resolved through the coarse patch map (periodic faces wrap, the
+// stencil clamps at an outflow face like the coarse ghosts).  The 8 children get U_C -+ 1/4 minmod slopes,
+// accumulated in the order x, y, z (O8).
 template <class T>
-__global__ void __launch_bounds__(128) prolong_patches_kernel(T* __restrict__ Unew, size_t fs_new, int nf, int n,
-                                                              const int* __restrict__ born,
-                                                              const long long* __restrict__ c7, int nparents,
+__global__ void __launch_bounds__(128) prolong_patches_kernel(T* __restrict__ Unew, size_t fs_new, int nf, ProlongGeom G,
+                                                              const int4* __restrict__ born,
+                                                              const int* __restrict__ cmap, int nparents,
                                                               const T* __restrict__ Uc, size_t fs_c) {
   const int e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= nparents) return;
-  const int h = n >> 1, h3 = h * h * h;
+  const int n = G.n, h = n >> 1, h3 = h * h * h;
   const int b = e / h3, r = e - b * h3;
   const int ci = r % h, cj = (r / h) % h, ck = r / (h * h);
-  long long s[7];
+  const int4 bo = born[b];
+  const int C[3] = {(bo.y >> 1) + ci, (bo.z >> 1) + cj, (bo.w >> 1) + ck};
+  auto coarse_flat = [&](int cx, int cy, int cz) -> long long {
+    int c[3] = {cx, cy, cz};
 #pragma unroll
-  for (int k = 0; k < 7; ++k) s[k] = c7[(size_t)e * 7 + k];
-  T* dst0 = Unew + (size_t)born[b] * n * n * n + ((size_t)(2 * ck) * n + 2 * cj) * n + 2 * ci;
+    for (int a = 0; a < 3; ++a) {
+      if (c[a] < 0) c[a] = G.per_lo[a] ? c[a] + G.domc[a] : 0;
+      else if (c[a] >= G.domc[a]) c[a] = G.per_hi[a] ? c[a] - G.domc[a] : G.domc[a] - 1;
+    }
+    const int pc = cmap[((c[2] / n) * G.cdims[1] + c[1] / n) * G.cdims[0] + c[0] / n];   // nesting was checked by the host
+    return (long long)pc * n * n * n + ((long long)(c[2] % n) * n + (c[1] % n)) * n + (c[0] % n);
+  };
+  long long s[7];
+  s[0] = coarse_flat(C[0], C[1], C[2]);
+  s[1] = coarse_flat(C[0] - 1, C[1], C[2]); s[2] = coarse_flat(C[0] + 1, C[1], C[2]);
+  s[3] = coarse_flat(C[0], C[1] - 1, C[2]); s[4] = coarse_flat(C[0], C[1] + 1, C[2]);
+  s[5] = coarse_flat(C[0], C[1], C[2] - 1); s[6] = coarse_flat(C[0], C[1], C[2] + 1);
+  T* dst0 = Unew + (size_t)bo.x * n * n * n + ((size_t)(2 * ck) * n + 2 * cj) * n + 2 * ci;
   for (int q = 0; q < nf; ++q) {
     const T* a = Uc + (size_t)q * fs_c;
     T st[7];
@@ -264,12 +280,15 @@ __global__ void __launch_bounds__(128) prolong_patches_kernel(T* __restrict__ Un
     for (int dd = 0; dd < 3; ++dd) sl[dd] = minmod2<T>(st[0] - st[1 + 2 * dd], st[2 + 2 * dd] - st[0]);
     T* dst = dst0 + (size_t)q * fs_new;
 #pragma unroll
-    for (int c = 0; c < 8; ++c) {
-      T val = st[0];
-      val += ((c & 1) ? T(0.25) : T(-0.25)) * sl[0];
-      val += ((c & 2) ? T(0.25) : T(-0.25)) * sl[1];
-      val += ((c & 4) ? T(0.25) : T(-0.25)) * sl[2];
-      dst[((size_t)((c >> 2) & 1) * n + ((c >> 1) & 1)) * n + (c & 1)] = val;
+    for (int c = 0; c < 4; ++c) {       // the two x children of a (y, z) child pair go out as one vector store
+      T lo = st[0], hi = st[0];
+      lo += T(-0.25) * sl[0]; hi += T(0.25) * sl[0];
+      const T sy = ((c & 1) ? T(0.25) : T(-0.25)) * sl[1], sz = ((c & 2) ? T(0.25) : T(-0.25)) * sl[2];
+      lo += sy; hi += sy;
+      lo += sz; hi += sz;
+      T* d2 = dst + ((size_t)((c >> 1) & 1) * n + (c & 1)) * n;
+      if constexpr (sizeof(T) == 4) *reinterpret_cast<float2*>(d2) = make_float2(lo, hi);
+      else *reinterpret_cast<double2*>(d2) = make_double2(lo, hi);
     }
   }
 }
@@ -539,14 +558,23 @@ cudaError_t launch_copy_patches_in(int dtype, void* U, size_t fs, const void* pa
   return cudaGetLastError();
 }
 
-cudaError_t launch_prolong_patches(int dtype, void* Unew, size_t fs_new, int nf, int n, const int* born, const long long* c7,
-                                   int nparents, const void* Uc, size_t fs_c, cudaStream_t s) {
+cudaError_t launch_prolong_patches(int dtype, void* Unew, size_t fs_new, int nf, int n, const int* domc, const int* cdims,
+                                   const int* bc, const void* born, const int* cmap, int nparents, const void* Uc,
+                                   size_t fs_c, cudaStream_t s) {
   if (nparents == 0) return cudaSuccess;
+  ProlongGeom G;
+  G.n = n; G.g = 0; G.npf = 0;
+  for (int a = 0; a < 3; ++a) {
+    G.domf[a] = 2 * domc[a]; G.domc[a] = domc[a]; G.cdims[a] = cdims[a];
+    G.per_lo[a] = bc[2 * a] == 0; G.per_hi[a] = bc[2 * a + 1] == 0;   // AMR_BC_PERIODIC == 0
+  }
   const unsigned grid = (unsigned)((nparents + 127) / 128);
   if (dtype == 0)
-    prolong_patches_kernel<float><<<grid, 128, 0, s>>>((float*)Unew, fs_new, nf, n, born, c7, nparents, (const float*)Uc, fs_c);
+    prolong_patches_kernel<float><<<grid, 128, 0, s>>>((float*)Unew, fs_new, nf, G, (const int4*)born, cmap, nparents,
+                                                       (const float*)Uc, fs_c);
   else
-    prolong_patches_kernel<double><<<grid, 128, 0, s>>>((double*)Unew, fs_new, nf, n, born, c7, nparents, (const double*)Uc, fs_c);
+    prolong_patches_kernel<double><<<grid, 128, 0, s>>>((double*)Unew, fs_new, nf, G, (const int4*)born, cmap, nparents,
+                                                        (const double*)Uc, fs_c);
   return cudaGetLastError();
 }
 

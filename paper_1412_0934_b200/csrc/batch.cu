@@ -1132,11 +1132,10 @@ bool coarse_cell_flat(const amr_patch_batch* c, int Cx, int Cy, int Cz, long lon
 
 struct RegridHost {
   std::vector<int> pairs;       // (new, old) per kept patch
-  std::vector<int> born;        // new patch index per new-born patch
-  std::vector<long long> c7;    // [born][h^3][7]
+  std::vector<int> born;        // (new patch index, fine origin x, y, z) per new-born patch
 };
 
-struct RegridLayout { size_t pairs, born, c7, total; };
+struct RegridLayout { size_t pairs, born, cmap, total; };
 
 int check_regrid_args(const amr_patch_batch* nw, const amr_patch_batch* old, const amr_patch_batch* c) {
   if (!nw || !c) return fail(AMR_EINVAL, "null batch");
@@ -1151,38 +1150,38 @@ int check_regrid_args(const amr_patch_batch* nw, const amr_patch_batch* old, con
   return AMR_OK;
 }
 
+// The prolongation of a new-born patch resolves its parents in the kernel (prolong_patches_kernel); what the host
+// owes is the nesting check.  The parent block of a patch lies inside one coarse patch (origins are multiples of n,
+// the block spans n/2), so the 7-point stencils of all its cells exist iff that patch and, along each axis, the
+// coarse patch holding the cell one beyond the block's low and high face (wrapped / clamped) exist.
 int build_regrid(const amr_patch_batch* nw, const amr_patch_batch* old, const amr_patch_batch* c, RegridHost& H) {
   const int n = nw->d.n, h = n / 2;
+  long long flat;
   for (int p = 0; p < nw->d.npatch; ++p) {
     const int* o = &nw->origin[3 * p];
     const int po = old ? old->map.at(o[0] / n, o[1] / n, o[2] / n) : -1;
     if (po >= 0) { H.pairs.push_back(p); H.pairs.push_back(po); continue; }
+    const int C[3] = {o[0] / 2, o[1] / 2, o[2] / 2};
+    bool ok = coarse_cell_flat(c, C[0], C[1], C[2], &flat);
+    for (int a = 0; a < 3 && ok; ++a) {
+      int Cm[3] = {C[0], C[1], C[2]}, Cp[3] = {C[0], C[1], C[2]};
+      Cm[a] -= 1;
+      Cp[a] += h;
+      ok = coarse_cell_flat(c, Cm[0], Cm[1], Cm[2], &flat) && coarse_cell_flat(c, Cp[0], Cp[1], Cp[2], &flat);
+    }
+    if (!ok) return fail(AMR_EINVAL, "new patch %d is not properly nested in the coarse level (a parent cell or its stencil is missing)", p);
     H.born.push_back(p);
-    for (int ck = 0; ck < h; ++ck)
-      for (int cj = 0; cj < h; ++cj)
-        for (int ci = 0; ci < h; ++ci) {
-          const int C[3] = {o[0] / 2 + ci, o[1] / 2 + cj, o[2] / 2 + ck};
-          long long s7[7];
-          bool ok = coarse_cell_flat(c, C[0], C[1], C[2], &s7[0]);
-          for (int a = 0; a < 3 && ok; ++a) {
-            int Cm[3] = {C[0], C[1], C[2]}, Cp[3] = {C[0], C[1], C[2]};
-            Cm[a] -= 1;
-            Cp[a] += 1;
-            ok = coarse_cell_flat(c, Cm[0], Cm[1], Cm[2], &s7[1 + 2 * a]) && coarse_cell_flat(c, Cp[0], Cp[1], Cp[2], &s7[2 + 2 * a]);
-          }
-          if (!ok) return fail(AMR_EINVAL, "new patch %d is not properly nested in the coarse level (a parent cell or its stencil is missing)", p);
-          for (int q = 0; q < 7; ++q) H.c7.push_back(s7[q]);
-        }
+    for (int a = 0; a < 3; ++a) H.born.push_back(o[a]);
   }
   return AMR_OK;
 }
 
-RegridLayout make_regrid_layout(const RegridHost& H) {
+RegridLayout make_regrid_layout(const RegridHost& H, const amr_patch_batch* c) {
   RegridLayout L;
   size_t off = 0;
   L.pairs = off; off += up(H.pairs.size() * sizeof(int) + 8);
   L.born = off; off += up(H.born.size() * sizeof(int) + 8);
-  L.c7 = off; off += up(H.c7.size() * 8 + 8);
+  L.cmap = off; off += up(c->map.idx.size() * sizeof(int) + 8);
   L.total = off;
   return L;
 }
@@ -1213,7 +1212,7 @@ size_t amr_regrid_bytes(const amr_patch_batch* new_fine, const amr_patch_batch* 
   if (check_regrid_args(new_fine, old_fine, coarse) != AMR_OK) return 0;
   RegridHost H;
   if (build_regrid(new_fine, old_fine, coarse, H) != AMR_OK) return 0;
-  return make_regrid_layout(H).total;
+  return make_regrid_layout(H, coarse).total;
 }
 
 int amr_regrid_fill(amr_patch_batch* new_fine, const amr_patch_batch* old_fine, const amr_patch_batch* coarse, void* dev_ws,
@@ -1227,7 +1226,7 @@ int amr_regrid_fill(amr_patch_batch* new_fine, const amr_patch_batch* old_fine, 
   RegridHost H;
   rc = build_regrid(new_fine, old_fine, coarse, H);
   if (rc != AMR_OK) return rc;
-  const RegridLayout L = make_regrid_layout(H);
+  const RegridLayout L = make_regrid_layout(H, coarse);
   if (bytes < L.total) return fail(AMR_EINVAL, "workspace too small: %zu < %zu bytes", bytes, L.total);
   cudaStream_t s = new_fine->stream;
   char* ws = (char*)dev_ws;
@@ -1236,15 +1235,16 @@ int amr_regrid_fill(amr_patch_batch* new_fine, const amr_patch_batch* old_fine, 
   };
   cudaError_t e = h2d(ws + L.pairs, H.pairs.data(), H.pairs.size() * sizeof(int));
   if (e == cudaSuccess) e = h2d(ws + L.born, H.born.data(), H.born.size() * sizeof(int));
-  if (e == cudaSuccess) e = h2d(ws + L.c7, H.c7.data(), H.c7.size() * 8);
+  if (e == cudaSuccess) e = h2d(ws + L.cmap, coarse->map.idx.data(), coarse->map.idx.size() * sizeof(int));
   const int nf = new_fine->d.nfields, n = new_fine->d.n, h = n / 2;
   const size_t fs_new = (size_t)new_fine->d.npatch * new_fine->n3;
   if (e == cudaSuccess && old_fine)
     e = amr::launch_copy_patches(new_fine->d.dtype, new_fine->U[new_fine->cur], fs_new, old_fine->U[old_fine->cur],
                                  (size_t)old_fine->d.npatch * old_fine->n3, ws + L.pairs, (int)(H.pairs.size() / 2), nf, n, s);
   if (e == cudaSuccess)
-    e = amr::launch_prolong_patches(new_fine->d.dtype, new_fine->U[new_fine->cur], fs_new, nf, n, (const int*)(ws + L.born),
-                                    (const long long*)(ws + L.c7), (int)H.born.size() * h * h * h, coarse->U[coarse->cur],
+    e = amr::launch_prolong_patches(new_fine->d.dtype, new_fine->U[new_fine->cur], fs_new, nf, n, coarse->d.domain_cells,
+                                    coarse->map.dims, coarse->d.bc, ws + L.born, (const int*)(ws + L.cmap),
+                                    (int)(H.born.size() / 4) * h * h * h, coarse->U[coarse->cur],
                                     (size_t)coarse->d.npatch * coarse->n3, s);
   // the tables are host vectors: the copies above must have left them before they go out of scope
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
