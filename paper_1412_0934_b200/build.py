@@ -4,6 +4,10 @@
 with nvcc (``-gencode arch=compute_100a,code=sm_100a -lineinfo``), in parallel, and links them into
 ``paper_1412_0934_b200/libamrgodunov.so`` (in-tree, git-ignored; it travels to the GPU box with the
 snapshot).  nvcc cross-compiles without a GPU.
+
+``python -m paper_1412_0934_b200.build --microbench`` also compiles the stand-alone diagnostic programs of
+``csrc/microbench/*.cu`` into ``paper_1412_0934_b200/build/microbench/`` (not part of the library; the profiles
+that quote them name the command).
 """
 from __future__ import annotations
 
@@ -66,5 +70,24 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_microbench() -> list:
+    src_dir = os.path.join(CSRC, "microbench")
+    out_dir = os.path.join(OBJ, "microbench")
+    os.makedirs(out_dir, exist_ok=True)
+    outs = []
+    for f in sorted(os.listdir(src_dir)):
+        if not f.endswith(".cu"):
+            continue
+        exe = os.path.join(out_dir, f[:-3])
+        cmd = [NVCC] + ARCH + ["-O3", "-std=c++17", "-lineinfo", "-I", INCLUDE, "-I", CSRC, os.path.join(src_dir, f), "-o", exe]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("nvcc failed on %s:\n%s\n%s" % (f, r.stdout, r.stderr))
+        outs.append(exe)
+    return outs
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--microbench" in sys.argv:
+        print("\n".join(build_microbench()))
