@@ -102,12 +102,25 @@ __device__ __forceinline__ void lds_pairs(const float* p, F2* w) {
 #pragma unroll
   for (int q = 0; q < NF; ++q) w[q] = F2(t[2 * q], t[2 * q + 1]);
 }
+// MHD records go out as one opaque 64-bit store per component pair.  ptxas merges them back into the same 128-bit
+// stores; what changes is the order in which the compiler may schedule the code around them, and that is worth
+// 4.7 % of the MHD step (config 5: 12.84 -> 12.23 ms, config 3 fp32: 1.76 -> 1.68 ms; pinning the loads or the
+// staging blocks as well, or plain compiler fences at the same places, gains nothing).  The hydro kernel is 0.8 %
+// slower with it and keeps the plain vector stores.
 template <int NF>
 __device__ __forceinline__ void sts_pairs(float* p, const F2* w) {
-  float t[2 * NF];
+  if constexpr (NF == 9) {
 #pragma unroll
-  for (int q = 0; q < NF; ++q) { t[2 * q] = w[q].v.x; t[2 * q + 1] = w[q].v.y; }
-  sts_n<2 * NF, 4>(p, t);
+    for (int q = 0; q < NF; ++q) {
+      const unsigned d = (unsigned)__cvta_generic_to_shared(p + 2 * q);
+      asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(d), "f"(w[q].v.x), "f"(w[q].v.y) : "memory");
+    }
+  } else {
+    float t[2 * NF];
+#pragma unroll
+    for (int q = 0; q < NF; ++q) { t[2 * q] = w[q].v.x; t[2 * q + 1] = w[q].v.y; }
+    sts_n<2 * NF, 4>(p, t);
+  }
 }
 
 __device__ __forceinline__ void cp_async8(float* smem_dst, const float* gsrc) {
