@@ -13,7 +13,11 @@
 #include <vector>
 #include "godunov_step_x2.cuh"
 using namespace amr; using namespace amr::x2;
-constexpr int NF = 9, REC = 20, NPX = 18;
+#ifndef ITEM_NF
+#define ITEM_NF 9          // -DITEM_NF=5: the hydro items (HLLC)
+#endif
+constexpr int NF = ITEM_NF, REC = NF == 9 ? 20 : 12, NPX = 18;
+constexpr int RSV = NF == 9 ? X2_RS_HLLD : X2_RS_HLLC;
 
 template <int MODE, int MAXR, int BAR = 1>
 __global__ void __maxnreg__(MAXR) mb(const __grid_constant__ StepParams<float> P, const float* __restrict__ init, int RH, int npool, int niter,
@@ -55,7 +59,7 @@ __global__ void __maxnreg__(MAXR) mb(const __grid_constant__ StepParams<float> P
         F2 WL[NF], WR[NF], F[NF];
         lds_pairs<NF>(pool + lo * REC, WL);
         lds_pairs<NF>(pool + ro * REC, WR);
-        riemann2<NF, X2_RS_HLLD>(WL, WR, RC, F, B2(true), s_cnt);
+        riemann2<NF, RSV>(WL, WR, RC, F, B2(true), s_cnt);
         sts_pairs<NF>(fpool + ((tid + rep * NT) % (npool / 2)) * REC, F);
       }
     }
@@ -106,10 +110,12 @@ int main() {
       d[0 + half] = 1.f + 0.3f * rnd();
       d[2 + half] = 0.8f * rnd(); d[4 + half] = 0.8f * rnd(); d[6 + half] = 0.8f * rnd();
       d[8 + half] = 1.f + 0.3f * rnd();
-      d[10 + half] = 0.2f * rnd(); d[12 + half] = 0.2f * rnd(); d[14 + half] = 0.2f * rnd();
-      d[16 + half] = 0.01f * rnd();
+      if (NF == 9) {
+        d[10 + half] = 0.2f * rnd(); d[12 + half] = 0.2f * rnd(); d[14 + half] = 0.2f * rnd();
+        d[16 + half] = 0.01f * rnd();
+      }
     }
-    d[18] = d[19] = 0.f;
+    for (int i = 2 * NF; i < REC; ++i) d[i] = 0.f;
   }
   float *dinit, *dsink;
   cudaMalloc(&dinit, tot * 4);
