@@ -148,9 +148,11 @@ int amr_conserved_totals(amr_patch_batch* b, double* totals);
 int amr_step_counters(amr_patch_batch* b, long long* counters, int reset);
 
 /* ---- two-level operators (O8, O9; config 4) ------------------------------------------------- */
-/* Device workspace a link needs (flux registers, restriction and reflux tables, the coarse patch map and the fine
- * origins; the prolongation needs no table: its kernel resolves the parents itself); 0 on error.  Also checks proper
- * nesting: every fine halo region no sibling covers, and its +-1 stencil, must lie inside coarse patches. */
+/* Device workspace a link needs (flux registers, the patch maps of both levels, the fine origins and the list of
+ * coarse patches that record fluxes; prolongation, restriction and reflux need no per-cell table: their kernels
+ * resolve parents and neighbours through the maps); 0 on error.  Also checks proper nesting: every fine halo region
+ * no sibling covers, and its +-1 stencil, must lie inside coarse patches; every fine patch and the coarse cells
+ * outside its faces must be covered by the coarse level. */
 size_t amr_link_bytes(const amr_patch_batch* coarse, const amr_patch_batch* fine, int ratio);
 /* Ties a fine batch to its parent level (ratio must be 2).  dev_ws: device, borrowed like an arena.
  * From then on steps of both batches also record the face fluxes the reflux needs.

@@ -83,13 +83,22 @@ cudaError_t launch_prolong_halo(int dtype, void* halo, size_t fs_halo, int nf, i
                                 const int* domc, const int* cdims, const int* bc, const int* forigin, const int* nbr,
                                 const int* cmap, const void* Ucold, const void* Ucnew, size_t fs_c, double theta,
                                 cudaStream_t s);
-cudaError_t launch_restrict(int dtype, const void* Uf, size_t fs_f, int nf, int n, const long long* dst, int nent,
-                            void* Uc, size_t fs_c, cudaStream_t s);
-cudaError_t launch_reflux(int dtype, void* Uc, size_t fs_c, int nf, int n, const long long* faces, int nfaces,
-                          const void* Fc, const void* Ff, double dtdx, cudaStream_t s);
-
-// zeroes, for every entry of a reflux face table, the coarse flux slot it names (all fields)
-cudaError_t launch_zero_faces(int dtype, void* Fc, int nf, int n, const long long* faces, int nfaces, cudaStream_t s);
+// O9(6) without a table: the parent block of fine patch p is found through forigin (device, [npf][3]) and cmap
+cudaError_t launch_restrict(int dtype, const void* Uf, size_t fs_f, int nf, int n, int npf, const int* domc, const int* cdims,
+                            const int* bc, const int* forigin, const int* cmap, void* Uc, size_t fs_c, cudaStream_t s);
+// O9(7) without a host table.  cblk (device): int4 (coarse patch, its origin x, y, z) per coarse flux block, block
+// index = position (shared = 0) or = patch (shared = 1: the coarse level records per patch); fmap (device): fine patch
+// map [fdims z][y][x], -1 = not refined.  launch_reflux_find (link time) fills `list` (device, int2 per uncovered
+// coarse cell with a covered face neighbour: flat cell index, block position << 6 | mask of (direction, side)) and
+// *count (device; may exceed capacity: the caller checks); launch_reflux / launch_zero_faces give every entry a thread.
+cudaError_t launch_reflux_find(int nf, int n, int shared, const int* domc, const int* fdims, const int* bc, const void* cblk,
+                               int ncblk, const int* fmap, void* list, int* count, int capacity, cudaStream_t s);
+cudaError_t launch_reflux(int dtype, void* Uc, size_t fs_c, int nf, int n, int shared, const int* domc, const int* fdims,
+                          const int* bc, const void* cblk, const void* list, int nlist, const int* fmap, const int* forigin,
+                          void* Fc, const void* Ff, double dtdx, cudaStream_t s);
+// zeroes the coarse flux slots a reflux of this link reads (all fields)
+cudaError_t launch_zero_faces(int dtype, void* Fc, int nf, int n, int shared, const int* domc, const int* fdims, const int* bc,
+                              const void* cblk, const void* list, int nlist, cudaStream_t s);
 
 // regridding (aux_kernels.cu): block flags of one field [np*8]; whole-patch copies; whole-patch prolongation
 cudaError_t launch_flag_blocks(int dtype, const void* Ufield, int np, int n, double threshold, unsigned char* flags,

@@ -294,21 +294,24 @@ __global__ void __launch_bounds__(128) prolong_patches_kernel(T* __restrict__ Un
 }
 
 // ---- O9(6): restriction ---------------------------------------------------------------------------
-// entry e <-> (fine patch p, coarse-cell offset inside the patch); dst[e] = flat coarse interior index
+// No table: entry e <-> (fine patch p, coarse-cell offset (ci, cj, ck) inside the patch's parent block); the parent
+// block of a fine patch lies in ONE coarse patch, found through the coarse patch map (nesting was checked at link time).
 template <class T>
-__global__ void __launch_bounds__(256) restrict_kernel(const T* __restrict__ Uf, size_t fs_f, int nf, int n,
-                                                       const long long* __restrict__ dst, int nent,
-                                                       T* __restrict__ Uc, size_t fs_c) {
+__global__ void __launch_bounds__(256) restrict_kernel(const T* __restrict__ Uf, size_t fs_f, int nf, ProlongGeom G,
+                                                       const int* __restrict__ forigin, const int* __restrict__ cmap,
+                                                       int nent, T* __restrict__ Uc, size_t fs_c) {
   const int e = blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= nent) return;
-  const int h = n / 2, h3 = h * h * h;
+  const int n = G.n, h = n / 2, h3 = h * h * h;
   const int p = e / h3;
   int r = e - p * h3;
   const int ck = r / (h * h);
   r -= ck * h * h;
   const int cj = r / h, ci = r - cj * h;
   const size_t base = (size_t)p * n * n * n + ((size_t)(2 * ck) * n + 2 * cj) * n + 2 * ci;
-  const size_t d = (size_t)dst[e];
+  const int Cx = (forigin[3 * p] >> 1) + ci, Cy = (forigin[3 * p + 1] >> 1) + cj, Cz = (forigin[3 * p + 2] >> 1) + ck;
+  const int pc = cmap[((Cz / n) * G.cdims[1] + Cy / n) * G.cdims[0] + Cx / n];
+  const size_t d = (size_t)pc * n * n * n + ((size_t)(Cz % n) * n + (Cy % n)) * n + (Cx % n);
   for (int q = 0; q < nf; ++q) {
     const T* u = Uf + (size_t)q * fs_f + base;
     T s = T(0);
@@ -322,52 +325,132 @@ __global__ void __launch_bounds__(256) restrict_kernel(const T* __restrict__ Uf,
   }
 }
 
-template <class T>
-__global__ void __launch_bounds__(256) zero_faces_kernel(T* __restrict__ Fc, int nf, size_t fsz,
-                                                         const long long* __restrict__ faces, int nfaces) {
-  const int e = blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= nfaces) return;
-  const size_t oc = (size_t)faces[(size_t)e * 4 + 1];
-  for (int q = 0; q < nf; ++q) Fc[oc + (size_t)q * fsz] = T(0);
+// ---- O9(7): reflux --------------------------------------------------------------------------------
+// No host table.  At link time reflux_find_kernel scans the cells of every coarse patch that owns a flux block
+// (cblk[b] = (patch, origin x, y, z); block index = b, or = patch when the coarse level records per patch because it
+// is a fine level itself) and appends to a device list every cell that is not covered by the fine level but has a
+// covered face neighbour: entry = (flat cell index in the level, b << 6 | mask), mask bit d*2 + s set when the
+// neighbour across (direction d, fine side s) is covered - fine side 0: the neighbour above (the interface is the fine
+// patch's low face and this cell's upper face), 1: the neighbour below.  Neighbours are found through the fine patch
+// map (periodic faces wrap; beyond a non-periodic face there is nothing: a fine face on the domain boundary carries a
+// boundary flux of the composite grid).  The list order is arbitrary (atomic counter) and does
+// not matter: reflux_list_kernel gives every entry one thread, which applies
+//   U_C += s_f (dt/dx) (F_coarse - 1/4 * 1/2 * sum of the 4 fine face fluxes summed over the two substeps)
+// for its set bits in ascending (d, s) - every cell is corrected by one thread in a fixed order.  ZERO: instead clear
+// the coarse flux slots those corrections read (a middle level shares its blocks with its role as a fine level and
+// must not clear more than its own faces).
+// Flux blocks: [block][direction][field][3 face planes: index 0, n/2, n along the normal][n^2 in-plane, the lower
+// remaining axis fastest].
+struct RefluxGeom {
+  int n, nf, shared;
+  int domc[3], fdims[3];
+  int per_lo[3], per_hi[3];
+};
+
+__device__ __forceinline__ int fine_patch_of(const RefluxGeom& G, const int* __restrict__ fmap, const int* c) {
+  const int n = G.n;   // the fine patch covering the children of coarse cell c, or -1
+  return fmap[(((2 * c[2]) / n) * G.fdims[1] + (2 * c[1]) / n) * G.fdims[0] + (2 * c[0]) / n];
+}
+// neighbour of C across (d, side) in level coordinates; false beyond a non-periodic face
+__device__ __forceinline__ bool reflux_neighbour(const RefluxGeom& G, const int* C, int d, int side, int* Cn) {
+  Cn[0] = C[0]; Cn[1] = C[1]; Cn[2] = C[2];
+  Cn[d] += side ? -1 : 1;
+  if (Cn[d] < 0) { if (!G.per_lo[d]) return false; Cn[d] += G.domc[d]; }
+  else if (Cn[d] >= G.domc[d]) { if (!G.per_hi[d]) return false; Cn[d] -= G.domc[d]; }
+  return true;
 }
 
-// ---- O9(7): reflux --------------------------------------------------------------------------------
-// faces[e][4] = { flat coarse interior index of the cell to correct,
-//                 flat offset of the coarse flux inside field 0 of the coarse flux-block array,
-//                 flat offset of the first of the 4 fine fluxes inside field 0 of the fine flux-block array,
-//                 code: bit0 = sign (1: s_f = -1), bits 1..2 = d }.
-// elements between fields inside one (block, d) slab = 3 n^2 (the face planes 0, n/2, n).
-template <class T>
-__global__ void __launch_bounds__(256) reflux_kernel(T* __restrict__ Uc, size_t fs_c, int nf, int n,
-                                                     const long long* __restrict__ faces, int nfaces,
-                                                     const T* __restrict__ Fc, const T* __restrict__ Ff, T dtdx) {
-  int e = blockIdx.x * blockDim.x + threadIdx.x;
-  if (e >= nfaces) return;
-  // the table is sorted by coarse cell: the thread at the first entry of a cell applies all of that cell's entries
-  // in table order ((direction, side) ascending), every other thread of the run has nothing to do
-  const long long cell_ll = faces[(size_t)e * 4 + 0];
-  if (e > 0 && faces[(size_t)(e - 1) * 4 + 0] == cell_ll) return;
-  const size_t cell = (size_t)cell_ll;
-  const size_t fsz = (size_t)3 * n * n;
-  for (; e < nfaces && faces[(size_t)e * 4 + 0] == cell_ll; ++e) {
-    const size_t oc = (size_t)faces[(size_t)e * 4 + 1];
-    const size_t of = (size_t)faces[(size_t)e * 4 + 2];
-    const int code = (int)faces[(size_t)e * 4 + 3];
-    const T sf = (code & 1) ? T(-1) : T(1);
-    const int d = (code >> 1) & 3;
-    // strides of the two transverse directions t1 = (d+1)%3 (a), t2 = (d+2)%3 (b) inside a face plane, whose
-    // in-plane layout has the lower remaining axis fastest: d = 0: (z, y), d = 1: (z, x), d = 2: (y, x)
-    const size_t sa = (d == 1) ? (size_t)n : 1, sb = (d == 1) ? 1 : (size_t)n;
-    for (int q = 0; q < nf; ++q) {
-      const T Fcoarse = Fc[oc + (size_t)q * fsz];
-      const T* f = Ff + of + (size_t)q * fsz;
-      T sum = T(0);
-      sum += f[0];
-      sum += f[sa];
-      sum += f[sb];
-      sum += f[sa + sb];
-      const T Ffine = T(0.25) * T(0.5) * sum;
-      Uc[(size_t)q * fs_c + cell] += sf * dtdx * (Fcoarse - Ffine);
+__global__ void __launch_bounds__(256) reflux_find_kernel(RefluxGeom G, const int4* __restrict__ cblk,
+                                                          const int* __restrict__ fmap, int2* __restrict__ list,
+                                                          int* __restrict__ count, int capacity) {
+  const int n = G.n, n2 = n * n, n3 = n2 * n;
+  const int r = blockIdx.x * blockDim.x + threadIdx.x;   // grid.y = entry of cblk
+  if (r >= n3) return;
+  const int l[3] = {r % n, (r / n) % n, r / n2};
+  // a covered neighbour lies across the boundary of an aligned (n/2)^3 block: only cells on such a boundary go on
+  const int h = n >> 1;
+  unsigned cand = 0;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    if ((l[d] + 1) % h == 0) cand |= 1u << (2 * d);
+    if (l[d] % h == 0) cand |= 2u << (2 * d);
+  }
+  if (!cand) return;
+  const int4 cb = cblk[blockIdx.y];
+  const int C[3] = {cb.y + l[0], cb.z + l[1], cb.w + l[2]};
+  if (fine_patch_of(G, fmap, C) >= 0) return;
+  unsigned mask = 0;
+#pragma unroll
+  for (int d = 0; d < 3; ++d)
+#pragma unroll
+    for (int side = 0; side < 2; ++side) {
+      const unsigned bit = 1u << (2 * d + side);
+      int Cn[3];
+      if ((cand & bit) && reflux_neighbour(G, C, d, side, Cn) && fine_patch_of(G, fmap, Cn) >= 0) mask |= bit;
+    }
+  if (!mask) return;
+  const int at = atomicAdd(count, 1);
+  if (at < capacity) list[at] = make_int2(cb.x * n3 + r, (int)((blockIdx.y << 6) | mask));
+}
+
+template <class T, bool ZERO>
+__global__ void __launch_bounds__(128) reflux_list_kernel(T* __restrict__ Uc, size_t fs_c, RefluxGeom G,
+                                                          const int4* __restrict__ cblk, const int2* __restrict__ list,
+                                                          int nlist, const int* __restrict__ fmap,
+                                                          const int* __restrict__ forigin, T* __restrict__ Fc,
+                                                          const T* __restrict__ Ff, T dtdx) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= nlist) return;
+  const int n = G.n, n2 = n * n, n3 = n2 * n;
+  const int2 ent = list[e];
+  const int b = ent.y >> 6;
+  const unsigned mask = (unsigned)ent.y & 63u;
+  const int4 cb = cblk[b];
+  const int blk = G.shared ? cb.x : b;
+  const int r = ent.x - cb.x * n3;
+  const int l[3] = {r % n, (r / n) % n, r / n2};
+  const int C[3] = {cb.y + l[0], cb.z + l[1], cb.w + l[2]};
+  const size_t fsz = (size_t)3 * n2;
+  const size_t cell = (size_t)ent.x;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+#pragma unroll
+    for (int side = 0; side < 2; ++side) {
+      if (!(mask & (1u << (2 * d + side)))) continue;
+      // the face in this cell's patch: its upper face (index l[d] + 1) when the fine patch is above
+      int lc[3] = {l[0], l[1], l[2]};
+      if (!side) lc[d] += 1;
+      const int sc = lc[d] == 0 ? 0 : (lc[d] == n ? 2 : 1);     // 1 <=> n/2: fine patches sit on aligned (n/2)^3 blocks
+      const int ic = d == 0 ? lc[2] * n + lc[1] : (d == 1 ? lc[2] * n + lc[0] : lc[1] * n + lc[0]);
+      const size_t oc = ((size_t)blk * 3 + d) * G.nf * fsz + (size_t)sc * n2 + ic;
+      if (ZERO) {
+        for (int q = 0; q < G.nf; ++q) Fc[oc + (size_t)q * fsz] = T(0);
+        continue;
+      }
+      int Cn[3];
+      reflux_neighbour(G, C, d, side, Cn);
+      const int pf = fine_patch_of(G, fmap, Cn);
+      // the four fine faces: the fine patch's low (side 0) or high (side 1) face plane, children of Cn in-plane
+      int lf[3];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) lf[a] = 2 * Cn[a] - forigin[3 * pf + a];
+      lf[d] = side ? n : 0;
+      const int iff = d == 0 ? lf[2] * n + lf[1] : (d == 1 ? lf[2] * n + lf[0] : lf[1] * n + lf[0]);
+      const size_t of = ((size_t)pf * 3 + d) * G.nf * fsz + (size_t)(side ? 2 : 0) * n2 + iff;
+      // in-plane strides of the transverse directions t1 = (d+1)%3, t2 = (d+2)%3: d = 0: (z, y), 1: (z, x), 2: (y, x)
+      const size_t sa = (d == 1) ? (size_t)n : 1, sb = (d == 1) ? 1 : (size_t)n;
+      const T sf = side ? T(-1) : T(1);
+      for (int q = 0; q < G.nf; ++q) {
+        const T Fcoarse = Fc[oc + (size_t)q * fsz];
+        const T* f = Ff + of + (size_t)q * fsz;
+        T sum = T(0);
+        sum += f[0];
+        sum += f[sa];
+        sum += f[sb];
+        sum += f[sa + sb];
+        const T Ffine = T(0.25) * T(0.5) * sum;
+        Uc[(size_t)q * fs_c + cell] += sf * dtdx * (Fcoarse - Ffine);
+      }
     }
   }
 }
@@ -458,38 +541,75 @@ cudaError_t launch_prolong_halo(int dtype, void* halo, size_t fs_halo, int nf, i
   return cudaGetLastError();
 }
 
-cudaError_t launch_restrict(int dtype, const void* Uf, size_t fs_f, int nf, int n, const long long* dst, int nent,
-                            void* Uc, size_t fs_c, cudaStream_t s) {
+static ProlongGeom coarse_geom(int n, const int* domc, const int* cdims, const int* bc) {
+  ProlongGeom G;
+  G.n = n; G.g = 0; G.npf = 0;
+  for (int a = 0; a < 3; ++a) {
+    G.domf[a] = 2 * domc[a]; G.domc[a] = domc[a]; G.cdims[a] = cdims[a];
+    G.per_lo[a] = bc[2 * a] == 0; G.per_hi[a] = bc[2 * a + 1] == 0;   // AMR_BC_PERIODIC == 0
+  }
+  return G;
+}
+
+cudaError_t launch_restrict(int dtype, const void* Uf, size_t fs_f, int nf, int n, int npf, const int* domc, const int* cdims,
+                            const int* bc, const int* forigin, const int* cmap, void* Uc, size_t fs_c, cudaStream_t s) {
+  const int h = n / 2, nent = npf * h * h * h;
   if (nent == 0) return cudaSuccess;
+  const ProlongGeom G = coarse_geom(n, domc, cdims, bc);
   const unsigned grid = (unsigned)((nent + 255) / 256);
   if (dtype == 0)
-    restrict_kernel<float><<<grid, 256, 0, s>>>((const float*)Uf, fs_f, nf, n, dst, nent, (float*)Uc, fs_c);
+    restrict_kernel<float><<<grid, 256, 0, s>>>((const float*)Uf, fs_f, nf, G, forigin, cmap, nent, (float*)Uc, fs_c);
   else
-    restrict_kernel<double><<<grid, 256, 0, s>>>((const double*)Uf, fs_f, nf, n, dst, nent, (double*)Uc, fs_c);
+    restrict_kernel<double><<<grid, 256, 0, s>>>((const double*)Uf, fs_f, nf, G, forigin, cmap, nent, (double*)Uc, fs_c);
   return cudaGetLastError();
 }
 
-cudaError_t launch_reflux(int dtype, void* Uc, size_t fs_c, int nf, int n, const long long* faces, int nfaces,
-                          const void* Fc, const void* Ff, double dtdx, cudaStream_t s) {
-  if (nfaces == 0) return cudaSuccess;
-  const unsigned grid = (unsigned)((nfaces + 255) / 256);
-  if (dtype == 0)
-    reflux_kernel<float><<<grid, 256, 0, s>>>((float*)Uc, fs_c, nf, n, faces, nfaces, (const float*)Fc,
-                                             (const float*)Ff, (float)dtdx);
-  else
-    reflux_kernel<double><<<grid, 256, 0, s>>>((double*)Uc, fs_c, nf, n, faces, nfaces, (const double*)Fc,
-                                              (const double*)Ff, dtdx);
+static RefluxGeom reflux_geom(int nf, int n, int shared, const int* domc, const int* fdims, const int* bc) {
+  RefluxGeom G;
+  G.n = n; G.nf = nf; G.shared = shared;
+  for (int a = 0; a < 3; ++a) {
+    G.domc[a] = domc[a]; G.fdims[a] = fdims[a];
+    G.per_lo[a] = bc[2 * a] == 0; G.per_hi[a] = bc[2 * a + 1] == 0;
+  }
+  return G;
+}
+
+cudaError_t launch_reflux_find(int nf, int n, int shared, const int* domc, const int* fdims, const int* bc, const void* cblk,
+                               int ncblk, const int* fmap, void* list, int* count, int capacity, cudaStream_t s) {
+  cudaError_t e = cudaMemsetAsync(count, 0, sizeof(int), s);
+  if (e != cudaSuccess || ncblk == 0) return e;
+  const RefluxGeom G = reflux_geom(nf, n, shared, domc, fdims, bc);
+  const dim3 grid((unsigned)((n * n * n + 255) / 256), (unsigned)ncblk);
+  reflux_find_kernel<<<grid, 256, 0, s>>>(G, (const int4*)cblk, fmap, (int2*)list, count, capacity);
   return cudaGetLastError();
 }
 
-cudaError_t launch_zero_faces(int dtype, void* Fc, int nf, int n, const long long* faces, int nfaces, cudaStream_t s) {
-  if (nfaces == 0) return cudaSuccess;
-  const unsigned grid = (unsigned)((nfaces + 255) / 256);
-  const size_t fsz = (size_t)3 * n * n;
+cudaError_t launch_reflux(int dtype, void* Uc, size_t fs_c, int nf, int n, int shared, const int* domc, const int* fdims,
+                          const int* bc, const void* cblk, const void* list, int nlist, const int* fmap, const int* forigin,
+                          void* Fc, const void* Ff, double dtdx, cudaStream_t s) {
+  if (nlist == 0) return cudaSuccess;
+  const RefluxGeom G = reflux_geom(nf, n, shared, domc, fdims, bc);
+  const unsigned grid = (unsigned)((nlist + 127) / 128);
   if (dtype == 0)
-    zero_faces_kernel<float><<<grid, 256, 0, s>>>((float*)Fc, nf, fsz, faces, nfaces);
+    reflux_list_kernel<float, false><<<grid, 128, 0, s>>>((float*)Uc, fs_c, G, (const int4*)cblk, (const int2*)list, nlist, fmap,
+                                                          forigin, (float*)Fc, (const float*)Ff, (float)dtdx);
   else
-    zero_faces_kernel<double><<<grid, 256, 0, s>>>((double*)Fc, nf, fsz, faces, nfaces);
+    reflux_list_kernel<double, false><<<grid, 128, 0, s>>>((double*)Uc, fs_c, G, (const int4*)cblk, (const int2*)list, nlist, fmap,
+                                                           forigin, (double*)Fc, (const double*)Ff, dtdx);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_zero_faces(int dtype, void* Fc, int nf, int n, int shared, const int* domc, const int* fdims, const int* bc,
+                              const void* cblk, const void* list, int nlist, cudaStream_t s) {
+  if (nlist == 0) return cudaSuccess;
+  const RefluxGeom G = reflux_geom(nf, n, shared, domc, fdims, bc);
+  const unsigned grid = (unsigned)((nlist + 127) / 128);
+  if (dtype == 0)
+    reflux_list_kernel<float, true><<<grid, 128, 0, s>>>(nullptr, 0, G, (const int4*)cblk, (const int2*)list, nlist, nullptr,
+                                                         nullptr, (float*)Fc, nullptr, 0.f);
+  else
+    reflux_list_kernel<double, true><<<grid, 128, 0, s>>>(nullptr, 0, G, (const int4*)cblk, (const int2*)list, nlist, nullptr,
+                                                          nullptr, (double*)Fc, nullptr, 0.0);
   return cudaGetLastError();
 }
 

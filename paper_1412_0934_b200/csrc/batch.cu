@@ -144,11 +144,12 @@ struct amr_level_link {
   amr_patch_batch *c, *f;
   char* ws;
   size_t bytes;
-  int *forg, *cmap;   // device: fine patch origins [npf][3], coarse patch map [z][y][x] (the prolongation resolves parents itself)
-  long long* res_dst;
-  int nres;
-  long long* faces;  // all (direction, side) tables merged, sorted by coarse cell (stable in d*2+side)
-  int nfaces;
+  // device tables: fine patch origins [npf][3], coarse and fine patch maps [z][y][x] (prolongation, restriction and
+  // reflux resolve cells through them in the kernels), and per coarse flux block (patch, origin x, y, z)
+  int *forg, *cmap, *fmap, *cblk;
+  int ncblk;
+  int* rlist;   // device, built at link time: (cell, block << 6 | mask) per uncovered coarse cell next to a fine face
+  int nrlist;
   void *fblk_c, *fblk_f;
   size_t fblk_c_bytes, fblk_f_bytes;
   int nblk_c;
@@ -158,40 +159,38 @@ struct amr_level_link {
 namespace {
 
 struct LinkHost {
-  std::vector<long long> res_dst, faces[6], faces_all;
-  std::vector<int> fblk_of_c;
+  std::vector<int> fblk_of_c;   // per coarse patch: its flux block or -1
+  std::vector<int> cblk;        // per flux block of this link: (coarse patch, origin x, y, z)
   int nblk_c = 0;
+  long long ncf_faces = 0;  // coarse-fine faces of fine patches: (n/2)^2 coarse cells each bound the reflux list
   bool identity_c = false;  // coarse blocks are per patch (block index = patch index)
 };
 
 struct LinkLayout {
-  size_t forg, cmap, res_dst, faces, fblk_c, fblk_f, total, fblk_c_bytes, fblk_f_bytes;
+  size_t forg, cmap, fmap, cblk, rlist, rcount, fblk_c, fblk_f, total, fblk_c_bytes, fblk_f_bytes;
+  int rcap;
 };
 
 int wrapi(int v, int m) { return ((v % m) + m) % m; }
 
-// Host tables for O8 / O9 (restated from DESIGN.md §3; index conventions of include/amr_godunov.h).
+// Host side of a link (index conventions of include/amr_godunov.h).  O8, O9(6) and O9(7)
+// resolve their cells in the kernels through the patch maps; what the host owes is (i) the check of proper nesting
+// and (ii) the list of coarse patches that touch a coarse-fine face and therefore record fluxes.
 int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) {
-  const int n = f->d.n, g = f->d.nghost, M = n + 2 * g, nc = n / 2;
-  const size_t n3 = (size_t)n * n * n, M3 = (size_t)M * M * M;
+  const int n = f->d.n, g = f->d.nghost, nc = n / 2;
   const int* domf = f->d.domain_cells;
   const int* domc = c->d.domain_cells;
-  auto coarse_flat = [&](int Cx, int Cy, int Cz, long long* out) -> bool {
+  auto coarse_patch = [&](int Cx, int Cy, int Cz) -> int {   // wrapped / clamped by the level's boundary conditions
     int C[3] = {Cx, Cy, Cz};
     for (int a = 0; a < 3; ++a) {
       if (C[a] < 0) C[a] = (c->d.bc[2 * a] == AMR_BC_PERIODIC) ? C[a] + domc[a] : 0;
       else if (C[a] >= domc[a]) C[a] = (c->d.bc[2 * a + 1] == AMR_BC_PERIODIC) ? C[a] - domc[a] : domc[a] - 1;
     }
-    const int pc = c->map.at(C[0] / n, C[1] / n, C[2] / n);
-    if (pc < 0) return false;
-    const int* oc = &c->origin[3 * pc];
-    *out = (long long)pc * (long long)n3 + ((long long)(C[2] - oc[2]) * n + (C[1] - oc[1])) * n + (C[0] - oc[0]);
-    return true;
+    return c->map.at(C[0] / n, C[1] / n, C[2] / n);
   };
-  // O8 needs no table: prolong_halo_kernel resolves the parents itself.  What the host still owes is the check of
-  // proper nesting: every halo region of a fine patch that no sibling covers (and its +-1 stencil) must lie inside
-  // coarse patches.  Checked per region at coarse-PATCH granularity: the region's parent cells, grown by one, span at
-  // most two coarse patches per axis.
+  // O8: every halo region of a fine patch that no sibling covers (and its +-1 stencil) must lie inside coarse
+  // patches.  Checked per region at coarse-PATCH granularity: the region's parent cells, grown by one, span at most
+  // two coarse patches per axis.
   if (g > 4) return fail(AMR_EINVAL, "nghost > 4 is not supported by the prolongation kernel");
   for (int p = 0; p < f->d.npatch; ++p) {
     const int* o = &f->origin[3 * p];
@@ -210,87 +209,40 @@ int build_link(const amr_patch_batch* c, const amr_patch_batch* f, LinkHost& H) 
       }
       for (int cz = plo[2]; cz <= phi[2]; cz += (cz == phi[2] ? 1 : std::min(n, phi[2] - cz)))
         for (int cy = plo[1]; cy <= phi[1]; cy += (cy == phi[1] ? 1 : std::min(n, phi[1] - cy)))
-          for (int cx = plo[0]; cx <= phi[0]; cx += (cx == phi[0] ? 1 : std::min(n, phi[0] - cx))) {
-            long long dummy;
-            if (!coarse_flat(cx, cy, cz, &dummy)) return fail(AMR_EINVAL, "fine patch %d has a halo cell with no coarse parent", p);
-          }
+          for (int cx = plo[0]; cx <= phi[0]; cx += (cx == phi[0] ? 1 : std::min(n, phi[0] - cx)))
+            if (coarse_patch(cx, cy, cz) < 0) return fail(AMR_EINVAL, "fine patch %d has a halo cell with no coarse parent", p);
     }
   }
-  // O9(6) list: entry e = (p, ck, cj, ci)
+  // O9(6): the parent block of a fine patch ((n/2)^3 coarse cells, aligned) lies in one coarse patch
   for (int p = 0; p < f->d.npatch; ++p) {
     const int* o = &f->origin[3 * p];
-    for (int ck = 0; ck < nc; ++ck)
-      for (int cj = 0; cj < nc; ++cj)
-        for (int ci = 0; ci < nc; ++ci) {
-          long long flat;
-          if (!coarse_flat(o[0] / 2 + ci, o[1] / 2 + cj, o[2] / 2 + ck, &flat))
-            return fail(AMR_EINVAL, "fine patch %d is not covered by a coarse patch", p);
-          H.res_dst.push_back(flat);
-        }
+    if (o[0] % nc || o[1] % nc || o[2] % nc) return fail(AMR_EINVAL, "fine patch %d is not aligned to an (n/2)^3 block of its parent level", p);
+    if (c->map.at(o[0] / 2 / n, o[1] / 2 / n, o[2] / 2 / n) < 0) return fail(AMR_EINVAL, "fine patch %d is not covered by a coarse patch", p);
   }
-  // O9(7) list, one per (d, side) so that no coarse cell appears twice in a launch
+  // O9(7): the coarse cells outside one face of a fine patch form one aligned (n/2)^2 x 1 slab of ONE coarse block:
+  // either that block is refined too (fine-fine face, nothing to do) or its coarse patch records fluxes.  A fine face
+  // on a non-periodic domain face has no coarse cell outside it: its flux is a boundary flux of the composite grid.
   H.fblk_of_c.assign(c->d.npatch, -1);
-  // flux blocks: [block][direction][field][3 face planes: index 0, n/2, n along the normal][n^2 in-plane, the
-  // lower remaining axis fastest] - all a link can read (fine patches sit on aligned (n/2)^3 parent blocks)
-  const long long fsz = 3LL * n * n;
-  const int NF = f->d.nfields;
-  auto slab_off = [&](int d, const int l[3]) -> long long {  // l = (x,y,z) with the face index along d
-    const long long s = l[d] == 0 ? 0 : (l[d] == n ? 2 : (l[d] == n / 2 ? 1 : -1));
-    if (s < 0) return -1;
-    const long long idx = d == 0 ? (long long)l[2] * n + l[1] : (d == 1 ? (long long)l[2] * n + l[0] : (long long)l[1] * n + l[0]);
-    return s * n * n + idx;
-  };
   for (int p = 0; p < f->d.npatch; ++p) {
     const int* o = &f->origin[3 * p];
     for (int d = 0; d < 3; ++d)
       for (int side = 0; side < 2; ++side) {
-        const int t1 = (d + 1) % 3, t2 = (d + 2) % 3;
-        for (int b = 0; b < nc; ++b)
-          for (int a = 0; a < nc; ++a) {
-            int Cin[3];
-            Cin[d] = o[d] / 2 + (side ? nc : -1);
-            Cin[t1] = o[t1] / 2 + a;
-            Cin[t2] = o[t2] / 2 + b;
-            // a fine face on a non-periodic domain face has no coarse cell outside it: its flux is a boundary
-            // flux of the composite grid, nothing to correct
-            if ((Cin[d] < 0 && c->d.bc[2 * d] != AMR_BC_PERIODIC) || (Cin[d] >= domc[d] && c->d.bc[2 * d + 1] != AMR_BC_PERIODIC)) continue;
-            int C[3];
-            for (int e = 0; e < 3; ++e) C[e] = wrapi(Cin[e], domc[e]);
-            if (f->map.at(2 * C[0] / n, 2 * C[1] / n, 2 * C[2] / n) >= 0) continue;  // fine-fine face
-            const int pc = c->map.at(C[0] / n, C[1] / n, C[2] / n);
-            if (pc < 0) return fail(AMR_EINVAL, "no coarse patch next to fine patch %d", p);
-            const int* oc = &c->origin[3 * pc];
-            int lc[3] = {C[0] - oc[0], C[1] - oc[1], C[2] - oc[2]};
-            const long long cell = (long long)pc * (long long)n3 + ((long long)lc[2] * n + lc[1]) * n + lc[0];
-            if (H.fblk_of_c[pc] < 0) H.fblk_of_c[pc] = H.identity_c ? pc : H.nblk_c++;
-            int lface[3] = {lc[0], lc[1], lc[2]};
-            if (!side) lface[d] += 1;  // upper face of the outside cell
-            if (slab_off(d, lface) < 0) return fail(AMR_EINVAL, "fine patch %d is not aligned to an (n/2)^3 block of its parent level", p);
-            const long long oc_off = ((long long)H.fblk_of_c[pc] * 3 + d) * NF * fsz + slab_off(d, lface);
-            int lf[3];
-            lf[d] = side ? n : 0;
-            lf[t1] = 2 * a;
-            lf[t2] = 2 * b;
-            const long long of_off = ((long long)p * 3 + d) * NF * fsz + slab_off(d, lf);
-            auto& v = H.faces[d * 2 + side];
-            v.push_back(cell);
-            v.push_back(oc_off);
-            v.push_back(of_off);
-            v.push_back((long long)(side ? 1 : 0) | ((long long)d << 1));
-          }
+        int Cin[3] = {o[0] / 2, o[1] / 2, o[2] / 2};
+        Cin[d] += side ? nc : -1;
+        if ((Cin[d] < 0 && c->d.bc[2 * d] != AMR_BC_PERIODIC) || (Cin[d] >= domc[d] && c->d.bc[2 * d + 1] != AMR_BC_PERIODIC)) continue;
+        int C[3];
+        for (int e = 0; e < 3; ++e) C[e] = wrapi(Cin[e], domc[e]);
+        if (f->map.at(2 * C[0] / n, 2 * C[1] / n, 2 * C[2] / n) >= 0) continue;  // fine-fine face
+        const int pc = c->map.at(C[0] / n, C[1] / n, C[2] / n);
+        if (pc < 0) return fail(AMR_EINVAL, "no coarse patch next to fine patch %d", p);
+        H.ncf_faces++;
+        if (H.fblk_of_c[pc] < 0) {
+          H.fblk_of_c[pc] = H.identity_c ? pc : H.nblk_c++;
+          const int* oc = &c->origin[3 * pc];
+          H.cblk.push_back(pc); H.cblk.push_back(oc[0]); H.cblk.push_back(oc[1]); H.cblk.push_back(oc[2]);
+        }
       }
   }
-  // one table for one launch: entries sorted by coarse cell, (direction, side) order kept inside a cell, so a
-  // cell that touches fine patches on several sides gets its corrections in a fixed order from one thread
-  struct Ent { long long v[4]; int s; };
-  std::vector<Ent> all;
-  for (int sd = 0; sd < 6; ++sd)
-    for (size_t e = 0; e + 3 < H.faces[sd].size(); e += 4)
-      all.push_back(Ent{{H.faces[sd][e], H.faces[sd][e + 1], H.faces[sd][e + 2], H.faces[sd][e + 3]}, sd});
-  std::stable_sort(all.begin(), all.end(), [](const Ent& a, const Ent& b) { return a.v[0] < b.v[0]; });
-  H.faces_all.reserve(all.size() * 4);
-  for (const Ent& en : all)
-    for (int q = 0; q < 4; ++q) H.faces_all.push_back(en.v[q]);
   return AMR_OK;
 }
 
@@ -308,15 +260,18 @@ LinkLayout make_link_layout(const amr_patch_batch* c, const amr_patch_batch* f, 
   size_t off = 0;
   L.forg = off; off += up((size_t)f->d.npatch * 3 * sizeof(int) + 8);
   L.cmap = off; off += up(c->map.idx.size() * sizeof(int) + 8);
-  L.res_dst = off; off += up(H.res_dst.size() * 8 + 8);
-  L.faces = off; off += up(H.faces_all.size() * 8 + 8);
+  L.fmap = off; off += up(f->map.idx.size() * sizeof(int) + 8);
+  L.cblk = off; off += up(H.cblk.size() * sizeof(int) + 16);
+  // a coarse cell enters the reflux list once, however many of its faces are coarse-fine: the face count bounds it
+  L.rcap = (int)std::min<long long>(H.ncf_faces * (long long)(f->d.n / 2) * (f->d.n / 2), 0x7fffffffLL);
+  L.rlist = off; off += up((size_t)L.rcap * 2 * sizeof(int) + 16);
+  L.rcount = off; off += up(sizeof(int));
   const size_t n = f->d.n, blk = 3 * (size_t)f->d.nfields * 3 * n * n * f->esz;
   L.fblk_c_bytes = H.identity_c ? 0 : (size_t)H.nblk_c * blk;
   L.fblk_f_bytes = (size_t)f->d.npatch * blk;
   L.fblk_c = off; off += up(L.fblk_c_bytes + 8);
   L.fblk_f = off; off += up(L.fblk_f_bytes + 8);
   L.total = off;
-  (void)c;
   return L;
 }
 
@@ -838,10 +793,11 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   l->c = coarse; l->f = fine; l->ws = (char*)dev_ws; l->bytes = bytes;
   l->forg = (int*)(l->ws + L.forg);
   l->cmap = (int*)(l->ws + L.cmap);
-  l->res_dst = (long long*)(l->ws + L.res_dst);
-  l->nres = (int)H.res_dst.size();
-  l->faces = (long long*)(l->ws + L.faces);
-  l->nfaces = (int)(H.faces_all.size() / 4);
+  l->fmap = (int*)(l->ws + L.fmap);
+  l->cblk = (int*)(l->ws + L.cblk);
+  l->ncblk = (int)(H.cblk.size() / 4);
+  l->rlist = (int*)(l->ws + L.rlist);
+  l->nrlist = 0;
   l->fblk_c = l->ws + L.fblk_c; l->fblk_f = l->ws + L.fblk_f;
   l->fblk_c_bytes = L.fblk_c_bytes; l->fblk_f_bytes = L.fblk_f_bytes;
   l->nblk_c = H.nblk_c;
@@ -853,16 +809,24 @@ int amr_link_levels(amr_patch_batch* coarse, amr_patch_batch* fine, int ratio, v
   };
   cudaError_t e = h2d(l->forg, fine->origin.data(), fine->origin.size() * sizeof(int));
   if (e == cudaSuccess) e = h2d(l->cmap, coarse->map.idx.data(), coarse->map.idx.size() * sizeof(int));
-  if (e == cudaSuccess) e = h2d(l->res_dst, H.res_dst.data(), H.res_dst.size() * 8);
-  if (e == cudaSuccess) e = h2d(l->faces, H.faces_all.data(), H.faces_all.size() * 8);
+  if (e == cudaSuccess) e = h2d(l->fmap, fine->map.idx.data(), fine->map.idx.size() * sizeof(int));
+  if (e == cudaSuccess) e = h2d(l->cblk, H.cblk.data(), H.cblk.size() * sizeof(int));
   if (e == cudaSuccess && !l->shared_c) e = h2d(coarse->fblk_of, H.fblk_of_c.data(), H.fblk_of_c.size() * sizeof(int));
   std::vector<int> idf(fine->d.npatch);
   for (int p = 0; p < fine->d.npatch; ++p) idf[p] = p;
   if (e == cudaSuccess) e = h2d(fine->fblk_of, idf.data(), idf.size() * sizeof(int));
   if (e == cudaSuccess && !l->shared_c) e = cudaMemsetAsync(l->fblk_c, 0, L.fblk_c_bytes + 8, s);
   if (e == cudaSuccess) e = cudaMemsetAsync(l->fblk_f, 0, L.fblk_f_bytes + 8, s);
+  // the reflux list: found on the device from the tables just uploaded (same stream)
+  int nr = 0;
+  if (e == cudaSuccess)
+    e = amr::launch_reflux_find(coarse->d.nfields, coarse->d.n, l->shared_c ? 1 : 0, coarse->d.domain_cells, fine->map.dims,
+                                coarse->d.bc, l->cblk, l->ncblk, l->fmap, l->rlist, (int*)(l->ws + L.rcount), L.rcap, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&nr, l->ws + L.rcount, sizeof(int), cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e != cudaSuccess) { delete l; return fail(AMR_ECUDA, "link upload: %s", cudaGetErrorString(e)); }
+  if (nr > L.rcap) { delete l; return fail(AMR_EINVAL, "reflux list overflow: %d cells > %d (inconsistent patch maps)", nr, L.rcap); }
+  l->nrlist = nr;
   if (!l->shared_c) coarse->fblk = l->nblk_c ? l->fblk_c : nullptr;
   fine->fblk = l->fblk_f;
   coarse->link_down = fine->link_up = l;
@@ -901,7 +865,8 @@ int amr_flux_clear(amr_level_link* l) {
   if (!l) return fail(AMR_EINVAL, "null link");
   DeviceGuard guard(l->f->device);
   if (l->shared_c) {
-    cudaError_t e = amr::launch_zero_faces(l->c->d.dtype, l->fblk_c, l->c->d.nfields, l->c->d.n, l->faces, l->nfaces, l->c->stream);
+    cudaError_t e = amr::launch_zero_faces(l->c->d.dtype, l->fblk_c, l->c->d.nfields, l->c->d.n, 1, l->c->d.domain_cells,
+                                           l->f->map.dims, l->c->d.bc, l->cblk, l->rlist, l->nrlist, l->c->stream);
     if (e != cudaSuccess) return fail(AMR_ECUDA, "flux clear kernel launch: %s", cudaGetErrorString(e));
   } else if (l->fblk_c_bytes) {
     CUDA_TRY(cudaMemsetAsync(l->fblk_c, 0, l->fblk_c_bytes, l->c->stream));
@@ -914,8 +879,9 @@ int amr_restrict(amr_level_link* l) {
   if (!l) return fail(AMR_EINVAL, "null link");
   DeviceGuard guard(l->f->device);
   amr_patch_batch *c = l->c, *f = l->f;
-  cudaError_t e = amr::launch_restrict(f->d.dtype, f->U[f->cur], (size_t)f->d.npatch * f->n3, f->d.nfields, f->d.n, l->res_dst,
-                                       l->nres, c->U[c->cur], (size_t)c->d.npatch * c->n3, c->stream);
+  cudaError_t e = amr::launch_restrict(f->d.dtype, f->U[f->cur], (size_t)f->d.npatch * f->n3, f->d.nfields, f->d.n, f->d.npatch,
+                                       c->d.domain_cells, c->map.dims, c->d.bc, l->forg, l->cmap, c->U[c->cur],
+                                       (size_t)c->d.npatch * c->n3, c->stream);
   if (e != cudaSuccess) return fail(AMR_ECUDA, "restrict kernel launch: %s", cudaGetErrorString(e));
   c->smax_valid = false;
   return AMR_OK;
@@ -926,8 +892,9 @@ int amr_reflux(amr_level_link* l, double dt_coarse) {
   DeviceGuard guard(l->f->device);
   if (!(dt_coarse > 0) || !std::isfinite(dt_coarse)) return fail(AMR_EINVAL, "dt_coarse must be finite and > 0");
   amr_patch_batch* c = l->c;
-  cudaError_t e = amr::launch_reflux(c->d.dtype, c->U[c->cur], (size_t)c->d.npatch * c->n3, c->d.nfields, c->d.n, l->faces,
-                                     l->nfaces, l->fblk_c, l->fblk_f, dt_coarse / c->d.dx, c->stream);
+  cudaError_t e = amr::launch_reflux(c->d.dtype, c->U[c->cur], (size_t)c->d.npatch * c->n3, c->d.nfields, c->d.n, l->shared_c ? 1 : 0,
+                                     c->d.domain_cells, l->f->map.dims, c->d.bc, l->cblk, l->rlist, l->nrlist, l->fmap, l->forg,
+                                     l->fblk_c, l->fblk_f, dt_coarse / c->d.dx, c->stream);
   if (e != cudaSuccess) return fail(AMR_ECUDA, "reflux kernel launch: %s", cudaGetErrorString(e));
   c->smax_valid = false;
   return AMR_OK;
