@@ -524,7 +524,7 @@ def run_hierarchy(args):
         e2e = dict(value=updates / (ms2 * 1e-3), unit=UNIT, h2d_bytes_per_step=nbytes, d2h_bytes_per_step=nbytes,
                    ms_per_step=ms2, steps=3)
     # one regrid of the finest level between steps (amr_flag_blocks -> caller's selection -> new batch ->
-    # amr_regrid_fill -> relink), wall-clock per part; the host builds the link tables
+    # amr_regrid_fill -> relink), wall-clock per part
     def new_level2():
         torch.cuda.synchronize()
         t0 = time.perf_counter()
@@ -554,7 +554,7 @@ def run_hierarchy(args):
     torch.cuda.synchronize()
     regrid = dict(level=2, patches_before=int(np_before), patches_after=int(len(origin_new)), flag_ms=1e3 * (t1 - t0),
                   select_and_create_ms=1e3 * (t2 - t1), fill_ms=1e3 * (t3 - t2), relink_ms=1e3 * (r1 - r0),
-                  note="wall clock, one regrid after the timed steps (the same regrid run once before, untimed, as warm-up); selection and link tables are host work")
+                  note="wall clock, one regrid after the timed steps (the same regrid run once before, untimed, as warm-up); the block selection is host work (caller's policy), fill and link resolve cells on the device")
     pk = peaks()
     bpc = 2 * 9 * (4 if f32 else 8)
     ach = bpc * updates / (ms * 1e-3) / 1e9
