@@ -32,6 +32,7 @@ __global__ void __launch_bounds__(512) k(float* out, int niter, float a, float b
         if (MODE & 8) s[i] = __fmaf_rn(s[i], a, b);
         if (MODE & 16) w[i] = (w[i] > y[(i + 1) % NCH]) ? s[(i + 3) % NCH] : w[i];
         if (MODE & 32) { float t; asm("min.f32 %0, %1, %2, %3;" : "=f"(t) : "f"(y[i]), "f"(z[i]), "f"(w[i])); y[i] = t; }
+        if (MODE & 64) { s[i] = __fmaf_rn(s[i], x[i].x, x[(i + 1) % NCH].y); x[i].x = __fmaf_rn(x[i].x, s[(i + 3) % NCH], x[(i + 5) % NCH].y); }
       }
       if (MODE & 4) z[r % NCH] = rcpf(z[r % NCH]);
     }
@@ -79,5 +80,10 @@ int main() {
   run<2 | 4>("FMNMX x128 + MUFU x8", d, 136);
   run<1 | 2 | 4>("FFMA2 x64 + FMNMX x128 + MUFU x8", d, 200);
   run<1 | 16>("FFMA2 + FSETP/FSEL", d, 192);
+  // register-file operand bandwidth: 2 FFMA (3 distinct registers each) + FMNMX3 (3) = 9 operand reads per slot; the
+  // pipes alone would need 2 cycles (fma: 2 x 1, alu: 1 x 2)
+  run<64>("2 FFMA, distinct operands", d, 128);
+  run<64 | 32>("2 FFMA distinct + FMNMX3", d, 192);
+  run<64 | 2>("2 FFMA distinct + 2 FMNMX", d, 256);
   return 0;
 }
