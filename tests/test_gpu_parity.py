@@ -466,3 +466,106 @@ def test_api_rejects_bad_arguments(H):
         m.mhd_step(1e-3, 1.4, 1, 1, 1.0, 0.4)                                   # HLLC in the MHD step
     with pytest.raises(amr.AmrError):
         m.mhd_step(1e-3, 1.4, 1, 2, 0.0, 0.4)                                   # ch <= 0
+
+
+def _degenerate_level(case, n, np_dtype):
+    """32^3 periodic grid of 2^3 patches (or one self-neighbouring patch): white-noise gas (|v| ~ c_s) with the field
+    configurations at which HLLD's formulas degenerate (A7)."""
+    rng = np.random.default_rng([wk.SEED, 98, ["zero", "along_z", "strong", "tiny", "static", "one_patch"].index(case)])
+    N = n if case == "one_patch" else 32
+    rho = np.exp(0.4 * rng.standard_normal((N, N, N)))
+    v = 0.8 * rng.standard_normal((3, N, N, N))
+    p = np.exp(0.3 * rng.standard_normal((N, N, N)))
+    B = np.zeros((3, N, N, N))
+    if case == "along_z":          # B_n = 0 on every x and y face, B_t = 0 on every z face
+        B[2] = 0.5
+    elif case == "strong":         # beta ~ 0.01
+        B[:] = 10.0 * rng.standard_normal((3, N, N, N))
+    elif case == "tiny":           # B_n^2 far below eps p_T*: the rotational waves are skipped everywhere (A7)
+        B[:] = 1e-9 * rng.standard_normal((3, N, N, N))
+    elif case == "static":         # gas at rest in a uniform oblique field: an exact equilibrium
+        rho[:], p[:], v[:] = 1.0, 0.7, 0.0
+        B[0], B[1], B[2] = 0.3, -0.4, 0.5
+    elif case == "one_patch":
+        B[:] = 0.7 * rng.standard_normal((3, N, N, N))
+    G = wk.primitive_to_conserved(rho, v, p, 5.0 / 3.0, B=B)
+    wl = wk.uniform_grid_workload("degenerate_" + case, G, n, 5.0 / 3.0, True, wk.configs.LIM_MC, wk.configs.RS_HLLD, 0.3, 1)
+    wl.levels[0].U = wl.levels[0].U.astype(np_dtype).astype(np.float64)
+    return wl
+
+
+@pytest.mark.parametrize("np_dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("n", [16, 32])
+@pytest.mark.parametrize("case", ["zero", "along_z", "strong", "tiny", "static", "one_patch"])
+def test_degenerate_mhd_states(oracle, H, case, n, np_dtype):
+    """HLLD where its formulas degenerate: B = 0 (the solver must reduce to HLLC: same bits for rho, m, E as the
+    oracle's path through the same branch), B_n = 0 with B_t != 0 and the reverse, beta ~ 0.01, |B| ~ 1e-9, an exact
+    static equilibrium (preserved bitwise), and a single patch that is its own neighbour in all 26 directions.
+    One step against the oracle at the stated bounds; event counters as the oracle's (cells equal in fp64)."""
+    wl = _degenerate_level(case, n, np_dtype)
+    lev = wl.levels[0]
+    f32 = np.dtype(np_dtype) == np.float32
+    eps = oracle.default_eps(np_dtype)
+    ref = oracle.advance(lev, wl, 1, eps=eps)
+    got = H.gpu_advance(lev, wl, 1, np_dtype=np_dtype)
+    assert np.isfinite(got["U"]).all()
+    rel = abs(got["smaxs"][0] - ref["smaxs"][0]) / ref["smaxs"][0]
+    assert rel <= (1e-6 if f32 else 1e-14), rel
+    if case == "static":
+        assert np.array_equal(got["U"], lev.U.astype(np_dtype))
+        return
+    ps = _psi_scale(ref["U"], ref["smaxs"][0])
+    U = got["U"].astype(np.float64)
+    if case in ("zero", "tiny"):
+        # B (and psi) are zero or 1e-9: compare the gas, and B on its own scale
+        err = H.rel_err(U[:5], ref["U"][:5])
+        assert err.max() <= (TOL32 if f32 else TOL64_STEP), err
+        if case == "zero":
+            assert not U[5:].any() and not ref["U"][5:].any()
+        else:
+            db = np.abs(U[5:8] - ref["U"][5:8]).max() / np.abs(ref["U"][5:8]).max()
+            assert db <= (TOL32 if f32 else TOL64_STEP), db
+    else:
+        err = H.rel_err(U, ref["U"], psi_scale=ps)
+        assert err.max() <= (TOL32 if f32 else TOL64_STEP), err
+    if not f32:
+        # the GPU counts every cell once and a face on the boundary between two tiles twice (include/amr_godunov.h);
+        # the oracle counts, per patch, the cells whose face states it consumes: its interior and the face neighbours
+        # beyond it, so a fallback cell next to a patch boundary appears in two patches' counts
+        gc, rc = got["counters"], ref["counters"][0]
+        assert 0.7 * rc["positivity_fallback_cells"] - 2 <= gc["positivity_fallback_cells"] <= rc["positivity_fallback_cells"], (gc, rc)
+        assert gc["nonpositive_rho_after"] == rc["nonpositive_rho_after"] == 0
+        assert rc["hll_fallback_faces"] <= gc["hll_fallback_faces"] <= 1.25 * rc["hll_fallback_faces"] + 4, (gc, rc)
+        assert rc["degenerate_D"] <= gc["degenerate_D"] <= 1.25 * rc["degenerate_D"] + 4, (gc, rc)
+
+
+@pytest.mark.parametrize("np_dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("nf", [5, 9])
+def test_blast_wave_contrast(oracle, H, nf, np_dtype):
+    """A strong explosion into a thin medium: pressure contrast 1e6 and density contrast 1e3 across a spherical
+    interface that cuts through patch corners (32^3, 2^3 patches of 16^3, outflow faces), three steps from rest.
+    The positivity fallback (A10) and the solver's supersonic branches carry the step; every step from the previous
+    GPU state within the stated bounds, and no non-positive density afterwards."""
+    N, n = 32, 16
+    x = (np.arange(N) + 0.5) / N
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    r2 = (X - 0.47) ** 2 + (Y - 0.52) ** 2 + (Z - 0.5) ** 2
+    inside = r2 < 0.18 ** 2
+    rho = np.where(inside, 1.0, 1e-3)
+    p = np.where(inside, 1e3, 1e-3)
+    v = np.zeros((3, N, N, N))
+    B = None
+    if nf == 9:
+        B = np.zeros((3, N, N, N))
+        B[0], B[1] = 0.5, 0.5
+    G = wk.primitive_to_conserved(rho, v, p, 5.0 / 3.0, B=B)
+    wl = wk.uniform_grid_workload("blast", G, n, 5.0 / 3.0, nf == 9, wk.configs.LIM_MINMOD,
+                                  wk.configs.RS_HLLD if nf == 9 else wk.configs.RS_HLLC, 0.3, 3,
+                                  bc=(wk.configs.BC_OUTFLOW,) * 6)
+    lev = wl.levels[0]
+    lev.U = lev.U.astype(np_dtype).astype(np.float64)
+    f32 = np.dtype(np_dtype) == np.float32
+    errs, U, batch = H.per_step_parity(oracle, lev, wl, 3, np_dtype)
+    assert max(e.max() for e in errs) <= (TOL32 if f32 else TOL64_STEP), errs
+    assert (U[0] > 0).all() and np.isfinite(U).all()
+    assert batch.step_counters()["nonpositive_rho_after"] == 0
