@@ -143,6 +143,24 @@ int amr_hydro_step_ppm(amr_patch_batch* b, double dt, double gamma, int riemann,
 
 int amr_conserved_totals(amr_patch_batch* b, double* totals);
 
+/* The same reduction for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): no batch, no arena, no host copy, no synchronisation.
+ * dev_U: DEVICE, [nfields] arrays of dtype (AMR_F32 | AMR_F64), field f at dev_U + f*field_stride elements, the first
+ * ncells of each are summed (for a batch: amr_patch_batch_state(b, 0), ncells = field_stride = npatch*n^3).
+ * dev_totals: DEVICE, double [nfields], written by the kernel (valid once the stream has reached it).
+ * cuda_stream: the cudaStream_t to enqueue on (NULL = the default stream).  All pointers must belong to the CURRENT
+ * device; nothing is owned or kept.  Same partition and per-block summation order as amr_conserved_totals; the last
+ * sum over the 256 block results runs on the device as a double tree (there: long double on the host), so the two agree
+ * to a few ulp of sum|U|, not bitwise.
+ * Scratch: the block results live in ONE static device array of 33 024 bytes that every GPU loading the library holds
+ * until exit; it fits nfields <= AMR_NOALLOC_MAX_FIELDS, more is AMR_EINVAL.  The call allocates nothing (no
+ * cudaMalloc / cudaFree / allocating library routine; the first call on a device looks the array's address up).  All
+ * calls on a device share the array: calls ordered on one stream (or by events) are safe, calls that overlap on the GPU
+ * race on it and give wrong totals. */
+#define AMR_NOALLOC_MAX_FIELDS 16
+int amr_conserved_totals_noalloc(const void* dev_U, int dtype, int nfields, int64_t ncells, int64_t field_stride,
+                                 double* dev_totals, void* cuda_stream);
+
 /* Event counters accumulated since the last call with reset != 0.  counters: host [4] (AMR_CNT_*).
  * Face events are counted once per tile that computes the face. */
 int amr_step_counters(amr_patch_batch* b, long long* counters, int reset);

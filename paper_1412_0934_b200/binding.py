@@ -27,7 +27,7 @@ EXPORTS = (
     "amr_version", "amr_builder_bytes", "amr_builder_create", "amr_builder_destroy", "amr_builder_build",
     "amr_builder_results", "amr_builder_gather", "amr_hierarchy_cfl_dt", "amr_hierarchy_step",
     "amr_flag_blocks", "amr_regrid_bytes", "amr_regrid_fill", "amr_measure_fma_peak", "amr_hydro_sweep_ppm",
-    "amr_hydro_step_ppm", "amr_patch_batch_export", "amr_patch_batch_import",
+    "amr_hydro_step_ppm", "amr_patch_batch_export", "amr_patch_batch_import", "amr_conserved_totals_noalloc",
 )
 
 
@@ -74,6 +74,7 @@ def lib():
         L.amr_hydro_step.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int]
         L.amr_mhd_step.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double]
         L.amr_conserved_totals.argtypes = [C.c_void_p, C.c_void_p]
+        L.amr_conserved_totals_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
         L.amr_step_counters.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
         L.amr_link_bytes.restype = C.c_size_t
         L.amr_link_bytes.argtypes = [C.c_void_p, C.c_void_p, C.c_int]
@@ -122,6 +123,23 @@ def measure_fma_peak(dtype: int, ms_target: float = 2.0, device: str = "cuda:0")
         _check(lib().amr_measure_fma_peak(dtype, scratch.data_ptr(), int(torch.cuda.current_stream().cuda_stream),
                                           float(ms_target), C.byref(out)))
     return float(out.value)
+
+
+def conserved_totals_noalloc(dev_U, nfields: int, ncells: int, field_stride: int, dev_totals, dtype: int = None,
+                             stream: int = None):
+    """amr_conserved_totals_noalloc: dev_U / dev_totals are torch device tensors (or raw device addresses, then pass
+    dtype); only enqueues on `stream` (default: torch's current stream of the tensor's device)."""
+    import torch
+    if isinstance(dev_U, torch.Tensor):
+        if dtype is None:
+            dtype = AMR_F64 if dev_U.dtype == torch.float64 else AMR_F32
+        ctx, pu = torch.cuda.device(dev_U.device), dev_U.data_ptr()
+    else:
+        ctx, pu = torch.cuda.device(torch.cuda.current_device()), int(dev_U)
+    pt = dev_totals.data_ptr() if isinstance(dev_totals, torch.Tensor) else int(dev_totals)
+    with ctx:
+        st = int(torch.cuda.current_stream().cuda_stream) if stream is None else int(stream)
+        _check(lib().amr_conserved_totals_noalloc(pu, int(dtype), int(nfields), int(ncells), int(field_stride), pt, st))
 
 
 def _np_dtype(dtype: int):
