@@ -94,6 +94,21 @@ __device__ __forceinline__ void sts_n(float* p, const float* o) {
   if constexpr (N - R0 >= 2) *reinterpret_cast<float2*>(p + R0) = make_float2(o[R0], o[R0 + 1]);
   if constexpr ((N - R0) & 1) p[N - 1] = o[N - 1];
 }
+// A whole record through opaque vector loads.  When only one half of every pair is used (the x neighbours' records in
+// the slope stencil) the compiler turns a plain vector load into nine scalar loads, and scalar accesses at the record
+// stride of 20 words are 4-way bank conflicts (ncu: 8.9e6 wavefronts per instruction where 2.2e6 are ideal); five opaque
+// vector loads fetch the record in 20 wavefronts instead of 36.  Worth 0.7 % (config 5) to 1.1 % (config 3) of the MHD
+// step; the same for the right neighbour's flux record in phase 3 costs 3 % (more live registers there) and is not done.
+template <int N>
+__device__ __forceinline__ void lds_n_opaque(const float* p, float* o) {
+  static_assert(N == 18 || N == 10, "records of 9 or 5 pairs");
+  const unsigned a = (unsigned)__cvta_generic_to_shared(p);
+#pragma unroll
+  for (int i = 0; i < N / 4; ++i)
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                 : "=f"(o[4 * i]), "=f"(o[4 * i + 1]), "=f"(o[4 * i + 2]), "=f"(o[4 * i + 3]) : "r"(a + 16 * i));
+  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(o[N - 2]), "=f"(o[N - 1]) : "r"(a + 4 * (N - 2)));
+}
 // a pair record <-> F2[NF]
 template <int NF>
 __device__ __forceinline__ void lds_pairs(const float* p, F2* w) {
@@ -180,8 +195,8 @@ __device__ __forceinline__ int predict_pair(const float* Wm, const float* Wc, co
     const float* cc = Wc + rc;
     float c[2 * NF], a[2 * NF], b[2 * NF];
     lds_n<2 * NF, 4>(cc, c);
-    lds_n<2 * NF, 4>(cc - recstride, a);
-    lds_n<2 * NF, 4>(cc + recstride, b);
+    lds_n_opaque<2 * NF>(cc - recstride, a);   // only the odd halves are used
+    lds_n_opaque<2 * NF>(cc + recstride, b);   // only the even halves are used
 #pragma unroll
     for (int q = 0; q < NF; ++q) {
       w[q] = F2(c[2 * q], c[2 * q + 1]);
