@@ -17,7 +17,7 @@ Which flagged blocks become patches (growth, proper nesting) is geometry policy 
 
 Pins (tests/test_oracle_regrid.py): children average to the parent; kept patches are bitwise copies; a field
 linear in space is reproduced exactly; uniform stays uniform; flags against a hand-made field; composite totals
-unchanged by a regrid.
+unchanged by a regrid; at a non-periodic face the stencil sees the clamped cell, not the far side of the domain.
 """
 from __future__ import annotations
 
@@ -45,17 +45,28 @@ def minmod(a, b):
     return np.where((a > 0) & (b > 0), np.minimum(a, b), np.where((a < 0) & (b < 0), np.maximum(a, b), 0.0))
 
 
-def prolong_patch(Gc: np.ndarray, origin_f, n: int) -> np.ndarray:
-    """The n^3 fine cells of the patch at fine origin `origin_f` from the dense periodic coarse field Gc."""
+def prolong_patch(Gc: np.ndarray, origin_f, n: int, bc=(0,) * 6) -> np.ndarray:
+    """The n^3 fine cells of the patch at fine origin `origin_f` from the dense coarse field Gc.  bc = (xlo, xhi, ylo,
+    yhi, zlo, zhi) of the level pair, 0 = periodic: a +-1 stencil cell beyond a periodic face is the wrapped cell; beyond
+    any other face it is the coarse level's ghost cell there, i.e. the nearest in-domain cell (O0 rule (ii); DESIGN.md
+    section 3 "AMR at non-periodic domain faces": never data from the far side of the domain)."""
     nf = Gc.shape[0]
     Nz, Ny, Nx = Gc.shape[1:]
     h = n // 2
-    cx = (origin_f[0] // 2 + np.arange(h)) % Nx
-    cy = (origin_f[1] // 2 + np.arange(h)) % Ny
-    cz = (origin_f[2] // 2 + np.arange(h)) % Nz
+    cx = origin_f[0] // 2 + np.arange(h)
+    cy = origin_f[1] // 2 + np.arange(h)
+    cz = origin_f[2] // 2 + np.arange(h)
+
+    def idx(c, N, lo, hi):
+        c = np.asarray(c).copy()
+        below, above = c < 0, c >= N
+        c[below] = c[below] + N if lo == 0 else 0
+        c[above] = c[above] - N if hi == 0 else N - 1
+        return c
 
     def at(dz, dy, dx):
-        return Gc[:, ((cz + dz) % Nz)[:, None, None], ((cy + dy) % Ny)[None, :, None], ((cx + dx) % Nx)[None, None, :]]
+        return Gc[:, idx(cz + dz, Nz, bc[4], bc[5])[:, None, None], idx(cy + dy, Ny, bc[2], bc[3])[None, :, None],
+                  idx(cx + dx, Nx, bc[0], bc[1])[None, None, :]]
 
     U = at(0, 0, 0)
     sx = minmod(U - at(0, 0, -1), at(0, 0, 1) - U)
@@ -82,6 +93,6 @@ def regrid_fill(coarse, fine_old, origin_new: np.ndarray) -> np.ndarray:
         if key in old:
             out[:, p] = fine_old.U[:, old[key]]
         else:
-            out[:, p] = prolong_patch(Gc, key, n)
+            out[:, p] = prolong_patch(Gc, key, n, tuple(coarse.bc))
             assert np.isfinite(out[:, p]).all(), "new patch %d reaches outside the coarse level (not properly nested)" % p
     return out

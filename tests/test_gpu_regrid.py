@@ -104,3 +104,40 @@ def test_regrid_rejects_a_patch_outside_the_coarse_level(H):
     b2 = amr.PatchBatch.from_level(lev, amr.AMR_F64)
     with pytest.raises(amr.AmrError):
         b2.regrid_fill(None, b1)
+
+
+@pytest.mark.parametrize("np_dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("n", [8, 16])
+def test_regrid_fill_with_new_born_patches_on_outflow_faces(H, n, np_dtype):
+    """amr_regrid_fill where the new patches touch non-periodic domain faces (outflow x and z, periodic y), on the
+    faces, edges and a corner of the domain, beside interior ones: the O8 stencil clamps at the outflow faces and wraps
+    across the periodic one, against oracle/regrid.py."""
+    import paper_1412_0934_b200 as amr
+    from oracle import regrid as rg
+    rng = np.random.default_rng([wk.SEED, 97, n])
+    N = 4 * n
+    G = np.exp(0.5 * rng.standard_normal((5, N, N, N)))
+    bc = (1, 1, 0, 0, 1, 1)
+    origin0 = wk.morton_patch_origins(4, 4, 4, n)
+    l0 = wk.Level(n=n, g=3, level=0, dx=1.0 / N, origin=origin0, domain_cells=(N, N, N), bc=bc, self_periodic=False,
+                  U=wk.split_into_patches(G, n, origin0).astype(np_dtype).astype(np.float64))
+    F = 2 * N - n                                                   # fine origin of the last patch along an axis
+    origin_new = np.array([[0, 0, 0], [F, 0, 0], [0, F, F], [F, F, F], [0, 3 * n, 2 * n], [3 * n, 0, F], [2 * n, F, 0],
+                           [3 * n, 3 * n, 3 * n], [4 * n, 3 * n, 3 * n]], np.int32)
+    ref = rg.regrid_fill(l0, None, origin_new)
+    dt_ = H.gpu_dtype(np_dtype)
+    b0 = amr.PatchBatch.from_level(l0, dt_)
+    lev1 = wk.Level(n=n, g=3, level=1, dx=0.5 / N, origin=origin_new, domain_cells=(2 * N,) * 3, bc=bc, self_periodic=False,
+                    U=np.zeros((5, len(origin_new), n, n, n)))
+    b1 = amr.PatchBatch.from_level(lev1, dt_)
+    b1.regrid_fill(None, b0)
+    got = b1.download().astype(np.float64)
+    tol = 1e-6 if np_dtype == np.float32 else 1e-15
+    assert np.abs(got - ref).max() <= tol * np.abs(ref).max(), np.abs(got - ref).max()
+    # children average to their parents on the device too (conservation of the transfer)
+    h = n // 2
+    mean = got.reshape(5, len(origin_new), h, 2, h, 2, h, 2).mean(axis=(3, 5, 7))
+    Gc = wk.configs.join_patches(l0.U, l0.origin, (N, N, N))
+    for p, o in enumerate(origin_new):
+        par = Gc[:, o[2] // 2:o[2] // 2 + h, o[1] // 2:o[1] // 2 + h, o[0] // 2:o[0] // 2 + h]
+        assert np.abs(mean[:, p] - par).max() <= (2e-6 if np_dtype == np.float32 else 1e-14) * np.abs(par).max()

@@ -77,6 +77,51 @@ def test_linear_field_is_reproduced_exactly_and_uniform_stays_uniform():
         assert np.array_equal(U[2, p], np.full((n, n, n), 3.0))
 
 
+def test_new_born_patches_on_outflow_faces_never_see_the_far_side():
+    """DESIGN.md section 3 (AMR at non-periodic domain faces): beyond an OUTFLOW face the +-1 stencil of the O8
+    interpolation is the coarse ghost cell there = the nearest in-domain cell, never the cell on the far side of the
+    domain.  Outflow x faces, periodic y and z:
+      * a field linear in x: the outermost parent column of a patch on an x face gets no x slope (its one-sided
+        difference against the clamped cell is 0), the other columns are exact;
+      * changing ONLY the coarse cells on the far side of the domain leaves a patch on the x lo face bitwise unchanged
+        (and does change it when the faces are declared periodic);
+      * along periodic y the seam is in the stencil: the value across it decides the slope."""
+    n = 8
+    origin0 = wk.morton_patch_origins(4, 4, 4, n)
+    c = np.arange(32) + 0.5
+    Z, Y, X = np.meshgrid(c, c, c, indexing="ij")
+    lin = 1.0 + 0.5 * X
+    saw = np.where(Y < 1, 5.0, 1.0) + 0 * X            # along periodic y: cell 0 is 5, all others 1
+    G = np.stack([lin, 2 * lin, saw, -lin, lin + 7])
+    bc = (1, 1, 0, 0, 0, 0)
+    l0 = wk.Level(n=n, g=3, level=0, dx=1 / 32, origin=origin0, domain_cells=(32, 32, 32), bc=bc,
+                  self_periodic=False, U=wk.split_into_patches(G, n, origin0))
+    origin_new = np.array([[0, 24, 24], [56, 24, 24], [24, 0, 24]], np.int32)      # on x lo, on x hi, on the periodic y seam
+    U = rg.regrid_fill(l0, None, origin_new)
+    cf = (np.arange(64) + 0.5) / 2
+    linf = 1.0 + 0.5 * cf
+    # x lo patch: parent column 0 has slope minmod(U0 - U0, U1 - U0) = 0; columns 1..3 are exact
+    assert np.array_equal(U[0, 0, :, :, 0], U[0, 0, :, :, 1]) and np.all(U[0, 0, :, :, 0] == lin[0, 0, 0])
+    assert np.abs(U[0, 0, :, :, 2:] - linf[None, None, 2:8]).max() <= 1e-14
+    # x hi patch: parent column 31 likewise, columns 28..30 exact
+    assert np.array_equal(U[0, 1, :, :, 6], U[0, 1, :, :, 7]) and np.all(U[0, 1, :, :, 7] == lin[0, 0, 31])
+    assert np.abs(U[0, 1, :, :, :6] - linf[None, None, 56:62]).max() <= 1e-14
+    # only the far side changes: an outflow stencil must not notice, a periodic one must
+    Gc = rg._dense(l0)
+    plain = rg.prolong_patch(Gc, (0, 24, 24), n, bc)
+    wrapped = rg.prolong_patch(Gc, (0, 24, 24), n, (0,) * 6)
+    bump = Gc.copy()
+    bump[:, :, :, 31] -= 100.0                          # now below cell 0: a wrapped stencil sees a monotone profile
+    assert np.array_equal(rg.prolong_patch(bump, (0, 24, 24), n, bc), plain)
+    assert not np.array_equal(rg.prolong_patch(bump, (0, 24, 24), n, (0,) * 6), wrapped)
+    # along periodic y: cell 0 (5.0) is a strict maximum between cells 31 and 1 (both 1.0) -> no y slope ...
+    assert np.all(U[2, 2, :, 0:2, :] == 5.0) and np.all(U[2, 2, :, 2:, :] == 1.0)
+    bump = Gc.copy()
+    bump[2, :, 31, :] = 9.0                             # ... and between 9 and 1 it is monotone: slope minmod(-4, -4) = -4
+    Uy = rg.prolong_patch(bump, (24, 0, 24), n, bc)
+    assert np.all(Uy[2, :, 0, :] == 6.0) and np.all(Uy[2, :, 1, :] == 4.0)
+
+
 def test_a_local_extremum_gets_no_slope():
     """minmod: at a coarse cell that is a strict maximum along x the two children along x are equal."""
     n = 8
