@@ -595,6 +595,32 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
       }
       cur_rz = rz;
     };
+    // The sectors issue_plane(lz) is going to copy, requested into the L2 ahead of time (one request per 32-byte sector:
+    // the pair that starts it, plus every clamped / halo-buffer / first-column chunk).  The copies can only be issued
+    // once the ring slot is free (phase 2), and the copy-solve-convert chain of these warps ends phase 2 for the whole
+    // CTA: with two thirds of the plane's lines missing the L2 the copies' DRAM latency sat on that chain.  Asked for at
+    // the end of phase 1 they are L2 hits (config 5: 12.15 -> 11.61 ms, config 3 fp32: 1.672 -> 1.624 ms; from phase 2
+    // of the previous plane: slower, it lengthens the chain it is meant to shorten).
+    auto prefetch_plane = [&](int lz) {
+      const int rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
+      if (rz != cur_rz) setup_region(rz);
+      const int zt_int = (lz - (rz - 1) * n) * n2;
+      const int zt_clamp = (rz == 0 ? 0 : n - 1) * n2;
+      const int zt_halo = (lz + P.g) * M2;
+#pragma unroll
+      for (int l = 0; l < LC; ++l) {
+        if (lmask & (1u << l)) {
+          const bool fh = hmask & (1u << l);
+          const int off = goff[l] + (fh ? zt_halo : ((zmask & (1u << l)) ? zt_clamp : zt_int));
+          const float* src = (fh ? P.halo : P.Uin) + off;
+          const size_t fs = fh ? fs_halo : fs_int;
+          if ((smask & (1u << l)) || ((off & 7) == 0) || (((at + l * NA) % NPX) == 0)) {
+#pragma unroll
+            for (int q = 0; q < NF; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + q * fs));
+          }
+        }
+      }
+    };
     auto issue_plane = [&](int lz, float* dst) {
       const int rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
       if (rz != cur_rz) setup_region(rz);
@@ -700,6 +726,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
           rot_in<NF, 1>(o, wm);
         }
       }
+      if (NF == 9) prefetch_plane(kk + 2);   // MHD only: the hydro kernel (three CTAs per SM at 96 registers) loses 17 % to it
       __syncthreads();
 
       // ---- phase 2: copies of plane kk+2 into the slot plane kk-1 vacated; the tile's last x / y faces;
