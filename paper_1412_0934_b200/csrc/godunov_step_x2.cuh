@@ -557,7 +557,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
     //   goff  element offset of (source patch, z = 0, sy, sx)   hmask  source is the prolongation halo
     //   zmask the z index is clamped (outflow)                  smask  two 4-byte copies (x clamped: both
     //   from the same cell; halo buffer: odd element offset) instead of one 8-byte copy; dmask: second = +1
-    unsigned lmask = 0;
+    unsigned lmask = 0, pmask = 0;   // chunks this thread copies / chunks it prefetches for
 #pragma unroll
     for (int l = 0; l < LC; ++l) {
       const int c = at + l * NA;
@@ -565,6 +565,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
         const int ry = c / NPX, px = c - ry * NPX;
         const bool corner = (ry == 0 || ry == RH - 1) && (px == 0 || px == NPX - 1);
         if (!corner) lmask |= 1u << l;
+        if (!corner && (px <= 1 || px == NPX - 1)) pmask |= 1u << l;   // first pair of a halo / interior / halo run of a row
       }
     }
     int goff[LC];
@@ -596,8 +597,9 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
       }
       cur_rz = rz;
     };
-    // The sectors issue_plane(lz) is going to copy, requested into the L2 ahead of time (one request per 32-byte sector:
-    // the pair that starts it, plus every clamped / halo-buffer / first-column chunk).  The copies can only be issued
+    // The lines issue_plane(lz) is going to copy, requested into the L2 ahead of time (a request fetches its 128-byte line:
+    // one per run of a ring row - left halo pair, first interior pair, right halo pair - plus every clamped / halo-buffer
+    // chunk; which of its chunks a thread asks for is fixed, pmask).  The copies can only be issued
     // once the ring slot is free (phase 2), and the copy-solve-convert chain of these warps ends phase 2 for the whole
     // CTA: with two thirds of the plane's lines missing the L2 the copies' DRAM latency sat on that chain.  Asked for at
     // the end of phase 1 they are L2 hits (config 5: 12.15 -> 11.61 ms, config 3 fp32: 1.672 -> 1.624 ms; from phase 2
@@ -610,15 +612,13 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
       const int zt_halo = (lz + P.g) * M2;
 #pragma unroll
       for (int l = 0; l < LC; ++l) {
-        if (lmask & (1u << l)) {
+        if ((pmask | smask) & (1u << l)) {
           const bool fh = hmask & (1u << l);
           const int off = goff[l] + (fh ? zt_halo : ((zmask & (1u << l)) ? zt_clamp : zt_int));
           const float* src = (fh ? P.halo : P.Uin) + off;
           const size_t fs = fh ? fs_halo : fs_int;
-          if ((smask & (1u << l)) || ((off & 7) == 0) || (((at + l * NA) % NPX) == 0)) {
 #pragma unroll
-            for (int q = 0; q < NF; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + q * fs));
-          }
+          for (int q = 0; q < NF; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + q * fs));
         }
       }
     };
