@@ -557,7 +557,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
     //   goff  element offset of (source patch, z = 0, sy, sx)   hmask  source is the prolongation halo
     //   zmask the z index is clamped (outflow)                  smask  two 4-byte copies (x clamped: both
     //   from the same cell; halo buffer: odd element offset) instead of one 8-byte copy; dmask: second = +1
-    unsigned lmask = 0, pmask = 0;   // chunks this thread copies / chunks it prefetches for
+    unsigned lmask = 0;
 #pragma unroll
     for (int l = 0; l < LC; ++l) {
       const int c = at + l * NA;
@@ -565,7 +565,6 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
         const int ry = c / NPX, px = c - ry * NPX;
         const bool corner = (ry == 0 || ry == RH - 1) && (px == 0 || px == NPX - 1);
         if (!corner) lmask |= 1u << l;
-        if (!corner && (px <= 1 || px == NPX - 1)) pmask |= 1u << l;   // first pair of a halo / interior / halo run of a row
       }
     }
     int goff[LC];
@@ -597,28 +596,30 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
       }
       cur_rz = rz;
     };
-    // The lines issue_plane(lz) is going to copy, requested into the L2 ahead of time (a request fetches its 128-byte line:
-    // one per run of a ring row - left halo pair, first interior pair, right halo pair - plus every clamped / halo-buffer
-    // chunk; which of its chunks a thread asks for is fixed, pmask).  The copies can only be issued
+    // The lines issue_plane(lz) is going to copy, requested into the L2 ahead of time.  The copies can only be issued
     // once the ring slot is free (phase 2), and the copy-solve-convert chain of these warps ends phase 2 for the whole
     // CTA: with two thirds of the plane's lines missing the L2 the copies' DRAM latency sat on that chain.  Asked for at
     // the end of phase 1 they are L2 hits (config 5: 12.15 -> 11.61 ms, config 3 fp32: 1.672 -> 1.624 ms; from phase 2
-    // of the previous plane: slower, it lengthens the chain it is meant to shorten).
+    // of the previous plane: slower, it lengthens the chain it is meant to shorten).  A request fetches its 128-byte
+    // line, so one thread per (ring row, run of the row: left halo pair / interior / right halo pair) asks for the run's
+    // first pair in every field.  It is a hint: runs that come from a clamped cell (outflow) are simply not asked for.
+    const int pf_ry = at / 3, pf_run = at - 3 * pf_ry;
+    const bool pf_on = pf_ry < RH && !((pf_ry == 0 || pf_ry == RH - 1) && pf_run != 1);
     auto prefetch_plane = [&](int lz) {
-      const int rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
-      if (rz != cur_rz) setup_region(rz);
-      const int zt_int = (lz - (rz - 1) * n) * n2;
-      const int zt_clamp = (rz == 0 ? 0 : n - 1) * n2;
-      const int zt_halo = (lz + P.g) * M2;
+      if (pf_on) {
+        const int rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
+        const int lx = pf_run == 0 ? x0 - 2 : (pf_run == 1 ? x0 : x0 + TX), ly = y0 + pf_ry - 2;
+        const int gx = lx < 0 ? 0 : (lx >= n ? 2 : 1), gy = ly < 0 ? 0 : (ly >= n ? 2 : 1);
+        const int e = s_nbr[rz * 9 + gy * 3 + gx];
+        if (e >= 0 && (e >> NBR_MODE_SHIFT) == 0) {
+          const int off = (e & NBR_PATCH_MASK) * n3 + (lz - (rz - 1) * n) * n2 + (ly - (gy - 1) * n) * n + (lx - (gx - 1) * n);
+          const float* src = P.Uin + off;
 #pragma unroll
-      for (int l = 0; l < LC; ++l) {
-        if ((pmask | smask) & (1u << l)) {
-          const bool fh = hmask & (1u << l);
-          const int off = goff[l] + (fh ? zt_halo : ((zmask & (1u << l)) ? zt_clamp : zt_int));
-          const float* src = (fh ? P.halo : P.Uin) + off;
-          const size_t fs = fh ? fs_halo : fs_int;
+          for (int q = 0; q < NF; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + q * fs_int));
+        } else if (e < 0) {   // the run comes from the prolongation halo buffer (coarse-fine boundary)
+          const float* src = P.halo + (p * (M2 * M) + (lz + P.g) * M2 + (ly + P.g) * M + (lx + P.g));
 #pragma unroll
-          for (int q = 0; q < NF; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + q * fs));
+          for (int q = 0; q < NF; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + q * fs_halo));
         }
       }
     };
