@@ -623,27 +623,36 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
         }
       }
     };
+    // the common case (one 8-byte copy per component: a whole pair from a patch interior) first and on its own, the split
+    // copies of clamped / halo-buffer chunks behind a rare branch
     auto issue_plane = [&](int lz, float* dst) {
       const int rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
       if (rz != cur_rz) setup_region(rz);
       const int zt_int = (lz - (rz - 1) * n) * n2;
       const int zt_clamp = (rz == 0 ? 0 : n - 1) * n2;
-      const int zt_halo = (lz + P.g) * M2;
 #pragma unroll
       for (int l = 0; l < LC; ++l) {
-        if (lmask & (1u << l)) {
-          const bool fh = hmask & (1u << l);
-          const int off = goff[l] + (fh ? zt_halo : ((zmask & (1u << l)) ? zt_clamp : zt_int));
-          const float* src = (fh ? P.halo : P.Uin) + off;
-          const size_t fs = fh ? fs_halo : fs_int;
+        if (lmask & ~smask & (1u << l)) {
+          const int off = goff[l] + ((zmask & (1u << l)) ? zt_clamp : zt_int);
+          const float* src = P.Uin + off;
           float* d = dst + (at + l * NA) * REC;
+#pragma unroll
+          for (int q = 0; q < NF; ++q) cp_async8(d + 2 * q, src + q * fs_int);
+        }
+      }
+      if (X2_UNLIKELY(smask != 0)) {
+        const int zt_halo = (lz + P.g) * M2;
+#pragma unroll
+        for (int l = 0; l < LC; ++l) {
           if (smask & (1u << l)) {
+            const bool fh = hmask & (1u << l);
+            const int off = goff[l] + (fh ? zt_halo : ((zmask & (1u << l)) ? zt_clamp : zt_int));
+            const float* src = (fh ? P.halo : P.Uin) + off;
+            const size_t fs = fh ? fs_halo : fs_int;
+            float* d = dst + (at + l * NA) * REC;
             const int dx = (dmask >> l) & 1;
 #pragma unroll
             for (int q = 0; q < NF; ++q) { cp_async4(d + 2 * q, src + q * fs); cp_async4(d + 2 * q + 1, src + q * fs + dx); }
-          } else {
-#pragma unroll
-            for (int q = 0; q < NF; ++q) cp_async8(d + 2 * q, src + q * fs);
           }
         }
       }
