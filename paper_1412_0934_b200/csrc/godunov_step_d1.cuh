@@ -463,6 +463,27 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
       }
       cur_rz = rz;
     };
+    // the lines issue_plane(lz) is going to copy, asked for in the L2 at the end of phase 1 (see godunov_step_x2.cuh): one
+    // thread per (ring row, run of the row: left halo cells / interior / right halo cells); a hint, clamped runs skipped
+    const int pf_ry = at / 3, pf_run = at - 3 * pf_ry;
+    const bool pf_on = pf_ry < RH && !((pf_ry < 2 || pf_ry >= RH - 2) && pf_run != 1);
+    auto prefetch_plane = [&](int lz) {
+      if (pf_on) {
+        const int rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
+        const int lx = pf_run == 0 ? x0 - 2 : (pf_run == 1 ? x0 : x0 + HX), ly = y0 + pf_ry - 2;
+        const int gx = lx < 0 ? 0 : (lx >= n ? 2 : 1), gy = ly < 0 ? 0 : (ly >= n ? 2 : 1);
+        const int e = s_nbr[rz * 9 + gy * 3 + gx];
+        if (e >= 0 && (e >> NBR_MODE_SHIFT) == 0) {
+          const double* src = P.Uin + ((e & NBR_PATCH_MASK) * n3 + (lz - (rz - 1) * n) * n2 + (ly - (gy - 1) * n) * n + (lx - (gx - 1) * n));
+#pragma unroll
+          for (int q = 0; q < NF; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + q * fs_int));
+        } else if (e < 0) {
+          const double* src = P.halo + (p * (M2 * M) + (lz + P.g) * M2 + (ly + P.g) * M + (lx + P.g));
+#pragma unroll
+          for (int q = 0; q < NF; ++q) asm volatile("prefetch.global.L2 [%0];" ::"l"(src + q * fs_halo));
+        }
+      }
+    };
     auto issue_plane = [&](int lz, double* dst) {
       const int rz = lz < 0 ? 0 : (lz >= n ? 2 : 1);
       if (rz != cur_rz) setup_region(rz);
@@ -556,6 +577,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_d1_kernel(const __grid_constant__
           rot_in<NF, 1>(o, wm);
         }
       }
+      prefetch_plane(kk + 2);
       __syncthreads();
 
       // ---- phase 2: copies of plane kk+2 into the slot plane kk-1 vacated; the tile's last x / y faces;

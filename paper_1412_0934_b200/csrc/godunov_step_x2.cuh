@@ -737,7 +737,7 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
           rot_in<NF, 1>(o, wm);
         }
       }
-      if (NF == 9) prefetch_plane(kk + 2);   // MHD only: the hydro kernel (three CTAs per SM at 96 registers) loses 17 % to it
+      prefetch_plane(kk + 2);
       __syncthreads();
 
       // ---- phase 2: copies of plane kk+2 into the slot plane kk-1 vacated; the tile's last x / y faces;
