@@ -30,7 +30,7 @@
 //      state = staged W^+_z of the previous plane) are solved and the previous plane is updated, stored and
 //      its signal speed reduced.  aux: predictor of the ring pairs                          | barrier
 //   2  compute: the two x faces (left of the even cell, between the cells) and the two y faces below the
-//      pair.  aux: copies of plane k+2 (MHD: asked for in the L2 at the end of phase 1), the tile's last x / y
+//      pair.  aux: copies of plane k+2 (asked for in the L2 at the end of phase 1), the tile's last x / y
 //      faces, convert plane k+2                                                             | barrier
 //   3  compute: flux differences of this plane -> registers; falls through into 1 of the next plane
 // Every face flux is computed once per tile by one position-independent routine from bit-identical
