@@ -519,10 +519,10 @@ __global__ void __maxnreg__(MAXR) godunov_step_x2_kernel(const __grid_constant__
       if (mid) {
         float e0, e1;
         F2 xr[NF], fu[NF], fx[9], fy[9], dy[NF], dyu[NF];
-        lds_pairs<NF>(xpub, xr);     // the right neighbour's x fluxes: its lo face is the face right of this pair's odd cell
-        lds_pairs<NF>(ypub, fu);     // the upper pair's y fluxes (y solver's component order)
         ld_block(BX, fx, e0, e1);
         ld_block(BY, fy, e0, e1);
+        lds_pairs<NF>(xpub, xr);     // the right neighbour's x fluxes: its lo face is the face right of this pair's odd cell
+        lds_pairs<NF>(ypub, fu);     // the upper pair's y fluxes (y solver's component order)
 #pragma unroll
         for (int q = 0; q < NF; ++q) dy[q] = fu[q] - fy[q];
         rot_out<NF, 1>(dy, dyu);
